@@ -1,0 +1,139 @@
+/*
+ * fdham.h -- C ABI of libfdham: the batched finite-difference Kohn-Sham apply on one B200.
+ *
+ *     (H psi)_b[i] = sum_{d in x,y,z} (-1/2 / h_d^2) [ c_0 psi_b[i]
+ *                        + sum_{j=1..nn} c_j ( psi^_b(i + j e_d) + psi^_b(i - j e_d) ) ]
+ *                    + v_eff[i] psi_b[i]
+ *
+ * Operation defined by: the PAW Hamiltonian Eq. 6, first two terms "-1/2 nabla^2 + v~_KS(r)"
+ * (section III.A); the Laplacian is the "finite difference (FD) ...
+ * representation of kinetic energy operator on a uniform Cartesian grid" (section
+ * III.B.1), i.e. "applying a finite-difference stencil to a uniform grid", the first C hot spot
+ * the paper lists (section II.B).  Boundaries: zero ("potential go to zero on the
+ * cell boundaries") or periodic carrying the Bloch factor of Eq. 13
+ * (PAPER.md:225).  Bands are independent.  Stencil weights c_j are the standard
+ * central weights of order 2*nn (nn = 3: -49/18, 3/2, -3/20, 1/90, BASELINE.json); all readings
+ * taken where the paper is silent are listed in DESIGN.md.
+ *
+ * psi^ (fused halo handling): for a tap index p_d = i_d +- j outside [0, n_d)
+ *     zero-BC axis  -> 0
+ *     periodic axis -> psi[p - w n_d e_d] * exp(+2 pi i k_d w), w = +1 past the upper end, -1
+ *                      before the lower end (the array holds the full Bloch function).
+ *
+ * Conventions common to all calls
+ *   - every function returns FD_OK (0) or a negative fd_status; nothing throws, aborts,
+ *     allocates inside an apply, or synchronises the device (the *_host variant excepted);
+ *   - "device pointer" = memory of the plan's CUDA device; "host pointer" = ordinary CPU memory;
+ *   - arrays are C-contiguous, z fastest: psi/out [nbands, nx, ny, nz], v_eff [nx, ny, nz];
+ *     element = double (FD_F64) or interleaved (re, im) doubles (FD_C128); v_eff is always double;
+ *   - psi and v_eff are read-only; out is fully overwritten (no accumulate) and must not overlap
+ *     psi or v_eff;  the caller owns all three; the library owns only the plan;
+ *   - applies are enqueued on `cuda_stream` (a cudaStream_t cast to void*, NULL = legacy default
+ *     stream) and return immediately; a plan is immutable and may be used from several streams;
+ *   - there is no CPU fallback: without a usable CUDA device fd_create fails with FD_ERR_CUDA.
+ */
+#ifndef FDHAM_H
+#define FDHAM_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define FD_API __attribute__((visibility("default")))
+#else
+#define FD_API
+#endif
+
+typedef struct fd_plan fd_plan; /* opaque, owned by the library */
+
+enum { FD_BC_ZERO = 0, FD_BC_PERIODIC = 1 };
+enum { FD_F64 = 0, FD_C128 = 1 };
+enum {
+    FD_OK = 0,
+    FD_ERR_INVALID = -1,     /* NULL pointer, bad shape/h/nn/bc/dtype/nbands, misaligned pointer  */
+    FD_ERR_UNSUPPORTED = -2, /* valid request this build cannot run                               */
+    FD_ERR_ALIAS = -3,       /* out overlaps psi or v_eff                                         */
+    FD_ERR_CUDA = -4,        /* CUDA runtime failure (no device, launch error, ...)               */
+    FD_ERR_NOMEM = -5        /* host or device allocation failed                                  */
+};
+
+/* Kernel families, for fd_plan_set_kernel / fd_plan_get_kernel (diagnostics and A/B timing). */
+enum {
+    FD_KERNEL_AUTO = 0,    /* pick the fastest supported kernel for the plan (default)            */
+    FD_KERNEL_GENERIC = 1, /* one thread per grid point, any nn / shape / bc                      */
+    FD_KERNEL_SWEEP = 2    /* TMA-staged y-z tiles + register sweep along x (nn = 3 only)          */
+};
+
+/*
+ * fd_create -- build an immutable plan: stencil weights
+ * w_d[j] = -1/2 c_j / h_d^2, merged diagonal, per-axis wrap phases exp(+-2 pi i k_d), kernel and
+ * tile choice.  Host-side only apart from selecting `device`.
+ *   plan       out: receives the plan; untouched on failure
+ *   shape      host: nx, ny, nz = extents of the STORED arrays (>= 1)
+ *   h          host: grid spacings, atomic units (Bohr), finite and > 0
+ *   nn         stencil half width (order 2*nn), 1..6
+ *   bc         host: FD_BC_ZERO | FD_BC_PERIODIC per axis; a periodic axis needs n_d >= nn
+ *   k_reduced  host: Bloch vector in reduced coordinates, NULL = Gamma; must be 0 on zero-BC axes
+ *   dtype      FD_F64 (requires k = 0) or FD_C128
+ *   device     CUDA device ordinal
+ * Errors: FD_ERR_INVALID for any violated constraint above, FD_ERR_CUDA if the device cannot be
+ * used, FD_ERR_NOMEM.
+ */
+FD_API int fd_create(fd_plan **plan, const int32_t shape[3], const double h[3], int32_t nn,
+              const int32_t bc[3], const double k_reduced[3], int32_t dtype, int32_t device);
+
+/*
+ * fd_apply_kinetic -- out = T psi = -1/2 lap_FD psi  (steps a2+a3+a5+a6 of SURVEY 8(a); Eq. 6
+ * first term).
+ *   psi, out   device pointers, [nbands,nx,ny,nz] of the plan's dtype, 16-byte aligned
+ *   nbands     >= 0; 0 is a no-op returning FD_OK
+ * Errors: FD_ERR_INVALID (NULL plan/pointer, nbands < 0, misaligned), FD_ERR_ALIAS,
+ * FD_ERR_CUDA (launch failure, checked with cudaPeekAtLastError, no sync).
+ */
+FD_API int fd_apply_kinetic(const fd_plan *plan, const void *psi, void *out, int64_t nbands,
+                     void *cuda_stream);
+
+/*
+ * fd_apply_hamiltonian -- out = T psi + v_eff psi (adds step a4: the local potential of Eq. 6,
+ * one real array shared by all bands).
+ *   v_eff      device pointer, double [nx,ny,nz], 16-byte aligned
+ * Other arguments and errors as fd_apply_kinetic.
+ */
+FD_API int fd_apply_hamiltonian(const fd_plan *plan, const void *psi, const double *v_eff, void *out,
+                         int64_t nbands, void *cuda_stream);
+
+/*
+ * fd_apply_hamiltonian_host -- the same apply for HOST buffers (end-to-end path): copies psi and
+ * v_eff to the device, applies, copies H psi back, in band chunks that overlap H2D, kernel and
+ * D2H on internal streams.  v_eff may be NULL (kinetic only).  Blocks until `out` is complete.
+ * Buffers may be pageable or pinned (pinned = faster).  Allocates and frees its own staging
+ * device memory per call (FD_ERR_NOMEM if that fails).
+ */
+FD_API int fd_apply_hamiltonian_host(const fd_plan *plan, const void *psi_host, const double *v_eff_host,
+                              void *out_host, int64_t nbands);
+
+/* fd_destroy -- free the plan; NULL is a no-op.  The caller must have synchronised any stream
+ * still running an apply of this plan. */
+FD_API int fd_destroy(fd_plan *plan);
+
+/* fd_strerror -- static, thread-safe description of a status code. */
+FD_API const char *fd_strerror(int status);
+
+/* Diagnostics (not on the hot path).
+ * fd_plan_set_kernel: force a kernel family (FD_ERR_UNSUPPORTED if the plan cannot run it);
+ *   with `param` != 0 overriding the family's tile parameter (sweep: y rows per CTA).
+ * fd_plan_get_kernel: family the next apply will launch.
+ * fd_plan_launches: kernels launched by this plan so far (for bench.py's gpu_launches).
+ * fd_plan_get_weights: the 3*(nn+1) doubles w_d[j] = -1/2 c_j / h_d^2 (d-major) the kernels use. */
+FD_API int fd_plan_set_kernel(fd_plan *plan, int32_t kernel, int32_t param);
+FD_API int fd_plan_get_kernel(const fd_plan *plan);
+FD_API int64_t fd_plan_launches(const fd_plan *plan);
+FD_API int fd_plan_get_weights(const fd_plan *plan, double *w, int32_t capacity);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FDHAM_H */

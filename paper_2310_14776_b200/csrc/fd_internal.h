@@ -1,0 +1,54 @@
+// Internal declarations of libfdham (not part of the C ABI; see include/fdham.h).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#define FD_MAX_NN 6
+
+// Plan constants handed to every kernel by value.
+struct FdGeom {
+    int n[3];                    // nx, ny, nz
+    int bc[3];                   // FD_BC_*
+    int nn;
+    int cplx;                    // 0: double, 1: complex128
+    double w[3][FD_MAX_NN + 1];  // w[d][j] = -1/2 c_j / h_d^2
+    double wdiag;                // sum_d w[d][0]
+    double ph_re[3], ph_im[3];   // exp(+2 pi i k_d): factor when a tap runs past the UPPER end
+};
+
+// Launch description of the sweep kernel, fixed at plan time (tile choice) -- see fd_sweep.cu.
+struct FdSweepCfg {
+    int supported;     // 0: plan cannot use the sweep kernel
+    int ty, tc;        // thread micro tile: ty rows x tc 16-byte chunks
+    int lanes;         // threads per row group  (= chunks per row / tc, rounded up)
+    int rowgroups;     // row groups per CTA; tile rows tyc = rowgroups * ty
+    int tyc;           // y rows per CTA tile
+    int nytiles;       // ceil(ny / tyc)
+    int xchunk;        // x planes per CTA
+    int nxchunks;      // ceil(nx / xchunk)
+    int threads;       // CTA size (multiple of 32)
+    int stages;        // smem ring depth
+    int stage_bytes;   // bytes per ring stage
+    int smem_bytes;    // dynamic shared memory per CTA
+};
+
+struct fd_plan {
+    FdGeom g;
+    int device;
+    int sm_count;
+    int kernel;        // FD_KERNEL_GENERIC | FD_KERNEL_SWEEP actually used
+    FdSweepCfg sweep;
+    double h[3];
+    double k[3];
+    long long launches;  // kernels launched so far (diagnostic)
+};
+
+// fd_generic.cu
+cudaError_t fd_launch_generic(const fd_plan *plan, const void *psi, const double *v_eff, void *out,
+                              int64_t nbands, cudaStream_t stream);
+// fd_sweep.cu
+void fd_sweep_configure(fd_plan *plan, int tyc_override, int xchunk_override);
+cudaError_t fd_sweep_prepare(const fd_plan *plan);  // cudaFuncSetAttribute(max dynamic smem)
+cudaError_t fd_launch_sweep(const fd_plan *plan, const void *psi, const double *v_eff, void *out,
+                            int64_t nbands, cudaStream_t stream);

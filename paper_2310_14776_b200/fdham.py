@@ -1,0 +1,200 @@
+"""Thin Python binding of libfdham (include/fdham.h): argument marshalling only.
+
+Every step of the path (halo resolution, stencil, v_eff multiply-add, store) runs in the CUDA
+kernels behind the C ABI; torch is used for device memory and streams.  There is no CPU
+fallback: if libfdham.so is missing or no CUDA device is usable this module raises.
+
+Functions mirror the C names: fd_create, fd_apply_kinetic, fd_apply_hamiltonian,
+fd_apply_hamiltonian_host, fd_destroy (operation: Eq. 6 first two terms, with
+the FD kinetic operator of PAPER.md:232).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional, Sequence
+
+FD_BC_ZERO, FD_BC_PERIODIC = 0, 1
+FD_F64, FD_C128 = 0, 1
+FD_OK = 0
+FD_KERNEL_AUTO, FD_KERNEL_GENERIC, FD_KERNEL_SWEEP = 0, 1, 2
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libfdham.so")
+
+EXPORTED_SYMBOLS = [
+    "fd_create", "fd_apply_kinetic", "fd_apply_hamiltonian", "fd_apply_hamiltonian_host",
+    "fd_destroy", "fd_strerror", "fd_plan_set_kernel", "fd_plan_get_kernel", "fd_plan_launches",
+    "fd_plan_get_weights",
+]
+
+
+class FDError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        super().__init__(f"{where}: {strerror(status)} (fd_status {status})")
+
+
+_lib = None
+
+
+def load_library() -> ctypes.CDLL:
+    """dlopen libfdham.so (built in-tree by paper_2310_14776_b200.build). Raises if absent."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(
+            f"{LIB_PATH} is missing: build it with `python -m paper_2310_14776_b200.build` "
+            "(nvcc, sm_100a). libfdham has no CPU fallback.")
+    lib = ctypes.CDLL(LIB_PATH)
+    vp, i32, i64 = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64
+    i32p, f64p = ctypes.POINTER(ctypes.c_int32), ctypes.POINTER(ctypes.c_double)
+    lib.fd_create.argtypes = [ctypes.POINTER(vp), i32p, f64p, i32, i32p, f64p, i32, i32]
+    lib.fd_create.restype = ctypes.c_int
+    lib.fd_apply_kinetic.argtypes = [vp, vp, vp, i64, vp]
+    lib.fd_apply_kinetic.restype = ctypes.c_int
+    lib.fd_apply_hamiltonian.argtypes = [vp, vp, vp, vp, i64, vp]
+    lib.fd_apply_hamiltonian.restype = ctypes.c_int
+    lib.fd_apply_hamiltonian_host.argtypes = [vp, vp, vp, vp, i64]
+    lib.fd_apply_hamiltonian_host.restype = ctypes.c_int
+    lib.fd_destroy.argtypes = [vp]
+    lib.fd_destroy.restype = ctypes.c_int
+    lib.fd_strerror.argtypes = [ctypes.c_int]
+    lib.fd_strerror.restype = ctypes.c_char_p
+    lib.fd_plan_set_kernel.argtypes = [vp, i32, i32]
+    lib.fd_plan_set_kernel.restype = ctypes.c_int
+    lib.fd_plan_get_kernel.argtypes = [vp]
+    lib.fd_plan_get_kernel.restype = ctypes.c_int
+    lib.fd_plan_launches.argtypes = [vp]
+    lib.fd_plan_launches.restype = ctypes.c_int64
+    lib.fd_plan_get_weights.argtypes = [vp, f64p, i32]
+    lib.fd_plan_get_weights.restype = ctypes.c_int
+    _lib = lib
+    return lib
+
+
+def strerror(status: int) -> str:
+    return load_library().fd_strerror(int(status)).decode()
+
+
+def _check(status: int, where: str) -> None:
+    if status != FD_OK:
+        raise FDError(status, where)
+
+
+def fd_create(shape: Sequence[int], h: Sequence[float], nn: int = 3,
+              bc: Sequence[int] = (1, 1, 1), k: Optional[Sequence[float]] = None,
+              dtype: int = FD_F64, device: int = 0) -> ctypes.c_void_p:
+    """Returns an opaque plan handle (see include/fdham.h: fd_create)."""
+    lib = load_library()
+    plan = ctypes.c_void_p()
+    kk = (ctypes.c_double * 3)(*[float(x) for x in k]) if k is not None else None
+    rc = lib.fd_create(ctypes.byref(plan), (ctypes.c_int32 * 3)(*[int(s) for s in shape]),
+                       (ctypes.c_double * 3)(*[float(x) for x in h]), int(nn),
+                       (ctypes.c_int32 * 3)(*[int(b) for b in bc]), kk, int(dtype), int(device))
+    _check(rc, "fd_create")
+    return plan
+
+
+def fd_destroy(plan) -> None:
+    _check(load_library().fd_destroy(plan), "fd_destroy")
+
+
+def _stream_ptr(stream) -> ctypes.c_void_p:
+    if stream is None:
+        import torch
+        stream = torch.cuda.current_stream()
+    if hasattr(stream, "cuda_stream"):
+        return ctypes.c_void_p(stream.cuda_stream)
+    return ctypes.c_void_p(int(stream))
+
+
+def _dev_ptr(t) -> ctypes.c_void_p:
+    if not t.is_cuda or not t.is_contiguous():
+        raise ValueError("expected a contiguous CUDA tensor")
+    return ctypes.c_void_p(t.data_ptr())
+
+
+def fd_apply_kinetic(plan, psi, out, stream=None) -> None:
+    """out = T psi for torch CUDA tensors psi/out [nbands,nx,ny,nz] (float64 or complex128)."""
+    rc = load_library().fd_apply_kinetic(plan, _dev_ptr(psi), _dev_ptr(out), int(psi.shape[0]),
+                                         _stream_ptr(stream))
+    _check(rc, "fd_apply_kinetic")
+
+
+def fd_apply_hamiltonian(plan, psi, v_eff, out, stream=None) -> None:
+    """out = T psi + v_eff psi; v_eff is a float64 CUDA tensor [nx,ny,nz]."""
+    rc = load_library().fd_apply_hamiltonian(plan, _dev_ptr(psi), _dev_ptr(v_eff), _dev_ptr(out),
+                                             int(psi.shape[0]), _stream_ptr(stream))
+    _check(rc, "fd_apply_hamiltonian")
+
+
+def _host_ptr(a) -> ctypes.c_void_p:
+    if a is None:
+        return ctypes.c_void_p(0)
+    if hasattr(a, "data_ptr"):          # torch CPU tensor (pinned or not)
+        if a.is_cuda or not a.is_contiguous():
+            raise ValueError("expected a contiguous CPU tensor")
+        return ctypes.c_void_p(a.data_ptr())
+    if not a.flags.c_contiguous:        # numpy
+        raise ValueError("expected a C-contiguous array")
+    return ctypes.c_void_p(a.ctypes.data)
+
+
+def fd_apply_hamiltonian_host(plan, psi_host, v_eff_host, out_host) -> None:
+    """End-to-end apply on HOST arrays (numpy or torch CPU, ideally pinned); blocks until done."""
+    rc = load_library().fd_apply_hamiltonian_host(plan, _host_ptr(psi_host),
+                                                  _host_ptr(v_eff_host), _host_ptr(out_host),
+                                                  int(psi_host.shape[0]))
+    _check(rc, "fd_apply_hamiltonian_host")
+
+
+def fd_plan_set_kernel(plan, kernel: int, param: int = 0) -> None:
+    _check(load_library().fd_plan_set_kernel(plan, int(kernel), int(param)), "fd_plan_set_kernel")
+
+
+def fd_plan_get_kernel(plan) -> int:
+    return int(load_library().fd_plan_get_kernel(plan))
+
+
+def fd_plan_launches(plan) -> int:
+    return int(load_library().fd_plan_launches(plan))
+
+
+def fd_plan_get_weights(plan, nn: int):
+    buf = (ctypes.c_double * (3 * (nn + 1)))()
+    n = load_library().fd_plan_get_weights(plan, buf, 3 * (nn + 1))
+    if n < 0:
+        raise FDError(n, "fd_plan_get_weights")
+    return [[buf[d * (nn + 1) + j] for j in range(nn + 1)] for d in range(3)]
+
+
+class FDHamiltonian:
+    """Convenience owner of a plan: `H = FDHamiltonian(shape, h, ...); H.apply(psi, v_eff)`."""
+
+    def __init__(self, shape, h, nn=3, bc=(1, 1, 1), k=None, complex_=False, device=0):
+        self.shape = tuple(int(s) for s in shape)
+        self.complex = bool(complex_)
+        self.plan = fd_create(self.shape, h, nn, bc, k, FD_C128 if complex_ else FD_F64, device)
+
+    def apply(self, psi, v_eff=None, out=None, stream=None):
+        import torch
+        if out is None:
+            out = torch.empty_like(psi)
+        if v_eff is None:
+            fd_apply_kinetic(self.plan, psi, out, stream)
+        else:
+            fd_apply_hamiltonian(self.plan, psi, v_eff, out, stream)
+        return out
+
+    def close(self):
+        if self.plan is not None:
+            fd_destroy(self.plan)
+            self.plan = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

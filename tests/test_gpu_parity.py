@@ -1,0 +1,336 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on
+the same seeded inputs.  Tolerance (north_star):  max|d| <= 1e-12 (max|psi| S + max|v_eff psi|),
+S = 1/2 sum_d (|c_0| + 2 sum|c_j|)/h_d^2  (helpers.parity_tol).
+
+Full-size configs 3-5 run on the GPU in the launch configuration bench.py times (all bands, one
+apply); the oracle then checks a subset of bands in full plus sampled points from every band.
+"""
+import itertools
+
+import numpy as np
+import pytest
+
+import workloads as W
+from helpers import parity_tol, planewave, planewave_eig, kinetic_row_sum
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def fd():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2310_14776_b200 import build
+    build.build()
+    import paper_2310_14776_b200 as fd
+    fd.load_library()
+    return fd
+
+
+def gpu_apply(fd, cfg, psi, v, kernel=None, kinetic=False, tyc=0):
+    """psi, v: numpy arrays; returns numpy H psi computed by libfdham on cuda:0."""
+    plan = fd.fd_create(cfg.shape, cfg.h, cfg.nn, cfg.bc, cfg.k if cfg.complex else None,
+                        fd.FD_C128 if cfg.complex else fd.FD_F64, 0)
+    try:
+        if kernel is not None:
+            fd.fd_plan_set_kernel(plan, kernel, tyc)
+        d_psi = torch.from_numpy(psi).cuda()
+        d_out = torch.full_like(d_psi, float("nan"))
+        if kinetic or v is None:
+            fd.fd_apply_kinetic(plan, d_psi, d_out)
+        else:
+            fd.fd_apply_hamiltonian(plan, d_psi, torch.from_numpy(v).cuda(), d_out)
+        torch.cuda.synchronize()
+        used = fd.fd_plan_get_kernel(plan)
+        return d_out.cpu().numpy(), used
+    finally:
+        fd.fd_destroy(plan)
+
+
+def check(oracle, fd, cfg, psi, v, kernel=None, tyc=0):
+    got, used = gpu_apply(fd, cfg, psi, v, kernel, tyc=tyc)
+    want = oracle.apply(cfg.shape, cfg.h, cfg.nn, cfg.bc, cfg.k if cfg.complex else None, psi, v)
+    tol = parity_tol(cfg.h, cfg.nn, psi, v)
+    err = float(np.max(np.abs(got - want)))
+    assert np.isfinite(got).all()
+    assert err <= tol, f"{cfg.name} kernel={used}: max|d|={err:.3e} > tol={tol:.3e}"
+    return used
+
+
+# ------------------------------------------------------------------------------ BASELINE configs
+
+@pytest.mark.parametrize("idx", [1, 2])
+@pytest.mark.parametrize("kernel", ["auto", "generic"])
+def test_small_configs_full_compare(oracle, fd, idx, kernel):
+    cfg = W.get(idx)
+    psi, v = W.make_psi(cfg), W.make_veff(cfg)
+    used = check(oracle, fd, cfg, psi, v, None if kernel == "auto" else fd.FD_KERNEL_GENERIC)
+    if kernel == "auto":
+        assert used == fd.FD_KERNEL_SWEEP     # the bandwidth kernel is the one under test
+
+
+def _big_config_check(oracle, fd, cfg, full_bands, chunk=32, nsample=4000):
+    """All bands on the GPU in one apply; oracle on `full_bands` in full + sampled points."""
+    plan = fd.fd_create(cfg.shape, cfg.h, cfg.nn, cfg.bc, cfg.k if cfg.complex else None,
+                        fd.FD_C128 if cfg.complex else fd.FD_F64, 0)
+    try:
+        assert fd.fd_plan_get_kernel(plan) == fd.FD_KERNEL_SWEEP
+        tdt = torch.complex128 if cfg.complex else torch.float64
+        d_psi = torch.empty((cfg.nbands,) + cfg.shape, dtype=tdt, device="cuda")
+        for b0 in range(0, cfg.nbands, chunk):
+            bands = range(b0, min(cfg.nbands, b0 + chunk))
+            d_psi[b0:b0 + len(bands)] = torch.from_numpy(W.make_psi(cfg, bands)).cuda()
+        v = W.make_veff(cfg)
+        d_v = torch.from_numpy(v).cuda()
+        d_out = torch.full_like(d_psi, float("nan"))
+        fd.fd_apply_hamiltonian(plan, d_psi, d_v, d_out)
+        torch.cuda.synchronize()
+        assert bool(torch.isfinite(torch.view_as_real(d_out) if cfg.complex else d_out).all())
+        k = cfg.k if cfg.complex else None
+        # (1) full bands
+        psi_f = W.make_psi(cfg, full_bands)
+        want = oracle.apply(cfg.shape, cfg.h, cfg.nn, cfg.bc, k, psi_f, v)
+        got = d_out[list(full_bands)].cpu().numpy()
+        tol = parity_tol(cfg.h, cfg.nn, psi_f, v)
+        err = float(np.max(np.abs(got - want)))
+        assert err <= tol, f"{cfg.name}: max|d|={err:.3e} > tol={tol:.3e}"
+        # (2) sampled points of every band, biased towards faces / tile seams
+        rng = np.random.default_rng(cfg.seed)
+        per_band = max(4, nsample // cfg.nbands)
+        for b0 in range(0, cfg.nbands, chunk):
+            bands = list(range(b0, min(cfg.nbands, b0 + chunk)))
+            psi_c = W.make_psi(cfg, bands)
+            pts = []
+            for lb in range(len(bands)):
+                p = np.stack([rng.integers(0, n, per_band) for n in cfg.shape], axis=1)
+                edge = rng.integers(0, 2, size=p.shape).astype(bool)
+                lohi = np.where(rng.integers(0, 2, size=p.shape) == 0,
+                                rng.integers(0, 4, size=p.shape),
+                                np.array(cfg.shape)[None, :] - 1 - rng.integers(0, 4, size=p.shape))
+                p = np.where(edge, lohi, p)
+                pts.append(np.concatenate([np.full((per_band, 1), lb), p], axis=1))
+            pts = np.concatenate(pts).astype(np.int64)
+            want_p = oracle.points(cfg.shape, cfg.h, cfg.nn, cfg.bc, k, psi_c, v, pts)
+            idx = torch.from_numpy(pts).cuda()
+            got_p = d_out[idx[:, 0] + b0, idx[:, 1], idx[:, 2], idx[:, 3]].cpu().numpy()
+            tol = parity_tol(cfg.h, cfg.nn, psi_c, v)
+            err = float(np.max(np.abs(got_p - want_p)))
+            assert err <= tol, f"{cfg.name} bands {b0}..: sampled max|d|={err:.3e} > {tol:.3e}"
+    finally:
+        fd.fd_destroy(plan)
+
+
+def test_config3_96c_256_bands(oracle, fd):
+    _big_config_check(oracle, fd, W.get(3), [0, 1, 100, 127, 128, 254, 255, 37])
+
+
+def test_config4_bloch_c128_128_bands(oracle, fd):
+    _big_config_check(oracle, fd, W.get(4), [0, 1, 63, 64, 126, 127])
+
+
+def test_config5_slab_384_bands(oracle, fd):
+    _big_config_check(oracle, fd, W.get(5), [0, 191, 383], nsample=3000)
+
+
+# ------------------------------------------------------------------------------ shape sweep (M8)
+
+SWEEP_SHAPES = [(8, 8, 8), (9, 8, 10), (8, 17, 12), (33, 10, 8), (12, 50, 14), (16, 16, 16),
+                (10, 37, 24), (40, 8, 96)]
+
+
+@pytest.mark.parametrize("shape", SWEEP_SHAPES)
+def test_shape_sweep_all_bc_combinations_real(oracle, fd, shape):
+    for bc in itertools.product((0, 1), repeat=3):
+        cfg = W.custom(shape, (0.2, 0.23, 0.17), bc, nbands=3)
+        check(oracle, fd, cfg, W.make_psi(cfg), W.make_veff(cfg))
+
+
+@pytest.mark.parametrize("shape", [(8, 8, 8), (9, 12, 10), (8, 23, 12), (20, 10, 36)])
+def test_shape_sweep_complex_bloch(oracle, fd, shape):
+    for bc in [(1, 1, 1), (1, 0, 1), (0, 1, 1), (1, 1, 0), (0, 0, 0)]:
+        k = tuple(kk if b else 0.0 for kk, b in zip((0.25, 0.125, -0.3), bc))
+        cfg = W.custom(shape, (0.2, 0.23, 0.17), bc, k=k, complex_=True, nbands=3)
+        check(oracle, fd, cfg, W.make_psi(cfg), W.make_veff(cfg))
+
+
+@pytest.mark.parametrize("shape", [(3, 4, 5), (7, 7, 7), (6, 6, 6), (5, 9, 11), (3, 3, 3)])
+def test_generic_fallback_shapes(oracle, fd, shape):
+    """odd nz / tiny axes / n = nn / n = 2nn (double hit) run on the generic kernel."""
+    for bc in [(1, 1, 1), (0, 1, 0), (0, 0, 0)]:
+        cfg = W.custom(shape, (0.2, 0.23, 0.17), bc, nbands=2)
+        used = check(oracle, fd, cfg, W.make_psi(cfg), W.make_veff(cfg))
+        assert used == fd.FD_KERNEL_GENERIC
+        ck = W.custom(shape, (0.2, 0.23, 0.17), bc, complex_=True, nbands=2,
+                      k=tuple(0.3 * b for b in bc))
+        check(oracle, fd, ck, W.make_psi(ck), W.make_veff(ck))
+
+
+@pytest.mark.parametrize("nn", [1, 2, 4, 5, 6])
+def test_other_stencil_orders(oracle, fd, nn):
+    cfg = W.custom((12, 10, 14), (0.2, 0.23, 0.17), (1, 0, 1), nbands=2, nn=nn)
+    check(oracle, fd, cfg, W.make_psi(cfg), W.make_veff(cfg))
+
+
+@pytest.mark.parametrize("tyc", [4, 8, 12, 20])
+def test_tile_rows_override_ragged_tiles(oracle, fd, tyc):
+    """Several y tiles, ragged last tile, tile seams at different rows."""
+    for bc in [(1, 1, 1), (0, 0, 0), (1, 0, 1)]:
+        cfg = W.custom((10, 30, 16), (0.2, 0.23, 0.17), bc, nbands=5)
+        used = check(oracle, fd, cfg, W.make_psi(cfg), W.make_veff(cfg), fd.FD_KERNEL_SWEEP, tyc)
+        assert used == fd.FD_KERNEL_SWEEP
+    ck = W.custom((10, 30, 16), (0.2, 0.23, 0.17), (1, 1, 1), k=(0.25, 0.125, 0.4),
+                  complex_=True, nbands=3)
+    check(oracle, fd, ck, W.make_psi(ck), W.make_veff(ck), fd.FD_KERNEL_SWEEP, tyc)
+
+
+# ------------------------------------------------------------------------------ metamorphic (M1-M7)
+
+def test_band_independence_and_counts(oracle, fd):
+    cfg = W.custom((16, 24, 32), (0.2, 0.2, 0.2), (1, 1, 1), nbands=13)
+    psi, v = W.make_psi(cfg), W.make_veff(cfg)
+    full, _ = gpu_apply(fd, cfg, psi, v)
+    for sel in ([0], [12], [3, 4], [5, 1, 7, 2, 11]):
+        part, _ = gpu_apply(fd, cfg.with_bands(len(sel)), np.ascontiguousarray(psi[sel]), v)
+        assert np.max(np.abs(part - full[sel])) <= parity_tol(cfg.h, 3, psi, v)
+    for nb in (1, 2, 7, 149, 300):           # more / fewer bands than SMs, primes
+        c2 = cfg.with_bands(nb)
+        check(oracle, fd, c2, W.make_psi(c2), v)
+
+
+def test_kinetic_equals_hamiltonian_with_zero_v_and_linearity(oracle, fd):
+    cfg = W.custom((12, 16, 20), (0.2, 0.21, 0.19), (1, 0, 1), nbands=4)
+    psi, v1 = W.make_psi(cfg), W.make_veff(cfg)
+    v2 = np.random.default_rng(4).uniform(-2, 2, cfg.shape)
+    t, _ = gpu_apply(fd, cfg, psi, None, kinetic=True)
+    h0, _ = gpu_apply(fd, cfg, psi, np.zeros(cfg.shape))
+    assert np.max(np.abs(t - h0)) <= 1e-13 * kinetic_row_sum(cfg.h) * np.abs(psi).max()
+    ha, _ = gpu_apply(fd, cfg, psi, v1 + v2)
+    hb, _ = gpu_apply(fd, cfg, psi, v1)
+    assert np.max(np.abs((ha - hb) - v2[None] * psi)) <= parity_tol(cfg.h, 3, psi, v1 + v2)
+    want = oracle.apply(cfg.shape, cfg.h, 3, cfg.bc, None, psi)
+    assert np.max(np.abs(t - want)) <= parity_tol(cfg.h, 3, psi, None)
+
+
+def test_complex_gamma_equals_two_real_applies(fd):
+    shape, h, bc = (12, 16, 20), (0.2, 0.21, 0.19), (1, 0, 1)
+    cr = W.custom(shape, h, bc, nbands=2)
+    re, im = W.make_psi(cr), W.make_psi(W.custom(shape, h, bc, nbands=2, index=98))
+    v = W.make_veff(cr)
+    cc = W.custom(shape, h, bc, complex_=True, nbands=2)
+    c, _ = gpu_apply(fd, cc, re + 1j * im, v)
+    r, _ = gpu_apply(fd, cr, re, v)
+    i, _ = gpu_apply(fd, cr, im, v)
+    assert np.max(np.abs(c - (r + 1j * i))) <= parity_tol(h, 3, re + 1j * im, v)
+
+
+def test_translation_invariance_across_tile_seams(fd):
+    cfg = W.custom((16, 40, 24), (0.2, 0.2, 0.2), (1, 1, 1), nbands=2)
+    psi = W.make_psi(cfg)
+    base, _ = gpu_apply(fd, cfg, psi, None, fd.FD_KERNEL_SWEEP, kinetic=True, tyc=12)
+    tol = parity_tol(cfg.h, 3, psi, None)
+    for shift, ax in [(1, 1), (5, 1), (11, 2), (13, 2), (3, 3), (23, 3)]:
+        got, _ = gpu_apply(fd, cfg, np.ascontiguousarray(np.roll(psi, shift, axis=ax)), None,
+                           fd.FD_KERNEL_SWEEP, kinetic=True, tyc=12)
+        assert np.max(np.abs(got - np.roll(base, shift, axis=ax))) <= tol
+
+
+def test_axis_permutation(fd):
+    shape, h, bc = (10, 12, 16), (0.2, 0.25, 0.3), (1, 0, 1)
+    cfg = W.custom(shape, h, bc, nbands=2)
+    psi, v = W.make_psi(cfg), W.make_veff(cfg)
+    base, _ = gpu_apply(fd, cfg, psi, v)
+    for perm in [(1, 2, 0), (2, 0, 1), (0, 2, 1)]:
+        cp = W.custom([shape[p] for p in perm], [h[p] for p in perm], [bc[p] for p in perm],
+                      nbands=2)
+        pp = np.ascontiguousarray(psi.transpose((0,) + tuple(1 + p for p in perm)))
+        vp = np.ascontiguousarray(v.transpose(perm))
+        got, _ = gpu_apply(fd, cp, pp, vp)
+        want = base.transpose((0,) + tuple(1 + p for p in perm))
+        assert np.max(np.abs(got - want)) <= parity_tol(h, 3, psi, v)
+
+
+def test_plane_waves_on_device_closed_form(fd):
+    """GPU against the closed form directly (not via the oracle): Gamma and Bloch."""
+    n, h_ang = (24, 16, 32), (0.2, 0.21, 0.18)
+    for k, m in [((0, 0, 0), (1, 2, 3)), ((0.25, 0.125, 0.0), (3, -2, 1)),
+                 ((0.25, 0.125, -0.4), (0, 0, 0))]:
+        cfg = W.custom(n, h_ang, (1, 1, 1), k=k, complex_=True, nbands=1)
+        psi = planewave(n, k, m)[None]
+        got, used = gpu_apply(fd, cfg, psi, None, kinetic=True)
+        assert used == fd.FD_KERNEL_SWEEP
+        lam = planewave_eig(n, cfg.h, k, m)
+        assert np.max(np.abs(got - lam * psi)) <= 1e-12 * kinetic_row_sum(cfg.h)
+
+
+# ------------------------------------------------------------------------------ ABI behaviour on device
+
+def test_alias_and_alignment_errors(fd):
+    plan = fd.fd_create((8, 8, 8), (0.4,) * 3)
+    try:
+        x = torch.zeros((2, 8, 8, 8), dtype=torch.float64, device="cuda")
+        v = torch.zeros((8, 8, 8), dtype=torch.float64, device="cuda")
+        with pytest.raises(fd.FDError) as ei:
+            fd.fd_apply_kinetic(plan, x, x)
+        assert ei.value.status == -3
+        ov = x[1].view(8, 8, 8)                             # v_eff inside out
+        y = torch.zeros_like(x)
+        with pytest.raises(fd.FDError) as ei:
+            fd.fd_apply_hamiltonian(plan, y, ov, x)
+        assert ei.value.status == -3
+        big = torch.zeros(2 * 512 + 1, dtype=torch.float64, device="cuda")
+        mis = big[1:].view(2, 8, 8, 8)                      # 8-byte aligned only
+        with pytest.raises(fd.FDError) as ei:
+            fd.fd_apply_kinetic(plan, mis, x)
+        assert ei.value.status == -1
+        lib = fd.load_library()
+        assert lib.fd_apply_kinetic(plan, None, None, 0, None) == 0   # nbands == 0: no-op
+        assert lib.fd_apply_kinetic(plan, None, None, -1, None) == -1
+    finally:
+        fd.fd_destroy(plan)
+
+
+def test_async_on_a_side_stream(oracle, fd):
+    cfg = W.custom((16, 16, 16), (0.2,) * 3, (1, 1, 1), nbands=4)
+    psi, v = W.make_psi(cfg), W.make_veff(cfg)
+    plan = fd.fd_create(cfg.shape, cfg.h, 3, cfg.bc)
+    try:
+        s = torch.cuda.Stream()
+        d_psi, d_v = torch.from_numpy(psi).cuda(), torch.from_numpy(v).cuda()
+        d_out = torch.empty_like(d_psi)
+        torch.cuda.synchronize()
+        with torch.cuda.stream(s):
+            fd.fd_apply_hamiltonian(plan, d_psi, d_v, d_out)       # picks the current stream
+        fd.fd_apply_hamiltonian(plan, d_psi, d_v, torch.empty_like(d_psi), stream=s)
+        s.synchronize()
+        want = oracle.apply(cfg.shape, cfg.h, 3, cfg.bc, None, psi, v)
+        assert np.max(np.abs(d_out.cpu().numpy() - want)) <= parity_tol(cfg.h, 3, psi, v)
+        assert fd.fd_plan_launches(plan) == 2
+    finally:
+        fd.fd_destroy(plan)
+
+
+def test_host_buffer_apply(oracle, fd):
+    """fd_apply_hamiltonian_host: several chunks, pinned and pageable, real and complex."""
+    for cplx in (False, True):
+        cfg = W.custom((40, 48, 64), (0.2,) * 3, (1, 1, 0), complex_=cplx, nbands=150,
+                       k=(0.25, 0.125, 0.0) if cplx else (0, 0, 0))
+        psi, v = W.make_psi(cfg), W.make_veff(cfg)
+        plan = fd.fd_create(cfg.shape, cfg.h, 3, cfg.bc, cfg.k if cplx else None,
+                            fd.FD_C128 if cplx else fd.FD_F64)
+        try:
+            out = np.empty_like(psi)
+            fd.fd_apply_hamiltonian_host(plan, psi, v, out)          # pageable numpy
+            want = oracle.apply(cfg.shape, cfg.h, 3, cfg.bc, cfg.k if cplx else None, psi, v)
+            tol = parity_tol(cfg.h, 3, psi, v)
+            assert np.max(np.abs(out - want)) <= tol
+            p_psi = torch.from_numpy(psi).pin_memory()
+            p_out = torch.empty_like(p_psi).pin_memory()
+            fd.fd_apply_hamiltonian_host(plan, p_psi, torch.from_numpy(v).pin_memory(), p_out)
+            assert np.max(np.abs(p_out.numpy() - want)) <= tol
+            fd.fd_apply_hamiltonian_host(plan, p_psi, None, p_out)   # kinetic only
+            want_t = oracle.apply(cfg.shape, cfg.h, 3, cfg.bc, cfg.k if cplx else None, psi)
+            assert np.max(np.abs(p_out.numpy() - want_t)) <= tol
+        finally:
+            fd.fd_destroy(plan)
