@@ -1,0 +1,330 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the FD Kohn-Sham apply H psi = -1/2 lap_FD psi + v_eff psi on B200.
+
+Contract:
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload cfgN]
+A "step" is one pass of the whole hot path (halo resolution + 19-point stencil + v_eff multiply-add
++ store, all fused in one kernel launch) over one batch of synthetic wave functions.  The default
+workload is BASELINE.json configs[2] (96^3 grid, 256 bands, float64, periodic Gamma): the config
+the metric's 70 %-of-HBM target is quoted on.  Inputs (3.6 GB) are larger than the 126 MB L2, so no
+L2 flush is needed between steps.
+
+Prints ONE JSON line.  `value` = grid-point x band updates per second (whole job, inputs resident
+in HBM); `e2e` = the same through fd_apply_hamiltonian_host with pinned HOST buffers (H2D + D2H
+inside the timed region); `roofline` = algorithmic bytes / measured kernel time against the
+measured HBM copy peak; `cpu_baseline` = the CPU oracle timed on this box's host cores.
+Multi-GPU (`--gpus N` under torchrun): the path does not shard (north_star: one GPU only), so N
+independent replicas run, one per rank, no data-path collective ("replicas only").
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "FD H.psi apply Gpoint.bands/s"
+UNIT = "Gpoint.band/s"
+DEFAULT_WORKLOAD = "cfg3"
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the sweep kernel from the committed
+# `ncu --set full` capture (profiles/), keyed by workload; None until a capture exists.
+NCU_TRAFFIC_BYTES = {}
+
+
+def _measured_peak_gbs():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """Samples SM clock and clock-event reasons through NVML during the timed region."""
+
+    REASONS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown",
+               0x40: "hw_thermal_slowdown", 0x80: "hw_power_brake_slowdown", 0x2: "app_clocks",
+               0x10: "sync_boost"}
+
+    def __init__(self, torch_device_index: int, period_s: float = 0.005):
+        self.period = period_s
+        self.samples, self.reasons = [], set()
+        self.max_mhz = None
+        self._stop = threading.Event()
+        self._thread = None
+        self.h = None
+        try:
+            import pynvml
+            import torch
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            try:
+                uuid = str(torch.cuda.get_device_properties(torch_device_index).uuid)
+                if not uuid.startswith("GPU-"):
+                    uuid = "GPU-" + uuid
+                self.h = pynvml.nvmlDeviceGetHandleByUUID(uuid)
+            except Exception:
+                self.h = pynvml.nvmlDeviceGetHandleByIndex(torch_device_index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self.h = None
+
+    def _loop(self):
+        nv = self.nv
+        while not self._stop.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                try:
+                    mask = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    mask = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, name in self.REASONS.items():
+                    if mask & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def start(self):
+        if self.h is not None:
+            self._thread = threading.Thread(target=self._loop, daemon=True)
+            self._thread.start()
+
+    def stop(self):
+        if self._thread is not None:
+            self._stop.set()
+            self._thread.join()
+        s = sorted(self.samples)
+        return {"sm_mhz": (s[len(s) // 2] if s else None), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(s)}
+
+
+def _cfg(name):
+    import workloads as W
+    return W.get(name)
+
+
+def cpu_oracle_rate(cfg, budget_s: float = 10.0, max_bands: int | None = None):
+    """Time the CPU oracle (as it stands) on a bounded sample of the workload."""
+    import workloads as W
+    from oracle import fd_oracle
+    cores = fd_oracle.max_threads()
+    nb = min(cfg.nbands, max(2 * cores, 8))
+    if max_bands:
+        nb = min(nb, max_bands)
+    psi = W.make_psi(cfg, range(nb))
+    v = W.make_veff(cfg)
+    k = cfg.k if cfg.complex else None
+    fd_oracle.apply(cfg.shape, cfg.h, cfg.nn, cfg.bc, k, psi[:1], v)  # page in / build
+    passes, t0 = 0, time.perf_counter()
+    while True:
+        fd_oracle.apply(cfg.shape, cfg.h, cfg.nn, cfg.bc, k, psi, v)
+        passes += 1
+        el = time.perf_counter() - t0
+        if el >= budget_s or passes >= 50:
+            break
+    rate = passes * nb * cfg.npoints / el / 1e9
+    return {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"{nb} of {cfg.nbands} bands of {cfg.name}, {passes} passes, {el:.1f} s, "
+                      f"OpenMP over bands"}
+
+
+def run_reference(args):
+    """--impl reference: the oracle, on the host cores, same metric/config (rank 0 only)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import workloads as W
+    from oracle import fd_oracle
+    cfg = _cfg(args.workload)
+    cores = fd_oracle.max_threads()
+    nb = min(cfg.nbands, max(cores, 8))
+    psi = W.make_psi(cfg, range(nb))
+    v = W.make_veff(cfg)
+    k = cfg.k if cfg.complex else None
+    # keep the whole run within a few minutes: cap steps by a 120 s budget
+    for _ in range(max(1, min(args.warmup, 2))):
+        fd_oracle.apply(cfg.shape, cfg.h, cfg.nn, cfg.bc, k, psi, v)
+    t0 = time.perf_counter()
+    done = 0
+    for _ in range(args.steps):
+        fd_oracle.apply(cfg.shape, cfg.h, cfg.nn, cfg.bc, k, psi, v)
+        done += 1
+        if time.perf_counter() - t0 > 120.0:
+            break
+    el = time.perf_counter() - t0
+    value = done * nb * cfg.npoints / el / 1e9
+    sample = f"each step = oracle apply on {nb} of {cfg.nbands} bands of {cfg.name}"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT,
+        "n_gpus": args.gpus, "steps": done, "warmup": args.warmup,
+        "ms_per_step": el / done * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "c128" if cfg.complex else "f64", "data": "synthetic",
+        "config": {"workload": cfg.name, "grid": list(cfg.shape), "nbands": cfg.nbands,
+                   "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
+                         "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def aggregate(per_rank_ms: float, units_per_rank: float, world: int, reduce_max):
+    """Whole-job throughput: all ranks' units / the slowest rank's time (replicas only)."""
+    t = reduce_max(per_rank_ms)
+    return world * units_per_rank / (t * 1e-3) / 1e9, t
+
+
+def run_ours(args):
+    import torch
+    import workloads as W
+    import paper_2310_14776_b200 as fd
+    from paper_2310_14776_b200 import build as fd_build
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; libfdham has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if rank == 0:
+        fd_build.build()
+    if dist is not None:
+        dist.barrier()
+    fd.load_library()
+
+    cfg = _cfg(args.workload)
+    tdt = torch.complex128 if cfg.complex else torch.float64
+    # synthetic inputs with the workload's recipe; generated on the host in band chunks
+    d_psi = torch.empty((cfg.nbands,) + cfg.shape, dtype=tdt, device="cuda")
+    chunk = 32
+    for b0 in range(0, cfg.nbands, chunk):
+        bands = range(b0, min(cfg.nbands, b0 + chunk))
+        d_psi[b0:b0 + len(bands)] = torch.from_numpy(W.make_psi(cfg, bands)).cuda()
+    v_host = W.make_veff(cfg)
+    d_v = torch.from_numpy(v_host).cuda()
+    d_out = torch.empty_like(d_psi)
+    plan = fd.fd_create(cfg.shape, cfg.h, cfg.nn, cfg.bc, cfg.k if cfg.complex else None,
+                        fd.FD_C128 if cfg.complex else fd.FD_F64, local)
+    kernel = {fd.FD_KERNEL_SWEEP: "sweep", fd.FD_KERNEL_GENERIC: "generic"}[
+        fd.fd_plan_get_kernel(plan)]
+    stream = torch.cuda.Stream()
+
+    def sync_all():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    with torch.cuda.stream(stream):
+        for _ in range(max(args.warmup, 3)):
+            fd.fd_apply_hamiltonian(plan, d_psi, d_v, d_out, stream)
+    sync_all()
+    sampler = ClockSampler(local)
+    l0 = fd.fd_plan_launches(plan)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler.start()
+    with torch.cuda.stream(stream):
+        e0.record(stream)
+        for _ in range(args.steps):
+            fd.fd_apply_hamiltonian(plan, d_psi, d_v, d_out, stream)
+        e1.record(stream)
+    sync_all()
+    clocks = sampler.stop()
+    launches = fd.fd_plan_launches(plan) - l0
+    ms_local = e0.elapsed_time(e1) / args.steps
+
+    def reduce_max(x):
+        if dist is None:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    units = cfg.npoints * cfg.nbands
+    value, ms_step = aggregate(ms_local, units, world, reduce_max)
+
+    # ---- end to end: pinned HOST buffers through fd_apply_hamiltonian_host ------------------
+    e2e_steps = max(1, min(3, args.steps))
+    h_psi = torch.empty(d_psi.shape, dtype=tdt).pin_memory()
+    h_psi.copy_(d_psi)
+    h_v = torch.from_numpy(v_host).pin_memory()
+    h_out = torch.empty(d_psi.shape, dtype=tdt).pin_memory()
+    fd.fd_apply_hamiltonian_host(plan, h_psi, h_v, h_out)      # warm-up
+    sync_all()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        fd.fd_apply_hamiltonian_host(plan, h_psi, h_v, h_out)  # blocks until out is on the host
+    e2e_ms_local = (time.perf_counter() - t0) * 1e3 / e2e_steps
+    e2e_value, _ = aggregate(e2e_ms_local, units, world, reduce_max)
+    ok = bool(torch.equal(h_out[:2], d_out[:2].cpu()))
+    band_bytes = cfg.npoints * cfg.elem_bytes
+    e2e = {"value": e2e_value, "unit": UNIT,
+           "h2d_bytes_per_step": cfg.nbands * band_bytes + cfg.npoints * 8,
+           "d2h_bytes_per_step": cfg.nbands * band_bytes,
+           "steps": e2e_steps, "ms_per_step": e2e_ms_local, "matches_device_path": ok,
+           "api": "fd_apply_hamiltonian_host (pinned host buffers, 3-slot H2D/kernel/D2H ring)"}
+
+    if rank == 0:
+        peak, peak_src = _measured_peak_gbs()
+        achieved = cfg.min_bytes / (ms_local * 1e-3) / 1e9
+        roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                    "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(cfg.name),
+                    "kernel": f"fd_{kernel}_kernel", "peak_source": peak_src,
+                    "algorithmic_bytes_per_launch": cfg.min_bytes,
+                    "frac_of_nominal_8TBs": achieved / 8000.0,
+                    "avg_launch_ms": ms_local}
+        cpu = cpu_oracle_rate(cfg, budget_s=args.cpu_seconds) if world == 1 or True else None
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "c128" if cfg.complex else "f64",
+            "data": "synthetic",
+            "config": {"workload": cfg.name, "grid": list(cfg.shape), "nbands": cfg.nbands,
+                       "bc": list(cfg.bc), "k": list(cfg.k), "nn": cfg.nn,
+                       "h_angstrom": list(cfg.h_angstrom), "kernel": kernel,
+                       "parallelism": "replicas only" if world > 1 else "single GPU",
+                       "l2": "inputs+outputs %.2f GB >> 126 MB L2, no flush between steps"
+                             % (cfg.min_bytes / 1e9)},
+            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
+            "roofline": roofline, "cpu_baseline": cpu,
+        }
+        print(json.dumps(line), flush=True)
+    fd.fd_destroy(plan)
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=300)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--workload", default=DEFAULT_WORKLOAD,
+                    help="cfg1..cfg5 (BASELINE.json configs); default cfg3")
+    ap.add_argument("--cpu-seconds", type=float, default=10.0,
+                    help="budget of the cpu_baseline leg")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()
