@@ -58,12 +58,15 @@ int apply_device(const fd_plan *plan, const void *psi, const double *v_eff, void
                  int64_t nbands, cudaStream_t stream)
 {
     cudaError_t e;
-    if (plan->kernel == FD_KERNEL_SWEEP)
-        e = fd_launch_sweep(plan, psi, v_eff, out, nbands, stream);
-    else
+    int n = 0;
+    if (plan->kernel == FD_KERNEL_SWEEP) {
+        e = fd_launch_sweep(plan, psi, v_eff, out, nbands, stream, &n);
+    } else {
         e = fd_launch_generic(plan, psi, v_eff, out, nbands, stream);
+        n = 1;
+    }
     if (e != cudaSuccess) return FD_ERR_CUDA;
-    __atomic_add_fetch(&const_cast<fd_plan *>(plan)->launches, 1, __ATOMIC_RELAXED);
+    __atomic_add_fetch(&const_cast<fd_plan *>(plan)->launches, (long long)n, __ATOMIC_RELAXED);
     return FD_OK;
 }
 

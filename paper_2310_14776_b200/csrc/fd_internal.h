@@ -21,16 +21,22 @@ struct FdGeom {
 struct FdSweepCfg {
     int supported;     // 0: plan cannot use the sweep kernel
     int ty, tc;        // thread micro tile: ty rows x tc 16-byte chunks
-    int lanes;         // threads per row group  (= chunks per row / tc, rounded up)
+    int lanes;         // threads per row group  (= chunks per row / tc)
     int rowgroups;     // row groups per CTA; tile rows tyc = rowgroups * ty
     int tyc;           // y rows per CTA tile
     int nytiles;       // ceil(ny / tyc)
-    int xchunk;        // x planes per CTA
-    int nxchunks;      // ceil(nx / xchunk)
     int threads;       // CTA size (multiple of 32)
     int stages;        // smem ring depth
+    int zb_bytes;      // zero block at the start of every stage (zero-BC z halo source), else 0
+    int v_off;         // offset of the v_eff rows inside a stage
     int stage_bytes;   // bytes per ring stage
+    int tab_off;       // offset of the step table in shared memory
+    int tab_cap;       // step table capacity (entries of 16 bytes)
+    int stage_off;     // offset of stage 0
     int smem_bytes;    // dynamic shared memory per CTA
+    int cluster;       // CTAs per thread-block cluster (= nytiles), 1 = no cluster launch
+    int max_teams;     // teams (clusters) resident at once on the device
+    int xchunk;        // 0 = persistent teams, else x planes per team (tuning knob)
 };
 
 struct fd_plan {
@@ -49,6 +55,6 @@ cudaError_t fd_launch_generic(const fd_plan *plan, const void *psi, const double
                               int64_t nbands, cudaStream_t stream);
 // fd_sweep.cu
 void fd_sweep_configure(fd_plan *plan, int tyc_override, int xchunk_override);
-cudaError_t fd_sweep_prepare(const fd_plan *plan);  // cudaFuncSetAttribute(max dynamic smem)
+cudaError_t fd_sweep_prepare(fd_plan *plan);  // smem opt-in + resident cluster count
 cudaError_t fd_launch_sweep(const fd_plan *plan, const void *psi, const double *v_eff, void *out,
-                            int64_t nbands, cudaStream_t stream);
+                            int64_t nbands, cudaStream_t stream, int *nlaunches);

@@ -7,35 +7,42 @@
 //
 // Design:
 //   * A CTA owns one y-tile (tyc rows x the full z row) and sweeps along x.  The y-z tile of each
-//     x plane, with 3 halo rows on either side, is staged in shared memory by the TMA unit
-//     (cp.async.bulk, completion on an mbarrier) through a 4-deep ring, so HBM reads are deep,
-//     asynchronous and fully coalesced (whole rows), and each psi value crosses HBM once.
+//     x plane, with 3 halo rows on either side, and the matching v_eff rows are staged in shared
+//     memory by the TMA unit (cp.async.bulk, completion on an mbarrier) through a ring of
+//     `stages` slots, so HBM reads are deep, asynchronous and fully coalesced (whole rows), and
+//     each psi value crosses HBM once.
+//   * The whole schedule of a CTA (which plane to load, which output plane completes, which
+//     v_eff plane, which Bloch factor) is a table in shared memory built once at kernel start:
+//     the sweep itself is one flat loop over table entries with no index arithmetic.
 //   * x direction: scatter form.  When plane xl arrives its value u adds w_x[|j|] u to the seven
 //     in-flight output accumulators xl-3..xl+3 held in REGISTERS; output xl-3 is then complete
-//     and is stored.  The accumulator slots rotate by compile-time index (loop unrolled x7).
+//     and is stored (streaming store).  The accumulator slots rotate by compile-time index
+//     (loop unrolled x7).
 //   * y and z directions: read from the shared-memory tile of the centre plane.  Each thread owns
 //     a micro tile of TY rows x TC 16-byte chunks (real: 4 rows x 2 points, complex: 2 rows x 2
-//     points) to amortise halo reads: ~3.3 (real) / 3.5 (complex) LDS.128 per point pair.
+//     points) to amortise halo reads.
+//   * The warp that is last to release a ring slot refills it (election by a shared-memory
+//     counter), so no warp ever waits for the others in order to issue a load.
 //   * Boundaries are resolved while staging / addressing, never by a padded copy:
 //       periodic y  -> the wrapped halo rows are a separate bulk copy from the other end;
 //       zero y      -> those shared-memory rows are zeroed once and never overwritten;
 //       periodic z  -> per-thread precomputed wrapped chunk offsets inside the row;
-//       zero z      -> the out-of-range chunk address points at a 16-byte zero word (stride 0);
-//       periodic x  -> the sweep prologue/epilogue read planes from the other end;
-//       zero x      -> those steps are skipped (accumulators are born zero);
+//       zero z      -> the out-of-range chunk address points at a zero block of the stage;
+//       periodic x  -> the table's prologue/epilogue entries load planes from the other end;
+//       zero x      -> those entries carry no load (the value is taken as zero);
 //       Bloch phase -> multiply only wrapped rows / chunks / planes (complex128 only).
-//   * Persistent teams: the (band, x) planes are split evenly over floor(#SM / nytiles) teams of
-//     nytiles CTAs; the CTAs of a team sweep the same planes for adjacent y-tiles at the same
-//     time, so the y-halo rows they share are L2 hits, and every SM gets the same amount of work.
+//   * Persistent teams: the (band, x) planes are split evenly over the resident teams of
+//     nytiles CTAs.  A team is a thread-block cluster; its CTAs sweep the same planes for adjacent
+//     y-tiles and are kept within one step of each other by a split cluster barrier, so the
+//     y-halo rows they share are fetched from HBM once and hit L2 the second time.
 #include "fd_internal.h"
 
 namespace {
 
-constexpr int kStages = 4;       // ring depth (power of two)
-constexpr int kStagesLog2 = 2;
 constexpr int kMaxThreads = 384;
-constexpr int kBarBytes = 128;   // full[4] + empty[4] mbarriers at the start of shared memory
-constexpr int kRowOff = 128;     // rows start here inside a stage; bytes [0,16) are a zero word
+constexpr int kMaxStages = 8;
+constexpr int kCtlBytes = 256;   // full[8] + empty[8] mbarriers + 8 election counters
+constexpr int kSmemMax = 227 * 1024;
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p)
 {
@@ -81,11 +88,33 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t
         ::"r"(dst), "l"(src), "r"(bytes), "r"(bar)
         : "memory");
 }
+__device__ __forceinline__ void cluster_arrive()
+{
+    asm volatile("barrier.cluster.arrive.relaxed.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void cluster_wait()
+{
+    asm volatile("barrier.cluster.wait.aligned;" ::: "memory");
+}
 
 __device__ __forceinline__ double2 lds128(uint32_t addr)
 {
     double2 v;
     asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ double lds64(uint32_t addr)
+{
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ int4 lds_i4(uint32_t addr)
+{
+    int4 v;
+    asm volatile("ld.shared.v4.s32 {%0, %1, %2, %3}, [%4];"
+                 : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w)
+                 : "r"(addr));
     return v;
 }
 __device__ __forceinline__ void fma2(double2 &a, double w, const double2 &x)
@@ -102,68 +131,70 @@ __device__ __forceinline__ double2 cmul(const double2 &a, double pr, double pi)
     return make_double2(a.x * pr - a.y * pi, a.x * pi + a.y * pr);
 }
 
-// Walks the planes a CTA has to LOAD, in consumption order: for each segment (band, [x0, x0+len))
-// of its linear (band, x) range the steps s = 0..len+5 with plane xl = x0 - 3 + s; planes outside
-// [0, nx) wrap on a periodic x axis and are skipped on a zero one.
-struct PlaneIter {
-    long long L, L1;
-    long long band;
-    int nx, per_x;
-    int x0, len, s;
-    __device__ void init(long long l0, long long l1, int nx_, int per)
+// The linear (band, x) plane range [L0, L1) of a team, cut into segments of one band each:
+// segment 0 = (b0, [x00, x00+len0)), segment k >= 1 = (b0+k, [0, len_k)).  A segment of `len`
+// output planes takes len + 6 steps s = 0..len+5; step s brings in plane xl = x0 - 3 + s.
+struct TeamRange {
+    long long L0, L1;
+    int nx;
+    int b0, x00, len0;
+    int nsteps;
+    __device__ void init(long long l0, long long l1, int nx_)
     {
-        L = l0;
+        L0 = l0;
         L1 = l1;
         nx = nx_;
-        per_x = per;
-        seg();
+        b0 = (int)(l0 / nx_);
+        x00 = (int)(l0 - (long long)b0 * nx_);
+        const long long n = l1 - l0;
+        len0 = (n < (long long)(nx_ - x00)) ? (int)n : (nx_ - x00);
+        const long long rest = n - len0;
+        const int nseg = 1 + (int)((rest + nx_ - 1) / nx_);
+        nsteps = (int)n + 6 * nseg;
     }
-    __device__ void seg()
+    // Table entry of step e: x = plane to load (band*nx + x, or -1: no data, value is zero),
+    // y = output plane completed by this step (or -1), z = x index of the plane if it is a centre
+    // plane (y/z taps, v_eff), else -1, w = 0 | +1 (wrapped past the upper x end) | -1 (lower).
+    __device__ int4 entry(int e, int per_x) const
     {
-        s = 0;
-        if (L < L1) {
-            band = L / nx;
-            x0 = (int)(L - band * nx);
-            const long long rem = L1 - L;
-            len = (rem < (long long)(nx - x0)) ? (int)rem : (nx - x0);
+        int band, x0, len, s;
+        if (e < len0 + 6) {
+            band = b0;
+            x0 = x00;
+            len = len0;
+            s = e;
         } else {
-            band = 0;
+            const int e2 = e - (len0 + 6);
+            const int k = e2 / (nx + 6);
+            s = e2 - k * (nx + 6);
+            band = b0 + 1 + k;
             x0 = 0;
-            len = 0;
+            const long long rem = L1 - (L0 + len0 + (long long)k * nx);
+            len = (rem < (long long)nx) ? (int)rem : nx;
         }
-    }
-    // next plane to load: returns false when exhausted
-    __device__ bool next(long long &b, int &xg)
-    {
-        while (L < L1) {
-            if (s >= len + 6) {
-                L += len;
-                seg();
-                continue;
-            }
-            const int xl = x0 - 3 + s;
-            ++s;
-            if (xl < 0) {
-                if (!per_x) continue;
-                xg = xl + nx;
-            } else if (xl >= nx) {
-                if (!per_x) continue;
-                xg = xl - nx;
-            } else {
-                xg = xl;
-            }
-            b = band;
-            return true;
+        const int xl = x0 - 3 + s;
+        int4 m;
+        m.w = 0;
+        if (xl < 0) {
+            m.x = per_x ? band * nx + xl + nx : -1;
+            m.w = per_x ? -1 : 0;
+        } else if (xl >= nx) {
+            m.x = per_x ? band * nx + xl - nx : -1;
+            m.w = per_x ? 1 : 0;
+        } else {
+            m.x = band * nx + xl;
         }
-        return false;
+        m.y = (s >= 6) ? band * nx + x0 + s - 6 : -1;
+        m.z = (s >= 3 && s < len + 3) ? xl : -1;
+        return m;
     }
 };
 
 template <bool CPLX, bool HAS_V>
 __global__ void __launch_bounds__(kMaxThreads, 1)
-fd_sweep_kernel(const FdGeom g, const FdSweepCfg cfg, const double *__restrict__ psi,
-                const double *__restrict__ v_eff, double *__restrict__ out,
-                const long long total_planes, const int quota)
+fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSweepCfg cfg,
+                const double *__restrict__ psi, const double *__restrict__ v_eff,
+                double *__restrict__ out, const long long total_planes, const int quota)
 {
     constexpr int TY = CPLX ? 2 : 4;   // rows per thread
     constexpr int TC = CPLX ? 2 : 1;   // 16-byte chunks per thread per row
@@ -172,17 +203,23 @@ fd_sweep_kernel(const FdGeom g, const FdSweepCfg cfg, const double *__restrict__
 
     extern __shared__ __align__(128) unsigned char smem[];
     const uint32_t smem_base = smem_u32(smem);
-    const uint32_t full_bar = smem_base;        // kStages x 8 bytes
-    const uint32_t empty_bar = smem_base + 64;  // kStages x 8 bytes
-    const uint32_t stage0 = smem_base + kBarBytes;
+    const uint32_t full_bar = smem_base;         // kMaxStages x 8 bytes
+    const uint32_t empty_bar = smem_base + 64;   // kMaxStages x 8 bytes
+    unsigned int *const elect_cnt = reinterpret_cast<unsigned int *>(smem + 128);
+    const uint32_t tab = smem_base + (uint32_t)cfg.tab_off;
+    const uint32_t stage0 = smem_base + (uint32_t)cfg.stage_off;
+    const uint32_t stage_bytes = (uint32_t)cfg.stage_bytes;
+    const int K = cfg.stages;
 
     const int nx = g.n[0], ny = g.n[1], nz = g.n[2];
-    const int pitch = nz * (CPLX ? 16 : 8);  // bytes per z row
+    const int pitch = nz * (CPLX ? 16 : 8);  // bytes per z row of psi
+    const int pitchv = nz * 8;               // bytes per z row of v_eff
     const int cpr = pitch >> 4;              // 16-byte chunks per row
     const int rowd = pitch >> 3;             // doubles per row
     const int tid = threadIdx.x;
     const int lane = tid & 31;
-    const int nwarps = blockDim.x >> 5;
+    const unsigned nwarps = blockDim.x >> 5;
+    const bool clustered = cfg.cluster > 1;
 
     const int yt = (int)(blockIdx.x % (unsigned)cfg.nytiles);
     const long long team = blockIdx.x / (unsigned)cfg.nytiles;
@@ -190,39 +227,73 @@ fd_sweep_kernel(const FdGeom g, const FdSweepCfg cfg, const double *__restrict__
     const int rows_valid = min(cfg.tyc, ny - y0);
     const long long L0 = team * (long long)quota;
     const long long L1 = (L0 + quota < total_planes) ? (L0 + quota) : total_planes;
-    if (L0 >= L1) return;  // whole CTA exits together
+    if (L0 >= L1) return;  // the whole team (cluster) exits together
 
     // ---- y segments of the staged tile: smem row R <-> global row y0 - 3 + R ------------------
     const int per_y = g.bc[1], per_x = g.bc[0], per_z = g.bc[2];
     const int nlo = max(0, 3 - y0);                     // rows below row 0
     const int nhi = max(0, y0 + rows_valid + 3 - ny);   // rows past row ny-1
     const int nmid = rows_valid + 6 - nlo - nhi;
-    const uint32_t stage_bytes = (uint32_t)cfg.stage_bytes;
-    const uint32_t tx_bytes = (uint32_t)((nmid + (per_y ? nlo + nhi : 0)) * pitch);
+    const uint32_t zb = (uint32_t)cfg.zb_bytes;
+    const uint32_t tx_psi = (uint32_t)((nmid + (per_y ? nlo + nhi : 0)) * pitch);
+    const uint32_t tx_v = (uint32_t)(rows_valid * pitchv);
+
+    TeamRange tr;
+    tr.init(L0, L1, nx);
+    const int nsteps = tr.nsteps;
 
     // ---- one-time shared memory setup ------------------------------------------------------
     if (tid == 0) {
-        for (int i = 0; i < kStages; ++i) {
+        for (int i = 0; i < K; ++i) {
             mbar_init(full_bar + 8 * i, 1);
             mbar_init(empty_bar + 8 * i, nwarps);
+            elect_cnt[i] = 0;
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    for (int st = 0; st < kStages; ++st) {
-        unsigned char *sb = smem + kBarBytes + (size_t)st * stage_bytes;
-        if (tid < 2) reinterpret_cast<double *>(sb)[tid] = 0.0;  // the zero word
-        if (!per_y) {                                            // zero halo rows, written once
-            for (int i = tid; i < nlo * rowd; i += blockDim.x)
-                reinterpret_cast<double *>(sb + kRowOff)[i] = 0.0;
+    for (int e = tid; e < nsteps; e += blockDim.x)
+        reinterpret_cast<int4 *>(smem + cfg.tab_off)[e] = tr.entry(e, per_x);
+    for (int st = 0; st < K; ++st) {
+        unsigned char *sb = smem + cfg.stage_off + (size_t)st * stage_bytes;
+        for (int i = tid; i < (int)(zb >> 3); i += blockDim.x)  // the zero block
+            reinterpret_cast<double *>(sb)[i] = 0.0;
+        double *rows = reinterpret_cast<double *>(sb + zb);
+        if (!per_y) {  // zero halo rows, written once
+            for (int i = tid; i < nlo * rowd; i += blockDim.x) rows[i] = 0.0;
             for (int i = tid; i < nhi * rowd; i += blockDim.x)
-                reinterpret_cast<double *>(sb + kRowOff + (size_t)(nlo + nmid) * pitch)[i] = 0.0;
+                rows[(size_t)(nlo + nmid) * rowd + i] = 0.0;
         }
         // rows past the ragged end of the last tile are never loaded: define them
         for (int i = tid; i < (cfg.tyc - rows_valid) * rowd; i += blockDim.x)
-            reinterpret_cast<double *>(sb + kRowOff + (size_t)(rows_valid + 6) * pitch)[i] = 0.0;
+            rows[(size_t)(rows_valid + 6) * rowd + i] = 0.0;
     }
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     __syncthreads();
+
+    // ---- the load of table entry e into ring slot st (one thread) ------------------------------
+    auto issue = [&](int e, uint32_t st) {
+        const int4 me = lds_i4(tab + 16u * (uint32_t)e);
+        const uint32_t bar = full_bar + 8 * st;
+        if (me.x < 0) {
+            mbar_arrive(bar);
+            return;
+        }
+        const uint32_t dst = stage0 + st * stage_bytes + zb;
+        const double *src = psi + (long long)me.x * ((long long)ny * rowd);
+        const bool with_v = HAS_V && me.z >= 0;
+        mbar_expect_tx(bar, tx_psi + (with_v ? tx_v : 0u));
+        if (per_y && nlo > 0)
+            bulk_g2s(dst, src + (long long)(ny - nlo) * rowd, (uint32_t)(nlo * pitch), bar);
+        bulk_g2s(dst + nlo * pitch, src + (long long)(y0 - 3 + nlo) * rowd, (uint32_t)(nmid * pitch),
+                 bar);
+        if (per_y && nhi > 0)
+            bulk_g2s(dst + (nlo + nmid) * pitch, src, (uint32_t)(nhi * pitch), bar);
+        if (with_v)
+            bulk_g2s(stage0 + st * stage_bytes + (uint32_t)cfg.v_off,
+                     v_eff + ((long long)me.z * ny + y0) * nz, tx_v, bar);
+    };
+    if (tid == 0)
+        for (int i = 0; i < K && i < nsteps; ++i) issue(i, (uint32_t)i);
 
     // ---- thread -> micro tile ---------------------------------------------------------------
     int rg = tid / cfg.lanes;
@@ -231,10 +302,12 @@ fd_sweep_kernel(const FdGeom g, const FdSweepCfg cfg, const double *__restrict__
     if (!tactive) rg = cfg.rowgroups - 1;  // surplus threads shadow the last row group, never store
     const int r0 = rg * TY;                // first halo row (smem row index) of this thread
     const int zc0 = lz * TC;               // first own chunk in the row
-    const uint32_t own_off = kRowOff + (uint32_t)(r0 * pitch + zc0 * 16);
+    const uint32_t own_off = zb + (uint32_t)(r0 * pitch + zc0 * 16);
+    const uint32_t v_off = (uint32_t)cfg.v_off + (uint32_t)(r0 * pitchv + lz * 16);
 
-    // halo chunks along z: k < ZH left of the own chunks, k >= ZH right of them
-    uint32_t hb[2 * ZH], hs[2 * ZH];
+    // halo chunks along z: k < ZH left of the own chunks, k >= ZH right of them; an out-of-range
+    // chunk on a zero-BC axis reads the zero block at the start of the stage (offset 0).
+    uint32_t hb[2 * ZH];
     int zwrap = 0;  // 2 bits per halo chunk: 1 = wrapped below 0, 2 = wrapped past nz (complex only)
 #pragma unroll
     for (int k = 0; k < 2 * ZH; ++k) {
@@ -245,259 +318,232 @@ fd_sweep_kernel(const FdGeom g, const FdSweepCfg cfg, const double *__restrict__
         } else if (cz >= cpr) {
             if (per_z) { cz -= cpr; zwrap |= 2 << (2 * k); } else valid = false;
         }
-        hb[k] = valid ? (uint32_t)(kRowOff + (r0 + 3) * pitch + cz * 16) : 0u;
-        hs[k] = valid ? (uint32_t)pitch : 0u;
+        hb[k] = valid ? zb + (uint32_t)((r0 + 3) * pitch + cz * 16) : 0u;
     }
-    const bool zphase = CPLX && per_z && (g.ph_re[2] != 1.0 || g.ph_im[2] != 0.0);
+    const bool zphase = CPLX && per_z && (g.ph_re[2] != 1.0 || g.ph_im[2] != 0.0) && zwrap != 0;
     const bool yphase = CPLX && per_y && (g.ph_re[1] != 1.0 || g.ph_im[1] != 0.0);
     const bool xphase = CPLX && per_x && (g.ph_re[0] != 1.0 || g.ph_im[0] != 0.0);
 
-    // store / v_eff addressing: row i of the micro tile is global row y0 + r0 + i
-    bool row_ok[TY];
-    long long row_goff[TY];  // offset in doubles of (y, own chunk) inside an x plane of psi / out
-    long long row_voff[TY];  // offset in doubles inside an x plane of v_eff
+    // store addressing: row i of the micro tile is global row y0 + r0 + i
+    unsigned row_ok = 0;
 #pragma unroll
-    for (int i = 0; i < TY; ++i) {
-        const int yl = r0 + i;
-        row_ok[i] = tactive && (yl < rows_valid) && (zc0 < cpr);
-        const int y = min(y0 + yl, ny - 1);
-        const int zc = min(zc0, cpr - TC);
-        row_goff[i] = (long long)y * rowd + zc * 2;
-        row_voff[i] = (long long)y * nz + (CPLX ? zc : zc * 2);
-    }
+    for (int i = 0; i < TY; ++i)
+        if (tactive && (r0 + i) < rows_valid) row_ok |= 1u << i;
+    double *const obase = out + (long long)(y0 + r0) * rowd + zc0 * 2;
     const long long plane_d = (long long)ny * rowd;  // doubles per x plane of psi / out
-    const long long plane_v = (long long)ny * nz;
 
     const double wx1 = g.w[0][1], wx2 = g.w[0][2], wx3 = g.w[0][3];
     const double wy1 = g.w[1][1], wy2 = g.w[1][2], wy3 = g.w[1][3];
     const double wz1 = g.w[2][1], wz2 = g.w[2][2], wz3 = g.w[2][3];
     const double wdiag = g.wdiag;
 
-    // ---- producer state (thread 0) -------------------------------------------------------------
-    PlaneIter it;
-    long long q_issued = 0;
-    auto issue = [&](long long qi, long long b, int xg) {
-        const uint32_t st = (uint32_t)(qi & (kStages - 1));
-        const uint32_t bar = full_bar + 8 * st;
-        const uint32_t dst = stage0 + st * stage_bytes + kRowOff;
-        const double *src = psi + ((b * nx + xg) * (long long)ny) * rowd;
-        mbar_expect_tx(bar, tx_bytes);
-        if (per_y && nlo > 0)
-            bulk_g2s(dst, src + (long long)(ny - nlo) * rowd, (uint32_t)(nlo * pitch), bar);
-        bulk_g2s(dst + nlo * pitch, src + (long long)(y0 - 3 + nlo) * rowd, (uint32_t)(nmid * pitch),
-                 bar);
-        if (per_y && nhi > 0)
-            bulk_g2s(dst + (nlo + nmid) * pitch, src, (uint32_t)(nhi * pitch), bar);
-    };
-    if (tid == 0) {
-        it.init(L0, L1, nx, per_x);
-        long long b;
-        int xg;
-        for (int i = 0; i < kStages; ++i) {
-            if (!it.next(b, xg)) break;
-            issue(q_issued, b, xg);
-            ++q_issued;
-        }
-    }
-
-    // ---- consumer sweep ----------------------------------------------------------------------
-    long long q = 0;  // planes consumed so far by this thread
+    // ---- the sweep: one flat loop over the step table ------------------------------------------
     double2 acc[7][NP];
 #pragma unroll
     for (int a = 0; a < 7; ++a)
 #pragma unroll
         for (int p = 0; p < NP; ++p) acc[a][p] = make_double2(0.0, 0.0);
 
-    for (long long L = L0; L < L1;) {
-        const long long band = L / nx;
-        const int x0 = (int)(L - band * nx);
-        const int len = ((L1 - L) < (long long)(nx - x0)) ? (int)(L1 - L) : (nx - x0);
-        const int nsteps = len + 6;
-        const double *vplane = HAS_V ? v_eff + (long long)x0 * plane_v : nullptr;
-        double *oplane = out + (band * nx + x0) * plane_d;
+    uint32_t st = 0, par = 0;  // ring slot and mbarrier phase parity of the current step
+    for (int q7 = 0; q7 < nsteps; q7 += 7) {
+#pragma unroll
+        for (int J = 0; J < 7; ++J) {
+            const int q = q7 + J;
+            if (q < nsteps) {
+                const int4 m = lds_i4(tab + 16u * (uint32_t)q);
+                if (clustered) {  // keep the team's CTAs within one step of each other
+                    if (q > 0) cluster_wait();
+                    cluster_arrive();
+                }
+                mbar_wait(full_bar + 8 * st, par);
+                const uint32_t sb = stage0 + st * stage_bytes;
 
-        for (int s7 = 0; s7 < nsteps; s7 += 7) {
+                // ---- own values of the incoming plane
+                double2 u[NP];
+                if (m.x >= 0) {
 #pragma unroll
-            for (int J = 0; J < 7; ++J) {
-                const int s = s7 + J;
-                if (s < nsteps) {
-                    const int xl = x0 - 3 + s;
-                    const bool center = (s >= 3) && (s < 3 + len);
-                    const bool valid = per_x || (xl >= 0 && xl < nx);
-                    if (valid) {
-                        // producer: refill the stage plane q-1 lived in with plane q-1+kStages
-                        if (tid == 0 && q >= 1 && q_issued == q - 1 + kStages) {
-                            long long b;
-                            int xg;
-                            if (it.next(b, xg)) {
-                                const long long qp = q - 1;
-                                mbar_wait(empty_bar + 8 * (uint32_t)(qp & (kStages - 1)),
-                                          (uint32_t)((qp >> kStagesLog2) & 1));
-                                issue(q_issued, b, xg);
-                                ++q_issued;
-                            }
-                        }
-                        double2 vv[TY];
-                        if (HAS_V && center) {
+                    for (int i = 0; i < TY; ++i)
 #pragma unroll
-                            for (int i = 0; i < TY; ++i)
-                                vv[i] = __ldg(reinterpret_cast<const double2 *>(
-                                    vplane + (long long)(s - 3) * plane_v + row_voff[i]));
-                        }
-                        const uint32_t st = (uint32_t)(q & (kStages - 1));
-                        mbar_wait(full_bar + 8 * st, (uint32_t)((q >> kStagesLog2) & 1));
-                        const uint32_t sb = stage0 + st * stage_bytes;
-                        double2 u[NP];
-                        if (center) {
-                            // ---- y taps (+ own values) from the staged tile
-                            double2 c[TY + 6][TC];
-#pragma unroll
-                            for (int rr = 0; rr < TY + 6; ++rr)
-#pragma unroll
-                                for (int t = 0; t < TC; ++t)
-                                    c[rr][t] = lds128(sb + own_off + rr * pitch + t * 16);
-                            if (yphase) {
-#pragma unroll
-                                for (int rr = 0; rr < TY + 6; ++rr) {
-                                    const int R = r0 + rr;
-                                    if (R < nlo) {
-#pragma unroll
-                                        for (int t = 0; t < TC; ++t)
-                                            c[rr][t] = cmul(c[rr][t], g.ph_re[1], -g.ph_im[1]);
-                                    } else if (R >= nlo + nmid) {
-#pragma unroll
-                                        for (int t = 0; t < TC; ++t)
-                                            c[rr][t] = cmul(c[rr][t], g.ph_re[1], g.ph_im[1]);
-                                    }
-                                }
-                            }
-#pragma unroll
-                            for (int i = 0; i < TY; ++i)
-#pragma unroll
-                                for (int t = 0; t < TC; ++t) {
-                                    double2 &a = acc[J][i * TC + t];
-                                    u[i * TC + t] = c[3 + i][t];
-                                    fma2(a, wy1, c[2 + i][t]);
-                                    fma2(a, wy1, c[4 + i][t]);
-                                    fma2(a, wy2, c[1 + i][t]);
-                                    fma2(a, wy2, c[5 + i][t]);
-                                    fma2(a, wy3, c[i][t]);
-                                    fma2(a, wy3, c[6 + i][t]);
-                                }
-                            // ---- z taps
-#pragma unroll
-                            for (int i = 0; i < TY; ++i) {
-                                double2 hz[2 * ZH];
-#pragma unroll
-                                for (int k = 0; k < 2 * ZH; ++k)
-                                    hz[k] = lds128(sb + hb[k] + i * hs[k]);
-                                if (zphase && zwrap != 0) {
-#pragma unroll
-                                    for (int k = 0; k < 2 * ZH; ++k) {
-                                        const int wbits = (zwrap >> (2 * k)) & 3;
-                                        if (wbits == 1) hz[k] = cmul(hz[k], g.ph_re[2], -g.ph_im[2]);
-                                        if (wbits == 2) hz[k] = cmul(hz[k], g.ph_re[2], g.ph_im[2]);
-                                    }
-                                }
-                                if constexpr (CPLX) {
-                                    // chunks are complex points: own C0,C1; hz = L3,L2,L1,R1,R2,R3
-                                    double2 &a0 = acc[J][i * TC + 0];
-                                    double2 &a1 = acc[J][i * TC + (TC - 1)];
-                                    const double2 C0 = u[i * TC + 0], C1 = u[i * TC + (TC - 1)];
-                                    fma2(a0, wz1, hz[ZH - 1]);
-                                    fma2(a0, wz1, C1);
-                                    fma2(a0, wz2, hz[ZH - 2]);
-                                    fma2(a0, wz2, hz[ZH]);
-                                    fma2(a0, wz3, hz[0]);
-                                    fma2(a0, wz3, hz[ZH + 1]);
-                                    fma2(a1, wz1, C0);
-                                    fma2(a1, wz1, hz[ZH]);
-                                    fma2(a1, wz2, hz[ZH - 1]);
-                                    fma2(a1, wz2, hz[ZH + 1]);
-                                    fma2(a1, wz3, hz[ZH - 2]);
-                                    fma2(a1, wz3, hz[2 * ZH - 1]);
-                                } else {
-                                    // chunk = points (z, z+1); hz = L2,L1,R1,R2
-                                    double2 &a = acc[J][i];
-                                    const double2 o = u[i];
-                                    a.x = fma(wz1, hz[1].y, a.x);
-                                    a.x = fma(wz1, o.y, a.x);
-                                    a.x = fma(wz2, hz[1].x, a.x);
-                                    a.x = fma(wz2, hz[2].x, a.x);
-                                    a.x = fma(wz3, hz[0].y, a.x);
-                                    a.x = fma(wz3, hz[2].y, a.x);
-                                    a.y = fma(wz1, o.x, a.y);
-                                    a.y = fma(wz1, hz[2].x, a.y);
-                                    a.y = fma(wz2, hz[1].y, a.y);
-                                    a.y = fma(wz2, hz[2].y, a.y);
-                                    a.y = fma(wz3, hz[1].x, a.y);
-                                    a.y = fma(wz3, hz[3].x, a.y);
-                                }
-                            }
-                        } else {
-#pragma unroll
-                            for (int i = 0; i < TY; ++i)
-#pragma unroll
-                                for (int t = 0; t < TC; ++t)
-                                    u[i * TC + t] = lds128(sb + own_off + (3 + i) * pitch + t * 16);
-                            if (xphase && (xl < 0 || xl >= nx)) {
-                                const double pi_ = (xl < 0) ? -g.ph_im[0] : g.ph_im[0];
-#pragma unroll
-                                for (int p = 0; p < NP; ++p) u[p] = cmul(u[p], g.ph_re[0], pi_);
-                            }
-                        }
-                        // done with the stage: release it to the producer
-                        __syncwarp();
-                        if (lane == 0) mbar_arrive(empty_bar + 8 * st);
-                        ++q;
-
-                        // ---- diagonal (+ v_eff) and x taps (scatter into the 7 in-flight outputs)
-                        if (center) {
-#pragma unroll
-                            for (int i = 0; i < TY; ++i) {
-                                if constexpr (CPLX) {
-                                    const double d0 = HAS_V ? wdiag + vv[i].x : wdiag;
-                                    const double d1 = HAS_V ? wdiag + vv[i].y : wdiag;
-                                    fma2(acc[J][i * TC + 0], d0, u[i * TC + 0]);
-                                    fma2(acc[J][i * TC + (TC - 1)], d1, u[i * TC + (TC - 1)]);
-                                } else {
-                                    const double d0 = HAS_V ? wdiag + vv[i].x : wdiag;
-                                    const double d1 = HAS_V ? wdiag + vv[i].y : wdiag;
-                                    acc[J][i].x = fma(d0, u[i].x, acc[J][i].x);
-                                    acc[J][i].y = fma(d1, u[i].y, acc[J][i].y);
-                                }
-                            }
-                        }
-#pragma unroll
-                        for (int p = 0; p < NP; ++p) {
-                            acc[(J + 3) % 7][p] = mul2(wx3, u[p]);
-                            fma2(acc[(J + 2) % 7][p], wx2, u[p]);
-                            fma2(acc[(J + 1) % 7][p], wx1, u[p]);
-                            fma2(acc[(J + 6) % 7][p], wx1, u[p]);
-                            fma2(acc[(J + 5) % 7][p], wx2, u[p]);
-                            fma2(acc[(J + 4) % 7][p], wx3, u[p]);
-                        }
-                    } else {
-#pragma unroll
-                        for (int p = 0; p < NP; ++p) acc[(J + 3) % 7][p] = make_double2(0.0, 0.0);
-                    }
-                    // ---- output x0 + s - 6 is complete
-                    if (s >= 6) {
-                        double *o = oplane + (long long)(s - 6) * plane_d;
+                        for (int t = 0; t < TC; ++t)
+                            u[i * TC + t] = lds128(sb + own_off + (3 + i) * pitch + t * 16);
+                    if (CPLX && yphase) {
+                        // rows past a ragged tile end are wrapped rows: neighbours of the last
+                        // valid rows, so they carry the y Bloch factor like any halo row
 #pragma unroll
                         for (int i = 0; i < TY; ++i)
-                            if (row_ok[i]) {
+                            if (r0 + 3 + i >= nlo + nmid) {
 #pragma unroll
                                 for (int t = 0; t < TC; ++t)
-                                    __stcs(reinterpret_cast<double2 *>(o + row_goff[i]) + t,
-                                           acc[(J + 4) % 7][i * TC + t]);
+                                    u[i * TC + t] = cmul(u[i * TC + t], g.ph_re[1], g.ph_im[1]);
                             }
                     }
+                    if (CPLX && xphase && m.w != 0) {
+                        const double pi_ = (m.w < 0) ? -g.ph_im[0] : g.ph_im[0];
+#pragma unroll
+                        for (int p = 0; p < NP; ++p) u[p] = cmul(u[p], g.ph_re[0], pi_);
+                    }
+                } else {
+#pragma unroll
+                    for (int p = 0; p < NP; ++p) u[p] = make_double2(0.0, 0.0);
                 }
+
+                // ---- x taps, oldest output first: it is complete after this and leaves
+#pragma unroll
+                for (int p = 0; p < NP; ++p) fma2(acc[(J + 4) % 7][p], wx3, u[p]);
+                if (m.y >= 0) {
+                    double *o = obase + (long long)m.y * plane_d;
+#pragma unroll
+                    for (int i = 0; i < TY; ++i)
+                        if (row_ok & (1u << i)) {
+#pragma unroll
+                            for (int t = 0; t < TC; ++t)
+                                __stcs(reinterpret_cast<double2 *>(o + (long long)i * rowd) + t,
+                                       acc[(J + 4) % 7][i * TC + t]);
+                        }
+                }
+#pragma unroll
+                for (int p = 0; p < NP; ++p) {
+                    fma2(acc[(J + 5) % 7][p], wx2, u[p]);
+                    fma2(acc[(J + 6) % 7][p], wx1, u[p]);
+                    fma2(acc[(J + 1) % 7][p], wx1, u[p]);
+                    fma2(acc[(J + 2) % 7][p], wx2, u[p]);
+                }
+
+                if (m.z >= 0) {
+                    // ---- diagonal (+ v_eff)
+#pragma unroll
+                    for (int i = 0; i < TY; ++i) {
+                        double d0 = wdiag, d1 = wdiag;
+                        if (HAS_V) {
+                            const double2 vv = lds128(sb + v_off + i * pitchv);
+                            d0 += vv.x;
+                            d1 += vv.y;
+                        }
+                        if constexpr (CPLX) {
+                            fma2(acc[J][i * TC + 0], d0, u[i * TC + 0]);
+                            fma2(acc[J][i * TC + (TC - 1)], d1, u[i * TC + (TC - 1)]);
+                        } else {
+                            acc[J][i].x = fma(d0, u[i].x, acc[J][i].x);
+                            acc[J][i].y = fma(d1, u[i].y, acc[J][i].y);
+                        }
+                    }
+                    // ---- y taps: stream the TY + 6 rows of the thread's column through
+#pragma unroll
+                    for (int rr = 0; rr < TY + 6; ++rr) {
+                        if (rr >= 3 && rr < 3 + TY) continue;  // own rows: already in u
+                        double2 c[TC];
+#pragma unroll
+                        for (int t = 0; t < TC; ++t) c[t] = lds128(sb + own_off + rr * pitch + t * 16);
+                        if (CPLX && yphase) {
+                            const int R = r0 + rr;
+                            if (R < nlo) {
+#pragma unroll
+                                for (int t = 0; t < TC; ++t) c[t] = cmul(c[t], g.ph_re[1], -g.ph_im[1]);
+                            } else if (R >= nlo + nmid) {
+#pragma unroll
+                                for (int t = 0; t < TC; ++t) c[t] = cmul(c[t], g.ph_re[1], g.ph_im[1]);
+                            }
+                        }
+#pragma unroll
+                        for (int i = 0; i < TY; ++i) {
+                            const int d = rr - 3 - i;
+                            const int ad = d < 0 ? -d : d;
+                            if (ad >= 1 && ad <= 3) {
+                                const double w = (ad == 1) ? wy1 : (ad == 2) ? wy2 : wy3;
+#pragma unroll
+                                for (int t = 0; t < TC; ++t) fma2(acc[J][i * TC + t], w, c[t]);
+                            }
+                        }
+                    }
+                    // own rows are y neighbours of each other
+#pragma unroll
+                    for (int i = 0; i < TY; ++i)
+#pragma unroll
+                        for (int i2 = 0; i2 < TY; ++i2) {
+                            const int ad = i2 > i ? i2 - i : i - i2;
+                            if (ad >= 1 && ad <= 3) {
+                                const double w = (ad == 1) ? wy1 : (ad == 2) ? wy2 : wy3;
+#pragma unroll
+                                for (int t = 0; t < TC; ++t)
+                                    fma2(acc[J][i * TC + t], w, u[i2 * TC + t]);
+                            }
+                        }
+                    // ---- z taps
+#pragma unroll
+                    for (int i = 0; i < TY; ++i) {
+                        if constexpr (CPLX) {
+                            double2 hz[2 * ZH];
+#pragma unroll
+                            for (int k = 0; k < 2 * ZH; ++k) hz[k] = lds128(sb + hb[k] + i * pitch);
+                            if (zphase) {
+#pragma unroll
+                                for (int k = 0; k < 2 * ZH; ++k) {
+                                    const int wbits = (zwrap >> (2 * k)) & 3;
+                                    if (wbits == 1) hz[k] = cmul(hz[k], g.ph_re[2], -g.ph_im[2]);
+                                    if (wbits == 2) hz[k] = cmul(hz[k], g.ph_re[2], g.ph_im[2]);
+                                }
+                            }
+                            // chunks are complex points: own C0,C1; hz = L3,L2,L1,R1,R2,R3
+                            double2 &a0 = acc[J][i * TC + 0];
+                            double2 &a1 = acc[J][i * TC + (TC - 1)];
+                            const double2 C0 = u[i * TC + 0], C1 = u[i * TC + (TC - 1)];
+                            fma2(a0, wz1, hz[ZH - 1]);
+                            fma2(a0, wz1, C1);
+                            fma2(a0, wz2, hz[ZH - 2]);
+                            fma2(a0, wz2, hz[ZH]);
+                            fma2(a0, wz3, hz[0]);
+                            fma2(a0, wz3, hz[ZH + 1]);
+                            fma2(a1, wz1, C0);
+                            fma2(a1, wz1, hz[ZH]);
+                            fma2(a1, wz2, hz[ZH - 1]);
+                            fma2(a1, wz2, hz[ZH + 1]);
+                            fma2(a1, wz3, hz[ZH - 2]);
+                            fma2(a1, wz3, hz[2 * ZH - 1]);
+                        } else {
+                            // chunk = points (z, z+1); halo = z-3 | z-2,z-1 | z+2,z+3 | z+4
+                            const double l3 = lds64(sb + hb[0] + i * pitch + 8);
+                            const double2 l21 = lds128(sb + hb[1] + i * pitch);
+                            const double2 r23 = lds128(sb + hb[2] + i * pitch);
+                            const double r4 = lds64(sb + hb[3] + i * pitch);
+                            double2 &a = acc[J][i];
+                            const double2 o = u[i];
+                            a.x = fma(wz1, l21.y, a.x);
+                            a.x = fma(wz1, o.y, a.x);
+                            a.x = fma(wz2, l21.x, a.x);
+                            a.x = fma(wz2, r23.x, a.x);
+                            a.x = fma(wz3, l3, a.x);
+                            a.x = fma(wz3, r23.y, a.x);
+                            a.y = fma(wz1, o.x, a.y);
+                            a.y = fma(wz1, r23.x, a.y);
+                            a.y = fma(wz2, l21.y, a.y);
+                            a.y = fma(wz2, r23.y, a.y);
+                            a.y = fma(wz3, l21.x, a.y);
+                            a.y = fma(wz3, r4, a.y);
+                        }
+                    }
+                }
+
+                // ---- release the slot; the last warp to do so refills it with step q + K
+                __syncwarp();
+                if (lane == 0) {
+                    mbar_arrive(empty_bar + 8 * st);
+                    if (atomicInc(&elect_cnt[st], nwarps - 1) == nwarps - 1 && q + K < nsteps) {
+                        mbar_wait(empty_bar + 8 * st, par);
+                        issue(q + K, st);
+                    }
+                }
+                if (++st == (uint32_t)K) {
+                    st = 0;
+                    par ^= 1u;
+                }
+
+                // ---- the output three planes ahead is born
+#pragma unroll
+                for (int p = 0; p < NP; ++p) acc[(J + 3) % 7][p] = mul2(wx3, u[p]);
             }
         }
-        L += len;
     }
+    if (clustered) cluster_wait();
 }
 
 inline int ceil_div(int a, int b) { return (a + b - 1) / b; }
@@ -509,91 +555,173 @@ void fd_sweep_configure(fd_plan *plan, int tyc_override, int xchunk_override)
     FdSweepCfg &c = plan->sweep;
     const FdGeom &g = plan->g;
     c = FdSweepCfg{};
-    c.xchunk = xchunk_override;  // 0 = automatic (persistent teams), else planes per CTA
+    c.xchunk = xchunk_override;  // 0 = automatic (persistent teams), else planes per team
     if (g.nn != 3) return;
     if (g.n[0] < 8 || g.n[1] < 8 || g.n[2] < 8 || (g.n[2] & 1)) return;
     c.ty = g.cplx ? 2 : 4;
     c.tc = g.cplx ? 2 : 1;
     const int pitch = g.n[2] * (g.cplx ? 16 : 8);
-    const int cpr = pitch / 16;
-    c.lanes = ceil_div(cpr, c.tc);
+    const int pitchv = g.n[2] * 8;
+    c.lanes = (pitch / 16) / c.tc;
     if (c.lanes > kMaxThreads) return;
-    const int smem_cap = 227 * 1024 - kBarBytes;
-    const int rows_cap = (smem_cap / kStages - kRowOff) / pitch - 6;  // tile rows that fit a stage
-    int max_rg = kMaxThreads / c.lanes;
-    if (max_rg * c.ty > rows_cap) max_rg = rows_cap / c.ty;
-    if (max_rg < 1) return;
-    int tyc;
+    c.zb_bytes = (g.bc[2] == 0) ? (c.ty * pitch + 127) / 128 * 128 : 0;
+    const int max_rg = kMaxThreads / c.lanes;
+    auto stage_bytes = [&](int tyc) {
+        return (c.zb_bytes + (tyc + 6) * pitch + tyc * pitchv + 127) / 128 * 128;
+    };
+    // fewest y tiles whose stage fits a ring of >= 3 slots beside a 4 KiB step table
+    int tyc = 0;
+    const int first = ceil_div(g.n[1], max_rg * c.ty);
+    for (int ntiles = first; ntiles <= g.n[1]; ++ntiles) {
+        const int t = ceil_div(ceil_div(g.n[1], ntiles), c.ty) * c.ty;
+        if (3 * stage_bytes(t) + kCtlBytes + 4096 <= kSmemMax) {
+            tyc = t;
+            break;
+        }
+        if (t == c.ty) break;
+    }
     if (tyc_override > 0) {
         tyc = ceil_div(tyc_override, c.ty) * c.ty;
         if (tyc > max_rg * c.ty) tyc = max_rg * c.ty;
-    } else {
-        const int ntiles = ceil_div(g.n[1], max_rg * c.ty);
-        tyc = ceil_div(ceil_div(g.n[1], ntiles), c.ty) * c.ty;
+        if (2 * stage_bytes(tyc) + kCtlBytes + 4096 > kSmemMax) return;
     }
-    if (tyc < 4) tyc = 4;
+    if (tyc <= 0) return;
     c.tyc = tyc;
     c.rowgroups = tyc / c.ty;
     c.nytiles = ceil_div(g.n[1], tyc);
     c.threads = ceil_div(c.rowgroups * c.lanes, 32) * 32;
-    c.stages = kStages;
-    c.stage_bytes = ((kRowOff + (tyc + 6) * pitch) + 127) / 128 * 128;
-    c.smem_bytes = kBarBytes + kStages * c.stage_bytes;
-    if (c.smem_bytes > 227 * 1024 || c.threads > kMaxThreads) return;
+    c.stage_bytes = stage_bytes(tyc);
+    c.v_off = c.zb_bytes + (tyc + 6) * pitch;
+    int tab_bytes = 16384;
+    int stages = (kSmemMax - kCtlBytes - tab_bytes) / c.stage_bytes;
+    if (stages < 3) {
+        tab_bytes = 4096;
+        stages = (kSmemMax - kCtlBytes - tab_bytes) / c.stage_bytes;
+    }
+    if (stages < 2) return;
+    if (stages > 6) stages = 6;
+    c.stages = stages;
+    tab_bytes = (kSmemMax - kCtlBytes - stages * c.stage_bytes) / 128 * 128;
+    if (tab_bytes > 65536) tab_bytes = 65536;
+    c.tab_off = kCtlBytes;
+    c.tab_cap = tab_bytes / 16;
+    c.stage_off = kCtlBytes + tab_bytes;
+    c.smem_bytes = c.stage_off + stages * c.stage_bytes;
+    c.cluster = (c.nytiles > 1 && c.nytiles <= 8) ? c.nytiles : 1;
+    c.max_teams = plan->sm_count / c.nytiles > 0 ? plan->sm_count / c.nytiles : 1;
+    if (c.smem_bytes > kSmemMax || c.threads > kMaxThreads) return;
     c.supported = 1;
 }
 
-cudaError_t fd_sweep_prepare(const fd_plan *plan)
+template <bool CPLX, bool HAS_V>
+static cudaError_t prepare_one(FdSweepCfg &c, int *max_clusters)
 {
-    const int bytes = plan->sweep.smem_bytes;
+    auto kern = fd_sweep_kernel<CPLX, HAS_V>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         c.smem_bytes);
+    if (e != cudaSuccess || c.cluster <= 1) return e;
+    cudaLaunchConfig_t lc = {};
+    lc.gridDim = dim3((unsigned)(c.cluster * 64));
+    lc.blockDim = dim3((unsigned)c.threads);
+    lc.dynamicSmemBytes = (size_t)c.smem_bytes;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = (unsigned)c.cluster;
+    at[0].val.clusterDim.y = 1;
+    at[0].val.clusterDim.z = 1;
+    lc.attrs = at;
+    lc.numAttrs = 1;
+    int n = 0;
+    e = cudaOccupancyMaxActiveClusters(&n, kern, &lc);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        n = 0;
+    }
+    if (n < *max_clusters) *max_clusters = n;
+    return cudaSuccess;
+}
+
+cudaError_t fd_sweep_prepare(fd_plan *plan)
+{
+    FdSweepCfg &c = plan->sweep;
+    int max_clusters = 1 << 30;
     cudaError_t e;
-    e = cudaFuncSetAttribute(fd_sweep_kernel<false, false>,
-                             cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-    if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(fd_sweep_kernel<false, true>,
-                             cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-    if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(fd_sweep_kernel<true, false>,
-                             cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-    if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(fd_sweep_kernel<true, true>,
-                                cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (plan->g.cplx) {
+        if ((e = prepare_one<true, false>(c, &max_clusters)) != cudaSuccess) return e;
+        if ((e = prepare_one<true, true>(c, &max_clusters)) != cudaSuccess) return e;
+    } else {
+        if ((e = prepare_one<false, false>(c, &max_clusters)) != cudaSuccess) return e;
+        if ((e = prepare_one<false, true>(c, &max_clusters)) != cudaSuccess) return e;
+    }
+    if (c.cluster > 1) {
+        if (max_clusters < 1) {  // clusters of this size cannot be resident: plain launch
+            c.cluster = 1;
+        } else {
+            c.max_teams = max_clusters;
+        }
+    }
+    return cudaSuccess;
+}
+
+template <bool CPLX, bool HAS_V>
+static cudaError_t launch_one(const fd_plan *plan, const double *psi, const double *v_eff,
+                              double *out, long long total, int quota, unsigned nblocks,
+                              cudaStream_t stream)
+{
+    const FdSweepCfg &c = plan->sweep;
+    cudaLaunchConfig_t lc = {};
+    lc.gridDim = dim3(nblocks);
+    lc.blockDim = dim3((unsigned)c.threads);
+    lc.dynamicSmemBytes = (size_t)c.smem_bytes;
+    lc.stream = stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = (unsigned)c.cluster;
+    at[0].val.clusterDim.y = 1;
+    at[0].val.clusterDim.z = 1;
+    lc.attrs = at;
+    lc.numAttrs = c.cluster > 1 ? 1 : 0;
+    return cudaLaunchKernelEx(&lc, fd_sweep_kernel<CPLX, HAS_V>, plan->g, c, psi, v_eff, out, total,
+                              quota);
 }
 
 cudaError_t fd_launch_sweep(const fd_plan *plan, const void *psi, const double *v_eff, void *out,
-                            int64_t nbands, cudaStream_t stream)
+                            int64_t nbands, cudaStream_t stream, int *nlaunches)
 {
     const FdSweepCfg &c = plan->sweep;
     const FdGeom &g = plan->g;
-    const long long total = (long long)nbands * g.n[0];
-    // persistent teams: one CTA per SM, nytiles CTAs per team, equal plane quota per team
-    long long nteams = plan->sm_count / c.nytiles;
-    if (nteams < 1) nteams = 1;
-    long long quota;
-    if (c.xchunk > 0) {
-        quota = c.xchunk;
-    } else {
-        quota = (total + nteams - 1) / nteams;
-        const int min_quota = g.n[0] < 16 ? g.n[0] : 16;  // below this the 6 halo planes dominate
-        if (quota < min_quota) quota = min_quota;
-    }
-    nteams = (total + quota - 1) / quota;
-    const long long nblocks = nteams * c.nytiles;
-    if (nblocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
-    dim3 grid((unsigned)nblocks), block((unsigned)c.threads);
-    const double *p = static_cast<const double *>(psi);
-    double *o = static_cast<double *>(out);
-    const int qi = (int)quota;
-    if (g.cplx) {
-        if (v_eff)
-            fd_sweep_kernel<true, true><<<grid, block, c.smem_bytes, stream>>>(g, c, p, v_eff, o, total, qi);
+    const long long band_d = (long long)g.n[0] * g.n[1] * g.n[2] * (g.cplx ? 2 : 1);
+    // plane indices in the step table are int32: very large batches go out in several launches
+    const int64_t bands_per_launch = (1LL << 30) / g.n[0];
+    for (int64_t b0 = 0; b0 < nbands; b0 += bands_per_launch) {
+        const int64_t nb = (nbands - b0 < bands_per_launch) ? nbands - b0 : bands_per_launch;
+        const long long total = (long long)nb * g.n[0];
+        long long quota;
+        if (c.xchunk > 0) {
+            quota = c.xchunk;
+        } else {
+            quota = (total + c.max_teams - 1) / c.max_teams;
+            const int min_quota = g.n[0] < 16 ? g.n[0] : 16;  // below this the 6 halo planes dominate
+            if (quota < min_quota) quota = min_quota;
+        }
+        // the team's steps (quota + 6 per band touched) must fit the step table
+        const long long quota_cap = ((long long)(c.tab_cap - 12) * g.n[0]) / (g.n[0] + 6);
+        if (quota > quota_cap) quota = quota_cap;
+        if (quota < 1) return cudaErrorInvalidConfiguration;
+        const long long nteams = (total + quota - 1) / quota;
+        const long long nblocks = nteams * c.nytiles;
+        if (nblocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
+        const double *p = static_cast<const double *>(psi) + b0 * band_d;
+        double *o = static_cast<double *>(out) + b0 * band_d;
+        cudaError_t e;
+        if (g.cplx)
+            e = v_eff ? launch_one<true, true>(plan, p, v_eff, o, total, (int)quota, (unsigned)nblocks, stream)
+                      : launch_one<true, false>(plan, p, nullptr, o, total, (int)quota, (unsigned)nblocks, stream);
         else
-            fd_sweep_kernel<true, false><<<grid, block, c.smem_bytes, stream>>>(g, c, p, nullptr, o, total, qi);
-    } else {
-        if (v_eff)
-            fd_sweep_kernel<false, true><<<grid, block, c.smem_bytes, stream>>>(g, c, p, v_eff, o, total, qi);
-        else
-            fd_sweep_kernel<false, false><<<grid, block, c.smem_bytes, stream>>>(g, c, p, nullptr, o, total, qi);
+            e = v_eff ? launch_one<false, true>(plan, p, v_eff, o, total, (int)quota, (unsigned)nblocks, stream)
+                      : launch_one<false, false>(plan, p, nullptr, o, total, (int)quota, (unsigned)nblocks, stream);
+        if (e != cudaSuccess) return e;
+        if (nlaunches) ++*nlaunches;
     }
     return cudaPeekAtLastError();
 }
