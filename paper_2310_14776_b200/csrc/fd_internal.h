@@ -34,8 +34,7 @@ struct FdSweepCfg {
     int tab_cap;       // step table capacity (entries of 16 bytes)
     int stage_off;     // offset of stage 0
     int smem_bytes;    // dynamic shared memory per CTA
-    int cluster;       // CTAs per thread-block cluster (= nytiles), 1 = no cluster launch
-    int max_teams;     // teams (clusters) resident at once on the device
+    int max_teams;     // teams of nytiles CTAs resident at once (one CTA per SM)
     int xchunk;        // 0 = persistent teams, else x planes per team (tuning knob)
 };
 
@@ -55,6 +54,6 @@ cudaError_t fd_launch_generic(const fd_plan *plan, const void *psi, const double
                               int64_t nbands, cudaStream_t stream);
 // fd_sweep.cu
 void fd_sweep_configure(fd_plan *plan, int tyc_override, int xchunk_override);
-cudaError_t fd_sweep_prepare(fd_plan *plan);  // smem opt-in + resident cluster count
+cudaError_t fd_sweep_prepare(fd_plan *plan);  // shared-memory opt-in of the plan's kernels
 cudaError_t fd_launch_sweep(const fd_plan *plan, const void *psi, const double *v_eff, void *out,
                             int64_t nbands, cudaStream_t stream, int *nlaunches);

@@ -12,8 +12,9 @@
 //     `stages` slots, so HBM reads are deep, asynchronous and fully coalesced (whole rows), and
 //     each psi value crosses HBM once.
 //   * The whole schedule of a CTA (which plane to load, which output plane completes, which
-//     v_eff plane, which Bloch factor) is a table in shared memory built once at kernel start:
-//     the sweep itself is one flat loop over table entries with no index arithmetic.
+//     v_eff plane, which Bloch factor, which L2 policy) is a table in shared memory built once at
+//     kernel start: the sweep itself is one flat loop over table entries with no index
+//     arithmetic; the next entry is fetched one step ahead.
 //   * x direction: scatter form.  When plane xl arrives its value u adds w_x[|j|] u to the seven
 //     in-flight output accumulators xl-3..xl+3 held in REGISTERS; output xl-3 is then complete
 //     and is stored (streaming store).  The accumulator slots rotate by compile-time index
@@ -21,8 +22,11 @@
 //   * y and z directions: read from the shared-memory tile of the centre plane.  Each thread owns
 //     a micro tile of TY rows x TC 16-byte chunks (real: 4 rows x 2 points, complex: 2 rows x 2
 //     points) to amortise halo reads.
+//   * The row length is a template parameter for the common grids (ROWD doubles per z row; 0 =
+//     run time), so every shared-memory and store address of a step is base register + immediate.
 //   * The warp that is last to release a ring slot refills it (election by a shared-memory
-//     counter), so no warp ever waits for the others in order to issue a load.
+//     counter whose result is consumed only at the end of the step), so no warp ever waits for
+//     the others in order to issue a load.
 //   * Boundaries are resolved while staging / addressing, never by a padded copy:
 //       periodic y  -> the wrapped halo rows are a separate bulk copy from the other end;
 //       zero y      -> those shared-memory rows are zeroed once and never overwritten;
@@ -31,18 +35,31 @@
 //       periodic x  -> the table's prologue/epilogue entries load planes from the other end;
 //       zero x      -> those entries carry no load (the value is taken as zero);
 //       Bloch phase -> multiply only wrapped rows / chunks / planes (complex128 only).
-//   * Persistent teams: the (band, x) planes are split evenly over the resident teams of
-//     nytiles CTAs.  A team is a thread-block cluster; its CTAs sweep the same planes for adjacent
-//     y-tiles and are kept within one step of each other by a split cluster barrier, so the
-//     y-halo rows they share are fetched from HBM once and hit L2 the second time.
+//   * Persistent teams: the (band, x) planes are split evenly over sm_count / nytiles teams of
+//     nytiles CTAs (one CTA per SM, plain launch, no cluster: 147 of 148 SMs for 3 tiles).  The
+//     CTAs of a team sweep the same planes for adjacent y-tiles; the y-halo rows they share are
+//     fetched from HBM once and hit L2 the second time.  Nothing synchronises the CTAs of a
+//     team: a CTA that falls behind finds its halo rows in L2 (its neighbours loaded them), runs
+//     faster and catches up, so the drift stays far below what the 126 MB L2 retains (measured:
+//     DRAM reads 1.92 GB against 1.82 GB algorithmic on the 96^3 x 256 workload).  A progress
+//     throttle through global memory was tried and removed: its polls sit behind the bulk
+//     traffic in the memory system and cost more than 2x (profiles/r1c notes).
+//   * L2 policy: planes that the periodic x wrap reads twice (the first and last three of a band)
+//     are loaded evict_last the first time, as is v_eff (shared by all bands).
 #include "fd_internal.h"
 
 namespace {
 
 constexpr int kMaxThreads = 384;
 constexpr int kMaxStages = 8;
-constexpr int kCtlBytes = 256;   // full[8] + empty[8] mbarriers + 8 election counters
+constexpr int kCtlBytes = 256;   // full[8] + empty[8] mbarriers, 8 election counters, misc
 constexpr int kSmemMax = 227 * 1024;
+
+// step-table flags (int4 .w)
+constexpr int kWrapLo = 1;   // plane wrapped from below 0: Bloch factor conj(ph_x)
+constexpr int kWrapHi = 2;   // plane wrapped from past nx-1: Bloch factor ph_x
+constexpr int kKeepL2 = 4;   // load evict_last: the x wrap reads this plane again
+constexpr int kZero = 8;     // no data: the plane lies outside a zero-BC x axis
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p)
 {
@@ -88,34 +105,42 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t
         ::"r"(dst), "l"(src), "r"(bytes), "r"(bar)
         : "memory");
 }
-__device__ __forceinline__ void cluster_arrive()
+__device__ __forceinline__ void bulk_g2s_hint(uint32_t dst, const void *src, uint32_t bytes,
+                                              uint32_t bar, unsigned long long policy)
 {
-    asm volatile("barrier.cluster.arrive.relaxed.aligned;" ::: "memory");
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint "
+        "[%0], [%1], %2, [%3], %4;"
+        ::"r"(dst), "l"(src), "r"(bytes), "r"(bar), "l"(policy)
+        : "memory");
 }
-__device__ __forceinline__ void cluster_wait()
+__device__ __forceinline__ unsigned long long policy_evict_last()
 {
-    asm volatile("barrier.cluster.wait.aligned;" ::: "memory");
+    unsigned long long p;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+// one lane of the (converged) warp
+__device__ __forceinline__ bool elect_one()
+{
+    uint32_t p;
+    asm volatile(
+        "{\n"
+        ".reg .pred P;\n"
+        "elect.sync _|P, 0xffffffff;\n"
+        "selp.u32 %0, 1, 0, P;\n"
+        "}\n"
+        : "=r"(p));
+    return p != 0;
 }
 
-__device__ __forceinline__ double2 lds128(uint32_t addr)
+__device__ __forceinline__ double2 lds128(const unsigned char *p)
 {
-    double2 v;
-    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr));
-    return v;
+    return *reinterpret_cast<const double2 *>(p);
 }
-__device__ __forceinline__ double lds64(uint32_t addr)
+__device__ __forceinline__ double lds64(const unsigned char *p)
 {
-    double v;
-    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr));
-    return v;
-}
-__device__ __forceinline__ int4 lds_i4(uint32_t addr)
-{
-    int4 v;
-    asm volatile("ld.shared.v4.s32 {%0, %1, %2, %3}, [%4];"
-                 : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w)
-                 : "r"(addr));
-    return v;
+    return *reinterpret_cast<const double *>(p);
 }
 __device__ __forceinline__ void fma2(double2 &a, double w, const double2 &x)
 {
@@ -152,9 +177,9 @@ struct TeamRange {
         const int nseg = 1 + (int)((rest + nx_ - 1) / nx_);
         nsteps = (int)n + 6 * nseg;
     }
-    // Table entry of step e: x = plane to load (band*nx + x, or -1: no data, value is zero),
-    // y = output plane completed by this step (or -1), z = x index of the plane if it is a centre
-    // plane (y/z taps, v_eff), else -1, w = 0 | +1 (wrapped past the upper x end) | -1 (lower).
+    // Table entry of step e: x = plane to load (band*nx + x, or -1: no load), y = output plane
+    // completed by this step (or -1), z = x index of the plane if it is a centre plane (y/z taps,
+    // v_eff), else -1, w = flags (kWrapLo | kWrapHi | kKeepL2 | kZero).
     __device__ int4 entry(int e, int per_x) const
     {
         int band, x0, len, s;
@@ -177,20 +202,23 @@ struct TeamRange {
         m.w = 0;
         if (xl < 0) {
             m.x = per_x ? band * nx + xl + nx : -1;
-            m.w = per_x ? -1 : 0;
+            m.w = per_x ? kWrapLo : kZero;
         } else if (xl >= nx) {
             m.x = per_x ? band * nx + xl - nx : -1;
-            m.w = per_x ? 1 : 0;
+            m.w = per_x ? kWrapHi : kZero;
         } else {
             m.x = band * nx + xl;
         }
+        // a whole periodic band: its last three planes (read first, as the wrap) and its first
+        // three come round again ~nx steps later
+        if (per_x && x0 == 0 && len == nx && s < 6) m.w |= kKeepL2;
         m.y = (s >= 6) ? band * nx + x0 + s - 6 : -1;
         m.z = (s >= 3 && s < len + 3) ? xl : -1;
         return m;
     }
 };
 
-template <bool CPLX, bool HAS_V>
+template <bool CPLX, bool HAS_V, int ROWD>
 __global__ void __launch_bounds__(kMaxThreads, 1)
 fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSweepCfg cfg,
                 const double *__restrict__ psi, const double *__restrict__ v_eff,
@@ -206,20 +234,20 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
     const uint32_t full_bar = smem_base;         // kMaxStages x 8 bytes
     const uint32_t empty_bar = smem_base + 64;   // kMaxStages x 8 bytes
     unsigned int *const elect_cnt = reinterpret_cast<unsigned int *>(smem + 128);
-    const uint32_t tab = smem_base + (uint32_t)cfg.tab_off;
+    unsigned long long *const l2pol = reinterpret_cast<unsigned long long *>(smem + 168);
+    const int4 *const tabp = reinterpret_cast<const int4 *>(smem + cfg.tab_off);
+    const unsigned char *const stage0p = smem + cfg.stage_off;
     const uint32_t stage0 = smem_base + (uint32_t)cfg.stage_off;
     const uint32_t stage_bytes = (uint32_t)cfg.stage_bytes;
     const int K = cfg.stages;
 
     const int nx = g.n[0], ny = g.n[1], nz = g.n[2];
-    const int pitch = nz * (CPLX ? 16 : 8);  // bytes per z row of psi
-    const int pitchv = nz * 8;               // bytes per z row of v_eff
-    const int cpr = pitch >> 4;              // 16-byte chunks per row
-    const int rowd = pitch >> 3;             // doubles per row
+    const int rowd = ROWD ? ROWD : nz * (CPLX ? 2 : 1);  // doubles per z row of psi
+    const int pitch = rowd * 8;                          // bytes per z row of psi
+    const int pitchv = CPLX ? pitch / 2 : pitch;         // bytes per z row of v_eff
+    const int cpr = rowd >> 1;                           // 16-byte chunks per row
     const int tid = threadIdx.x;
-    const int lane = tid & 31;
     const unsigned nwarps = blockDim.x >> 5;
-    const bool clustered = cfg.cluster > 1;
 
     const int yt = (int)(blockIdx.x % (unsigned)cfg.nytiles);
     const long long team = blockIdx.x / (unsigned)cfg.nytiles;
@@ -227,7 +255,7 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
     const int rows_valid = min(cfg.tyc, ny - y0);
     const long long L0 = team * (long long)quota;
     const long long L1 = (L0 + quota < total_planes) ? (L0 + quota) : total_planes;
-    if (L0 >= L1) return;  // the whole team (cluster) exits together
+    if (L0 >= L1) return;
 
     // ---- y segments of the staged tile: smem row R <-> global row y0 - 3 + R ------------------
     const int per_y = g.bc[1], per_x = g.bc[0], per_z = g.bc[2];
@@ -237,6 +265,7 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
     const uint32_t zb = (uint32_t)cfg.zb_bytes;
     const uint32_t tx_psi = (uint32_t)((nmid + (per_y ? nlo + nhi : 0)) * pitch);
     const uint32_t tx_v = (uint32_t)(rows_valid * pitchv);
+    const long long plane_d = (long long)ny * rowd;  // doubles per x plane of psi / out
 
     TeamRange tr;
     tr.init(L0, L1, nx);
@@ -249,10 +278,12 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
             mbar_init(empty_bar + 8 * i, nwarps);
             elect_cnt[i] = 0;
         }
+        l2pol[0] = policy_evict_last();
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    for (int e = tid; e < nsteps; e += blockDim.x)
-        reinterpret_cast<int4 *>(smem + cfg.tab_off)[e] = tr.entry(e, per_x);
+    for (int e = tid; e <= nsteps; e += blockDim.x)  // one entry past the end: prefetched, unused
+        reinterpret_cast<int4 *>(smem + cfg.tab_off)[e] =
+            (e < nsteps) ? tr.entry(e, per_x) : make_int4(-1, -1, -1, kZero);
     for (int st = 0; st < K; ++st) {
         unsigned char *sb = smem + cfg.stage_off + (size_t)st * stage_bytes;
         for (int i = tid; i < (int)(zb >> 3); i += blockDim.x)  // the zero block
@@ -270,27 +301,38 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     __syncthreads();
 
-    // ---- the load of table entry e into ring slot st (one thread) ------------------------------
-    auto issue = [&](int e, uint32_t st) {
-        const int4 me = lds_i4(tab + 16u * (uint32_t)e);
-        const uint32_t bar = full_bar + 8 * st;
+    // ---- the load of table entry e into ring slot s (one thread) --------------------------------
+    auto issue = [&](int e, uint32_t s) {
+        const int4 me = tabp[e];
+        const uint32_t bar = full_bar + 8 * s;
         if (me.x < 0) {
             mbar_arrive(bar);
             return;
         }
-        const uint32_t dst = stage0 + st * stage_bytes + zb;
-        const double *src = psi + (long long)me.x * ((long long)ny * rowd);
+        const uint32_t dst = stage0 + s * stage_bytes + zb;
+        const double *src = psi + (long long)me.x * plane_d;
         const bool with_v = HAS_V && me.z >= 0;
         mbar_expect_tx(bar, tx_psi + (with_v ? tx_v : 0u));
-        if (per_y && nlo > 0)
-            bulk_g2s(dst, src + (long long)(ny - nlo) * rowd, (uint32_t)(nlo * pitch), bar);
-        bulk_g2s(dst + nlo * pitch, src + (long long)(y0 - 3 + nlo) * rowd, (uint32_t)(nmid * pitch),
-                 bar);
-        if (per_y && nhi > 0)
-            bulk_g2s(dst + (nlo + nmid) * pitch, src, (uint32_t)(nhi * pitch), bar);
+        if (me.w & kKeepL2) {
+            const unsigned long long pol = l2pol[0];
+            if (per_y && nlo > 0)
+                bulk_g2s_hint(dst, src + (long long)(ny - nlo) * rowd, (uint32_t)(nlo * pitch), bar,
+                              pol);
+            bulk_g2s_hint(dst + nlo * pitch, src + (long long)(y0 - 3 + nlo) * rowd,
+                          (uint32_t)(nmid * pitch), bar, pol);
+            if (per_y && nhi > 0)
+                bulk_g2s_hint(dst + (nlo + nmid) * pitch, src, (uint32_t)(nhi * pitch), bar, pol);
+        } else {
+            if (per_y && nlo > 0)
+                bulk_g2s(dst, src + (long long)(ny - nlo) * rowd, (uint32_t)(nlo * pitch), bar);
+            bulk_g2s(dst + nlo * pitch, src + (long long)(y0 - 3 + nlo) * rowd,
+                     (uint32_t)(nmid * pitch), bar);
+            if (per_y && nhi > 0)
+                bulk_g2s(dst + (nlo + nmid) * pitch, src, (uint32_t)(nhi * pitch), bar);
+        }
         if (with_v)
-            bulk_g2s(stage0 + st * stage_bytes + (uint32_t)cfg.v_off,
-                     v_eff + ((long long)me.z * ny + y0) * nz, tx_v, bar);
+            bulk_g2s_hint(stage0 + s * stage_bytes + (uint32_t)cfg.v_off,
+                          v_eff + ((long long)me.z * ny + y0) * nz, tx_v, bar, l2pol[0]);
     };
     if (tid == 0)
         for (int i = 0; i < K && i < nsteps; ++i) issue(i, (uint32_t)i);
@@ -302,12 +344,12 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
     if (!tactive) rg = cfg.rowgroups - 1;  // surplus threads shadow the last row group, never store
     const int r0 = rg * TY;                // first halo row (smem row index) of this thread
     const int zc0 = lz * TC;               // first own chunk in the row
-    const uint32_t own_off = zb + (uint32_t)(r0 * pitch + zc0 * 16);
-    const uint32_t v_off = (uint32_t)cfg.v_off + (uint32_t)(r0 * pitchv + lz * 16);
+    const int own_off = (int)zb + r0 * pitch + zc0 * 16;
+    const int v_off = cfg.v_off + r0 * pitchv + lz * 16;
 
     // halo chunks along z: k < ZH left of the own chunks, k >= ZH right of them; an out-of-range
     // chunk on a zero-BC axis reads the zero block at the start of the stage (offset 0).
-    uint32_t hb[2 * ZH];
+    int hb[2 * ZH];
     int zwrap = 0;  // 2 bits per halo chunk: 1 = wrapped below 0, 2 = wrapped past nz (complex only)
 #pragma unroll
     for (int k = 0; k < 2 * ZH; ++k) {
@@ -318,7 +360,7 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
         } else if (cz >= cpr) {
             if (per_z) { cz -= cpr; zwrap |= 2 << (2 * k); } else valid = false;
         }
-        hb[k] = valid ? zb + (uint32_t)((r0 + 3) * pitch + cz * 16) : 0u;
+        hb[k] = valid ? (int)zb + (r0 + 3) * pitch + cz * 16 : 0;
     }
     const bool zphase = CPLX && per_z && (g.ph_re[2] != 1.0 || g.ph_im[2] != 0.0) && zwrap != 0;
     const bool yphase = CPLX && per_y && (g.ph_re[1] != 1.0 || g.ph_im[1] != 0.0);
@@ -330,7 +372,6 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
     for (int i = 0; i < TY; ++i)
         if (tactive && (r0 + i) < rows_valid) row_ok |= 1u << i;
     double *const obase = out + (long long)(y0 + r0) * rowd + zc0 * 2;
-    const long long plane_d = (long long)ny * rowd;  // doubles per x plane of psi / out
 
     const double wx1 = g.w[0][1], wx2 = g.w[0][2], wx3 = g.w[0][3];
     const double wy1 = g.w[1][1], wy2 = g.w[1][2], wy3 = g.w[1][3];
@@ -345,27 +386,25 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
         for (int p = 0; p < NP; ++p) acc[a][p] = make_double2(0.0, 0.0);
 
     uint32_t st = 0, par = 0;  // ring slot and mbarrier phase parity of the current step
+    int4 m = tabp[0];          // .y out plane, .z centre plane, .w flags of the current step
     for (int q7 = 0; q7 < nsteps; q7 += 7) {
 #pragma unroll
         for (int J = 0; J < 7; ++J) {
             const int q = q7 + J;
             if (q < nsteps) {
-                const int4 m = lds_i4(tab + 16u * (uint32_t)q);
-                if (clustered) {  // keep the team's CTAs within one step of each other
-                    if (q > 0) cluster_wait();
-                    cluster_arrive();
-                }
+                const int4 mn = tabp[q + 1];
                 mbar_wait(full_bar + 8 * st, par);
-                const uint32_t sb = stage0 + st * stage_bytes;
+                const unsigned char *const sb = stage0p + st * stage_bytes;
+                const unsigned char *const ub = sb + own_off;
 
                 // ---- own values of the incoming plane
                 double2 u[NP];
-                if (m.x >= 0) {
+                if (!(m.w & kZero)) {
 #pragma unroll
                     for (int i = 0; i < TY; ++i)
 #pragma unroll
                         for (int t = 0; t < TC; ++t)
-                            u[i * TC + t] = lds128(sb + own_off + (3 + i) * pitch + t * 16);
+                            u[i * TC + t] = lds128(ub + (3 + i) * pitch + t * 16);
                     if (CPLX && yphase) {
                         // rows past a ragged tile end are wrapped rows: neighbours of the last
                         // valid rows, so they carry the y Bloch factor like any halo row
@@ -377,8 +416,8 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
                                     u[i * TC + t] = cmul(u[i * TC + t], g.ph_re[1], g.ph_im[1]);
                             }
                     }
-                    if (CPLX && xphase && m.w != 0) {
-                        const double pi_ = (m.w < 0) ? -g.ph_im[0] : g.ph_im[0];
+                    if (CPLX && xphase && (m.w & (kWrapLo | kWrapHi))) {
+                        const double pi_ = (m.w & kWrapLo) ? -g.ph_im[0] : g.ph_im[0];
 #pragma unroll
                         for (int p = 0; p < NP; ++p) u[p] = cmul(u[p], g.ph_re[0], pi_);
                     }
@@ -397,7 +436,7 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
                         if (row_ok & (1u << i)) {
 #pragma unroll
                             for (int t = 0; t < TC; ++t)
-                                __stcs(reinterpret_cast<double2 *>(o + (long long)i * rowd) + t,
+                                __stcs(reinterpret_cast<double2 *>(o + i * rowd) + t,
                                        acc[(J + 4) % 7][i * TC + t]);
                         }
                 }
@@ -433,7 +472,7 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
                         if (rr >= 3 && rr < 3 + TY) continue;  // own rows: already in u
                         double2 c[TC];
 #pragma unroll
-                        for (int t = 0; t < TC; ++t) c[t] = lds128(sb + own_off + rr * pitch + t * 16);
+                        for (int t = 0; t < TC; ++t) c[t] = lds128(ub + rr * pitch + t * 16);
                         if (CPLX && yphase) {
                             const int R = r0 + rr;
                             if (R < nlo) {
@@ -523,27 +562,31 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
                     }
                 }
 
-                // ---- release the slot; the last warp to do so refills it with step q + K
+                // ---- release the slot; the last warp to do so will refill it with step q + K
+                bool last = false;
                 __syncwarp();
-                if (lane == 0) {
+                if (elect_one()) {
                     mbar_arrive(empty_bar + 8 * st);
-                    if (atomicInc(&elect_cnt[st], nwarps - 1) == nwarps - 1 && q + K < nsteps) {
-                        mbar_wait(empty_bar + 8 * st, par);
-                        issue(q + K, st);
-                    }
-                }
-                if (++st == (uint32_t)K) {
-                    st = 0;
-                    par ^= 1u;
+                    last = atomicInc(&elect_cnt[st], nwarps - 1) == nwarps - 1;
                 }
 
                 // ---- the output three planes ahead is born
 #pragma unroll
                 for (int p = 0; p < NP; ++p) acc[(J + 3) % 7][p] = mul2(wx3, u[p]);
+
+                if (last && q + K < nsteps) {
+                    const int e = q + K;
+                    mbar_wait(empty_bar + 8 * st, par);
+                    issue(e, st);
+                }
+                if (++st == (uint32_t)K) {
+                    st = 0;
+                    par ^= 1u;
+                }
+                m = mn;
             }
         }
     }
-    if (clustered) cluster_wait();
 }
 
 inline int ceil_div(int a, int b) { return (a + b - 1) / b; }
@@ -607,82 +650,52 @@ void fd_sweep_configure(fd_plan *plan, int tyc_override, int xchunk_override)
     c.tab_cap = tab_bytes / 16;
     c.stage_off = kCtlBytes + tab_bytes;
     c.smem_bytes = c.stage_off + stages * c.stage_bytes;
-    c.cluster = (c.nytiles > 1 && c.nytiles <= 8) ? c.nytiles : 1;
     c.max_teams = plan->sm_count / c.nytiles > 0 ? plan->sm_count / c.nytiles : 1;
     if (c.smem_bytes > kSmemMax || c.threads > kMaxThreads) return;
     c.supported = 1;
 }
 
+namespace {
+
+using SweepKernel = void (*)(const FdGeom, const FdSweepCfg, const double *, const double *,
+                             double *, const long long, const int);
+
+// Row lengths (doubles per z row) with a compile-time specialisation; anything else runs the
+// ROWD = 0 (run-time pitch) instantiation.
 template <bool CPLX, bool HAS_V>
-static cudaError_t prepare_one(FdSweepCfg &c, int *max_clusters)
+SweepKernel pick_kernel(int rowd)
 {
-    auto kern = fd_sweep_kernel<CPLX, HAS_V>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         c.smem_bytes);
-    if (e != cudaSuccess || c.cluster <= 1) return e;
-    cudaLaunchConfig_t lc = {};
-    lc.gridDim = dim3((unsigned)(c.cluster * 64));
-    lc.blockDim = dim3((unsigned)c.threads);
-    lc.dynamicSmemBytes = (size_t)c.smem_bytes;
-    cudaLaunchAttribute at[1];
-    at[0].id = cudaLaunchAttributeClusterDimension;
-    at[0].val.clusterDim.x = (unsigned)c.cluster;
-    at[0].val.clusterDim.y = 1;
-    at[0].val.clusterDim.z = 1;
-    lc.attrs = at;
-    lc.numAttrs = 1;
-    int n = 0;
-    e = cudaOccupancyMaxActiveClusters(&n, kern, &lc);
-    if (e != cudaSuccess) {
-        cudaGetLastError();
-        n = 0;
+    switch (rowd) {
+    case 24: return fd_sweep_kernel<CPLX, HAS_V, 24>;
+    case 48: return fd_sweep_kernel<CPLX, HAS_V, 48>;
+    case 64: return fd_sweep_kernel<CPLX, HAS_V, 64>;
+    case 96: return fd_sweep_kernel<CPLX, HAS_V, 96>;
+    case 128: return fd_sweep_kernel<CPLX, HAS_V, 128>;
+    case 144: return fd_sweep_kernel<CPLX, HAS_V, 144>;
+    case 192: return fd_sweep_kernel<CPLX, HAS_V, 192>;
+    default: return fd_sweep_kernel<CPLX, HAS_V, 0>;
     }
-    if (n < *max_clusters) *max_clusters = n;
-    return cudaSuccess;
 }
+
+SweepKernel kernel_for(const fd_plan *plan, bool has_v)
+{
+    const int rowd = plan->g.n[2] * (plan->g.cplx ? 2 : 1);
+    if (plan->g.cplx) return has_v ? pick_kernel<true, true>(rowd) : pick_kernel<true, false>(rowd);
+    return has_v ? pick_kernel<false, true>(rowd) : pick_kernel<false, false>(rowd);
+}
+
+}  // namespace
 
 cudaError_t fd_sweep_prepare(fd_plan *plan)
 {
-    FdSweepCfg &c = plan->sweep;
-    int max_clusters = 1 << 30;
-    cudaError_t e;
-    if (plan->g.cplx) {
-        if ((e = prepare_one<true, false>(c, &max_clusters)) != cudaSuccess) return e;
-        if ((e = prepare_one<true, true>(c, &max_clusters)) != cudaSuccess) return e;
-    } else {
-        if ((e = prepare_one<false, false>(c, &max_clusters)) != cudaSuccess) return e;
-        if ((e = prepare_one<false, true>(c, &max_clusters)) != cudaSuccess) return e;
-    }
-    if (c.cluster > 1) {
-        if (max_clusters < 1) {  // clusters of this size cannot be resident: plain launch
-            c.cluster = 1;
-        } else {
-            c.max_teams = max_clusters;
-        }
+    const FdSweepCfg &c = plan->sweep;
+    for (int has_v = 0; has_v < 2; ++has_v) {
+        cudaError_t e = cudaFuncSetAttribute(reinterpret_cast<const void *>(kernel_for(plan, has_v)),
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             c.smem_bytes);
+        if (e != cudaSuccess) return e;
     }
     return cudaSuccess;
-}
-
-template <bool CPLX, bool HAS_V>
-static cudaError_t launch_one(const fd_plan *plan, const double *psi, const double *v_eff,
-                              double *out, long long total, int quota, unsigned nblocks,
-                              cudaStream_t stream)
-{
-    const FdSweepCfg &c = plan->sweep;
-    cudaLaunchConfig_t lc = {};
-    lc.gridDim = dim3(nblocks);
-    lc.blockDim = dim3((unsigned)c.threads);
-    lc.dynamicSmemBytes = (size_t)c.smem_bytes;
-    lc.stream = stream;
-    cudaLaunchAttribute at[1];
-    at[0].id = cudaLaunchAttributeClusterDimension;
-    at[0].val.clusterDim.x = (unsigned)c.cluster;
-    at[0].val.clusterDim.y = 1;
-    at[0].val.clusterDim.z = 1;
-    lc.attrs = at;
-    lc.numAttrs = c.cluster > 1 ? 1 : 0;
-    return cudaLaunchKernelEx(&lc, fd_sweep_kernel<CPLX, HAS_V>, plan->g, c, psi, v_eff, out, total,
-                              quota);
 }
 
 cudaError_t fd_launch_sweep(const fd_plan *plan, const void *psi, const double *v_eff, void *out,
@@ -691,6 +704,7 @@ cudaError_t fd_launch_sweep(const fd_plan *plan, const void *psi, const double *
     const FdSweepCfg &c = plan->sweep;
     const FdGeom &g = plan->g;
     const long long band_d = (long long)g.n[0] * g.n[1] * g.n[2] * (g.cplx ? 2 : 1);
+    const SweepKernel kern = kernel_for(plan, v_eff != nullptr);
     // plane indices in the step table are int32: very large batches go out in several launches
     const int64_t bands_per_launch = (1LL << 30) / g.n[0];
     for (int64_t b0 = 0; b0 < nbands; b0 += bands_per_launch) {
@@ -704,8 +718,8 @@ cudaError_t fd_launch_sweep(const fd_plan *plan, const void *psi, const double *
             const int min_quota = g.n[0] < 16 ? g.n[0] : 16;  // below this the 6 halo planes dominate
             if (quota < min_quota) quota = min_quota;
         }
-        // the team's steps (quota + 6 per band touched) must fit the step table
-        const long long quota_cap = ((long long)(c.tab_cap - 12) * g.n[0]) / (g.n[0] + 6);
+        // the team's steps (quota + 6 per band touched, + 1 prefetched entry) must fit the table
+        const long long quota_cap = ((long long)(c.tab_cap - 13) * g.n[0]) / (g.n[0] + 6);
         if (quota > quota_cap) quota = quota_cap;
         if (quota < 1) return cudaErrorInvalidConfiguration;
         const long long nteams = (total + quota - 1) / quota;
@@ -713,15 +727,11 @@ cudaError_t fd_launch_sweep(const fd_plan *plan, const void *psi, const double *
         if (nblocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
         const double *p = static_cast<const double *>(psi) + b0 * band_d;
         double *o = static_cast<double *>(out) + b0 * band_d;
-        cudaError_t e;
-        if (g.cplx)
-            e = v_eff ? launch_one<true, true>(plan, p, v_eff, o, total, (int)quota, (unsigned)nblocks, stream)
-                      : launch_one<true, false>(plan, p, nullptr, o, total, (int)quota, (unsigned)nblocks, stream);
-        else
-            e = v_eff ? launch_one<false, true>(plan, p, v_eff, o, total, (int)quota, (unsigned)nblocks, stream)
-                      : launch_one<false, false>(plan, p, nullptr, o, total, (int)quota, (unsigned)nblocks, stream);
+        kern<<<dim3((unsigned)nblocks), dim3((unsigned)c.threads), (size_t)c.smem_bytes, stream>>>(
+            g, c, p, v_eff, o, total, (int)quota);
+        cudaError_t e = cudaPeekAtLastError();
         if (e != cudaSuccess) return e;
         if (nlaunches) ++*nlaunches;
     }
-    return cudaPeekAtLastError();
+    return cudaSuccess;
 }
