@@ -31,7 +31,7 @@ struct FdSweepCfg {
     int v_off;         // offset of the v_eff rows inside a stage
     int stage_bytes;   // bytes per ring stage
     int tab_off;       // offset of the step table in shared memory
-    int tab_cap;       // step table capacity (entries of 16 bytes)
+    int tab_cap;       // step table capacity (entries of 8 bytes)
     int stage_off;     // offset of stage 0
     int smem_bytes;    // dynamic shared memory per CTA
     int max_teams;     // teams of nytiles CTAs resident at once (one CTA per SM)

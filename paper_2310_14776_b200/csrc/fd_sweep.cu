@@ -20,8 +20,9 @@
 //     and is stored (streaming store).  The accumulator slots rotate by compile-time index
 //     (loop unrolled x7).
 //   * y and z directions: read from the shared-memory tile of the centre plane.  Each thread owns
-//     a micro tile of TY rows x TC 16-byte chunks (real: 4 rows x 2 points, complex: 2 rows x 2
-//     points) to amortise halo reads.
+//     a micro tile of 4 rows x one 16-byte chunk (real: 2 points, complex: 1 point) to amortise
+//     the y-halo reads; consecutive lanes own consecutive chunks, so every 16-byte shared-memory
+//     access of a warp is conflict free (the shared-memory data pipe is what bounds this kernel).
 //   * The row length is a template parameter for the common grids (ROWD doubles per z row; 0 =
 //     run time), so every shared-memory and store address of a step is base register + immediate.
 //   * The warp that is last to release a ring slot refills it (election by a shared-memory
@@ -55,11 +56,16 @@ constexpr int kMaxStages = 8;
 constexpr int kCtlBytes = 256;   // full[8] + empty[8] mbarriers, 8 election counters, misc
 constexpr int kSmemMax = 227 * 1024;
 
-// step-table flags (int4 .w)
-constexpr int kWrapLo = 1;   // plane wrapped from below 0: Bloch factor conj(ph_x)
-constexpr int kWrapHi = 2;   // plane wrapped from past nx-1: Bloch factor ph_x
-constexpr int kKeepL2 = 4;   // load evict_last: the x wrap reads this plane again
-constexpr int kZero = 8;     // no data: the plane lies outside a zero-BC x axis
+// Step-table entry (8 bytes): .x = plane to load (band*nx + x, low kPlaneBits bits) | flags,
+// .y = output plane completed by the step (band*nx + x) or ~0.
+constexpr int kPlaneBits = 26;
+constexpr unsigned kPlaneMask = (1u << kPlaneBits) - 1u;
+constexpr unsigned kWrapLo = 1u << 26;   // plane wrapped from below 0: Bloch factor conj(ph_x)
+constexpr unsigned kWrapHi = 1u << 27;   // plane wrapped from past nx-1: Bloch factor ph_x
+constexpr unsigned kKeepL2 = 1u << 28;   // load evict_last: the x wrap reads this plane again
+constexpr unsigned kZero = 1u << 29;     // no load: the plane lies outside a zero-BC x axis
+constexpr unsigned kCentre = 1u << 30;   // centre plane: y/z taps, diagonal and v_eff this step
+constexpr unsigned kNoPlane = 0xffffffffu;
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p)
 {
@@ -177,10 +183,8 @@ struct TeamRange {
         const int nseg = 1 + (int)((rest + nx_ - 1) / nx_);
         nsteps = (int)n + 6 * nseg;
     }
-    // Table entry of step e: x = plane to load (band*nx + x, or -1: no load), y = output plane
-    // completed by this step (or -1), z = x index of the plane if it is a centre plane (y/z taps,
-    // v_eff), else -1, w = flags (kWrapLo | kWrapHi | kKeepL2 | kZero).
-    __device__ int4 entry(int e, int per_x) const
+    // Table entry of step e (layout above).
+    __device__ uint2 entry(int e, int per_x) const
     {
         int band, x0, len, s;
         if (e < len0 + 6) {
@@ -198,22 +202,19 @@ struct TeamRange {
             len = (rem < (long long)nx) ? (int)rem : nx;
         }
         const int xl = x0 - 3 + s;
-        int4 m;
-        m.w = 0;
+        uint2 m;
         if (xl < 0) {
-            m.x = per_x ? band * nx + xl + nx : -1;
-            m.w = per_x ? kWrapLo : kZero;
+            m.x = per_x ? ((unsigned)(band * nx + xl + nx) | kWrapLo) : kZero;
         } else if (xl >= nx) {
-            m.x = per_x ? band * nx + xl - nx : -1;
-            m.w = per_x ? kWrapHi : kZero;
+            m.x = per_x ? ((unsigned)(band * nx + xl - nx) | kWrapHi) : kZero;
         } else {
-            m.x = band * nx + xl;
+            m.x = (unsigned)(band * nx + xl);
         }
         // a whole periodic band: its last three planes (read first, as the wrap) and its first
         // three come round again ~nx steps later
-        if (per_x && x0 == 0 && len == nx && s < 6) m.w |= kKeepL2;
-        m.y = (s >= 6) ? band * nx + x0 + s - 6 : -1;
-        m.z = (s >= 3 && s < len + 3) ? xl : -1;
+        if (per_x && x0 == 0 && len == nx && s < 6) m.x |= kKeepL2;
+        if (s >= 3 && s < len + 3) m.x |= kCentre;
+        m.y = (s >= 6) ? (unsigned)(band * nx + x0 + s - 6) : kNoPlane;
         return m;
     }
 };
@@ -224,8 +225,8 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
                 const double *__restrict__ psi, const double *__restrict__ v_eff,
                 double *__restrict__ out, const long long total_planes, const int quota)
 {
-    constexpr int TY = CPLX ? 2 : 4;   // rows per thread
-    constexpr int TC = CPLX ? 2 : 1;   // 16-byte chunks per thread per row
+    constexpr int TY = 4;              // rows per thread
+    constexpr int TC = 1;              // 16-byte chunks per thread per row (lane stride 16 B)
     constexpr int ZH = CPLX ? 3 : 2;   // halo chunks per side along z
     constexpr int NP = TY * TC;
 
@@ -235,7 +236,7 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
     const uint32_t empty_bar = smem_base + 64;   // kMaxStages x 8 bytes
     unsigned int *const elect_cnt = reinterpret_cast<unsigned int *>(smem + 128);
     unsigned long long *const l2pol = reinterpret_cast<unsigned long long *>(smem + 168);
-    const int4 *const tabp = reinterpret_cast<const int4 *>(smem + cfg.tab_off);
+    const uint2 *const tabp = reinterpret_cast<const uint2 *>(smem + cfg.tab_off);
     const unsigned char *const stage0p = smem + cfg.stage_off;
     const uint32_t stage0 = smem_base + (uint32_t)cfg.stage_off;
     const uint32_t stage_bytes = (uint32_t)cfg.stage_bytes;
@@ -282,8 +283,8 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     for (int e = tid; e <= nsteps; e += blockDim.x)  // one entry past the end: prefetched, unused
-        reinterpret_cast<int4 *>(smem + cfg.tab_off)[e] =
-            (e < nsteps) ? tr.entry(e, per_x) : make_int4(-1, -1, -1, kZero);
+        reinterpret_cast<uint2 *>(smem + cfg.tab_off)[e] =
+            (e < nsteps) ? tr.entry(e, per_x) : make_uint2(kZero, kNoPlane);
     for (int st = 0; st < K; ++st) {
         unsigned char *sb = smem + cfg.stage_off + (size_t)st * stage_bytes;
         for (int i = tid; i < (int)(zb >> 3); i += blockDim.x)  // the zero block
@@ -303,17 +304,17 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
 
     // ---- the load of table entry e into ring slot s (one thread) --------------------------------
     auto issue = [&](int e, uint32_t s) {
-        const int4 me = tabp[e];
+        const unsigned mx = tabp[e].x;
         const uint32_t bar = full_bar + 8 * s;
-        if (me.x < 0) {
+        if (mx & kZero) {
             mbar_arrive(bar);
             return;
         }
         const uint32_t dst = stage0 + s * stage_bytes + zb;
-        const double *src = psi + (long long)me.x * plane_d;
-        const bool with_v = HAS_V && me.z >= 0;
+        const double *src = psi + (long long)(mx & kPlaneMask) * plane_d;
+        const bool with_v = HAS_V && (mx & kCentre);
         mbar_expect_tx(bar, tx_psi + (with_v ? tx_v : 0u));
-        if (me.w & kKeepL2) {
+        if (mx & kKeepL2) {
             const unsigned long long pol = l2pol[0];
             if (per_y && nlo > 0)
                 bulk_g2s_hint(dst, src + (long long)(ny - nlo) * rowd, (uint32_t)(nlo * pitch), bar,
@@ -330,9 +331,11 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
             if (per_y && nhi > 0)
                 bulk_g2s(dst + (nlo + nmid) * pitch, src, (uint32_t)(nhi * pitch), bar);
         }
-        if (with_v)
+        if (with_v) {
+            const int xc = (int)((mx & kPlaneMask) % (unsigned)nx);
             bulk_g2s_hint(stage0 + s * stage_bytes + (uint32_t)cfg.v_off,
-                          v_eff + ((long long)me.z * ny + y0) * nz, tx_v, bar, l2pol[0]);
+                          v_eff + ((long long)xc * ny + y0) * nz, tx_v, bar, l2pol[0]);
+        }
     };
     if (tid == 0)
         for (int i = 0; i < K && i < nsteps; ++i) issue(i, (uint32_t)i);
@@ -345,7 +348,7 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
     const int r0 = rg * TY;                // first halo row (smem row index) of this thread
     const int zc0 = lz * TC;               // first own chunk in the row
     const int own_off = (int)zb + r0 * pitch + zc0 * 16;
-    const int v_off = cfg.v_off + r0 * pitchv + lz * 16;
+    const int v_off = cfg.v_off + r0 * pitchv + lz * (CPLX ? 8 : 16);
 
     // halo chunks along z: k < ZH left of the own chunks, k >= ZH right of them; an out-of-range
     // chunk on a zero-BC axis reads the zero block at the start of the stage (offset 0).
@@ -362,6 +365,10 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
         }
         hb[k] = valid ? (int)zb + (r0 + 3) * pitch + cz * 16 : 0;
     }
+    // real: lanes of odd 8-lane groups fetch z+4 first and z-3 second (see the z taps)
+    const bool swp = !CPLX && (tid & 8) != 0;
+    const int off8a = swp ? hb[2 * ZH - 1] : hb[0] + 8;
+    const int off8b = swp ? hb[0] + 8 : hb[2 * ZH - 1];
     const bool zphase = CPLX && per_z && (g.ph_re[2] != 1.0 || g.ph_im[2] != 0.0) && zwrap != 0;
     const bool yphase = CPLX && per_y && (g.ph_re[1] != 1.0 || g.ph_im[1] != 0.0);
     const bool xphase = CPLX && per_x && (g.ph_re[0] != 1.0 || g.ph_im[0] != 0.0);
@@ -386,20 +393,20 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
         for (int p = 0; p < NP; ++p) acc[a][p] = make_double2(0.0, 0.0);
 
     uint32_t st = 0, par = 0;  // ring slot and mbarrier phase parity of the current step
-    int4 m = tabp[0];          // .y out plane, .z centre plane, .w flags of the current step
+    uint2 m = tabp[0];         // .x flags (| load plane), .y out plane of the current step
     for (int q7 = 0; q7 < nsteps; q7 += 7) {
 #pragma unroll
         for (int J = 0; J < 7; ++J) {
             const int q = q7 + J;
             if (q < nsteps) {
-                const int4 mn = tabp[q + 1];
+                const uint2 mn = tabp[q + 1];
                 mbar_wait(full_bar + 8 * st, par);
                 const unsigned char *const sb = stage0p + st * stage_bytes;
                 const unsigned char *const ub = sb + own_off;
 
                 // ---- own values of the incoming plane
                 double2 u[NP];
-                if (!(m.w & kZero)) {
+                if (!(m.x & kZero)) {
 #pragma unroll
                     for (int i = 0; i < TY; ++i)
 #pragma unroll
@@ -416,8 +423,8 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
                                     u[i * TC + t] = cmul(u[i * TC + t], g.ph_re[1], g.ph_im[1]);
                             }
                     }
-                    if (CPLX && xphase && (m.w & (kWrapLo | kWrapHi))) {
-                        const double pi_ = (m.w & kWrapLo) ? -g.ph_im[0] : g.ph_im[0];
+                    if (CPLX && xphase && (m.x & (kWrapLo | kWrapHi))) {
+                        const double pi_ = (m.x & kWrapLo) ? -g.ph_im[0] : g.ph_im[0];
 #pragma unroll
                         for (int p = 0; p < NP; ++p) u[p] = cmul(u[p], g.ph_re[0], pi_);
                     }
@@ -429,7 +436,7 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
                 // ---- x taps, oldest output first: it is complete after this and leaves
 #pragma unroll
                 for (int p = 0; p < NP; ++p) fma2(acc[(J + 4) % 7][p], wx3, u[p]);
-                if (m.y >= 0) {
+                if (m.y != kNoPlane) {
                     double *o = obase + (long long)m.y * plane_d;
 #pragma unroll
                     for (int i = 0; i < TY; ++i)
@@ -448,23 +455,23 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
                     fma2(acc[(J + 2) % 7][p], wx2, u[p]);
                 }
 
-                if (m.z >= 0) {
+                if (m.x & kCentre) {
                     // ---- diagonal (+ v_eff)
 #pragma unroll
                     for (int i = 0; i < TY; ++i) {
                         double d0 = wdiag, d1 = wdiag;
                         if (HAS_V) {
-                            const double2 vv = lds128(sb + v_off + i * pitchv);
-                            d0 += vv.x;
-                            d1 += vv.y;
+                            if constexpr (CPLX) {
+                                d0 += lds64(sb + v_off + i * pitchv);
+                                d1 = d0;
+                            } else {
+                                const double2 vv = lds128(sb + v_off + i * pitchv);
+                                d0 += vv.x;
+                                d1 += vv.y;
+                            }
                         }
-                        if constexpr (CPLX) {
-                            fma2(acc[J][i * TC + 0], d0, u[i * TC + 0]);
-                            fma2(acc[J][i * TC + (TC - 1)], d1, u[i * TC + (TC - 1)]);
-                        } else {
-                            acc[J][i].x = fma(d0, u[i].x, acc[J][i].x);
-                            acc[J][i].y = fma(d1, u[i].y, acc[J][i].y);
-                        }
+                        acc[J][i].x = fma(d0, u[i].x, acc[J][i].x);
+                        acc[J][i].y = fma(d1, u[i].y, acc[J][i].y);
                     }
                     // ---- y taps: stream the TY + 6 rows of the thread's column through
 #pragma unroll
@@ -511,6 +518,7 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
 #pragma unroll
                     for (int i = 0; i < TY; ++i) {
                         if constexpr (CPLX) {
+                            // chunk = one complex point; hz = L3,L2,L1,R1,R2,R3
                             double2 hz[2 * ZH];
 #pragma unroll
                             for (int k = 0; k < 2 * ZH; ++k) hz[k] = lds128(sb + hb[k] + i * pitch);
@@ -522,28 +530,25 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
                                     if (wbits == 2) hz[k] = cmul(hz[k], g.ph_re[2], g.ph_im[2]);
                                 }
                             }
-                            // chunks are complex points: own C0,C1; hz = L3,L2,L1,R1,R2,R3
-                            double2 &a0 = acc[J][i * TC + 0];
-                            double2 &a1 = acc[J][i * TC + (TC - 1)];
-                            const double2 C0 = u[i * TC + 0], C1 = u[i * TC + (TC - 1)];
-                            fma2(a0, wz1, hz[ZH - 1]);
-                            fma2(a0, wz1, C1);
-                            fma2(a0, wz2, hz[ZH - 2]);
-                            fma2(a0, wz2, hz[ZH]);
-                            fma2(a0, wz3, hz[0]);
-                            fma2(a0, wz3, hz[ZH + 1]);
-                            fma2(a1, wz1, C0);
-                            fma2(a1, wz1, hz[ZH]);
-                            fma2(a1, wz2, hz[ZH - 1]);
-                            fma2(a1, wz2, hz[ZH + 1]);
-                            fma2(a1, wz3, hz[ZH - 2]);
-                            fma2(a1, wz3, hz[2 * ZH - 1]);
+                            double2 &a = acc[J][i];
+                            fma2(a, wz1, hz[2]);
+                            fma2(a, wz1, hz[3]);
+                            fma2(a, wz2, hz[1]);
+                            fma2(a, wz2, hz[4]);
+                            fma2(a, wz3, hz[0]);
+                            fma2(a, wz3, hz[5]);
                         } else {
-                            // chunk = points (z, z+1); halo = z-3 | z-2,z-1 | z+2,z+3 | z+4
-                            const double l3 = lds64(sb + hb[0] + i * pitch + 8);
+                            // chunk = points (z, z+1); halo = z-3 | z-2,z-1 | z+2,z+3 | z+4.
+                            // The two 8-byte halo words come in two loads whose lanes alternate
+                            // (by groups of 8) between z-3 and z+4, so each half warp touches 32
+                            // distinct banks (an 8-byte load at a 16-byte lane stride would be a
+                            // 2-way bank conflict).
+                            const double e0 = lds64(sb + off8a + i * pitch);
+                            const double e1 = lds64(sb + off8b + i * pitch);
+                            const double l3 = swp ? e1 : e0;
+                            const double r4 = swp ? e0 : e1;
                             const double2 l21 = lds128(sb + hb[1] + i * pitch);
                             const double2 r23 = lds128(sb + hb[2] + i * pitch);
-                            const double r4 = lds64(sb + hb[3] + i * pitch);
                             double2 &a = acc[J][i];
                             const double2 o = u[i];
                             a.x = fma(wz1, l21.y, a.x);
@@ -601,8 +606,8 @@ void fd_sweep_configure(fd_plan *plan, int tyc_override, int xchunk_override)
     c.xchunk = xchunk_override;  // 0 = automatic (persistent teams), else planes per team
     if (g.nn != 3) return;
     if (g.n[0] < 8 || g.n[1] < 8 || g.n[2] < 8 || (g.n[2] & 1)) return;
-    c.ty = g.cplx ? 2 : 4;
-    c.tc = g.cplx ? 2 : 1;
+    c.ty = 4;
+    c.tc = 1;
     const int pitch = g.n[2] * (g.cplx ? 16 : 8);
     const int pitchv = g.n[2] * 8;
     c.lanes = (pitch / 16) / c.tc;
@@ -612,7 +617,7 @@ void fd_sweep_configure(fd_plan *plan, int tyc_override, int xchunk_override)
     auto stage_bytes = [&](int tyc) {
         return (c.zb_bytes + (tyc + 6) * pitch + tyc * pitchv + 127) / 128 * 128;
     };
-    // fewest y tiles whose stage fits a ring of >= 3 slots beside a 4 KiB step table
+    // fewest y tiles whose stage fits a ring of >= 3 slots beside a 4 KiB (512-step) table
     int tyc = 0;
     const int first = ceil_div(g.n[1], max_rg * c.ty);
     for (int ntiles = first; ntiles <= g.n[1]; ++ntiles) {
@@ -647,7 +652,7 @@ void fd_sweep_configure(fd_plan *plan, int tyc_override, int xchunk_override)
     tab_bytes = (kSmemMax - kCtlBytes - stages * c.stage_bytes) / 128 * 128;
     if (tab_bytes > 65536) tab_bytes = 65536;
     c.tab_off = kCtlBytes;
-    c.tab_cap = tab_bytes / 16;
+    c.tab_cap = tab_bytes / 8;
     c.stage_off = kCtlBytes + tab_bytes;
     c.smem_bytes = c.stage_off + stages * c.stage_bytes;
     c.max_teams = plan->sm_count / c.nytiles > 0 ? plan->sm_count / c.nytiles : 1;
@@ -705,8 +710,9 @@ cudaError_t fd_launch_sweep(const fd_plan *plan, const void *psi, const double *
     const FdGeom &g = plan->g;
     const long long band_d = (long long)g.n[0] * g.n[1] * g.n[2] * (g.cplx ? 2 : 1);
     const SweepKernel kern = kernel_for(plan, v_eff != nullptr);
-    // plane indices in the step table are int32: very large batches go out in several launches
-    const int64_t bands_per_launch = (1LL << 30) / g.n[0];
+    // plane indices in the step table have kPlaneBits bits: very large batches go out in several
+    // launches
+    const int64_t bands_per_launch = (1LL << kPlaneBits) / g.n[0];
     for (int64_t b0 = 0; b0 < nbands; b0 += bands_per_launch) {
         const int64_t nb = (nbands - b0 < bands_per_launch) ? nbands - b0 : bands_per_launch;
         const long long total = (long long)nb * g.n[0];
