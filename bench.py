@@ -35,7 +35,10 @@ DEFAULT_WORKLOAD = "cfg3"
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the sweep kernel from the committed
 # `ncu --set full` capture (profiles/), keyed by workload; None until a capture exists.
-NCU_TRAFFIC_BYTES = {}
+NCU_TRAFFIC_BYTES = {
+    # profiles/r1f_sweep_cfg3_ncu_full.md: 1.928 GB read + 1.774 GB written per launch
+    "cfg3_96c_periodic_f64": 3702005000,
+}
 
 
 def _measured_peak_gbs():
