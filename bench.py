@@ -223,7 +223,7 @@ def run_ours(args):
     plan = fd.fd_create(cfg.shape, cfg.h, cfg.nn, cfg.bc, cfg.k if cfg.complex else None,
                         fd.FD_C128 if cfg.complex else fd.FD_F64, local)
     kernel = {fd.FD_KERNEL_SWEEP: "sweep", fd.FD_KERNEL_GENERIC: "generic"}[
-        fd.fd_plan_get_kernel(plan)]
+        fd.fd_plan_kernel_for(plan, cfg.nbands)]
     stream = torch.cuda.Stream()
 
     def sync_all():

@@ -125,11 +125,14 @@ FD_API const char *fd_strerror(int status);
 /* Diagnostics (not on the hot path).
  * fd_plan_set_kernel: force a kernel family (FD_ERR_UNSUPPORTED if the plan cannot run it);
  *   with `param` != 0 overriding the family's tile parameter (sweep: y rows per CTA).
- * fd_plan_get_kernel: family the next apply will launch.
+ * fd_plan_get_kernel: family of the plan (the sweep family hands batches that are far too small
+ *   to fill its persistent CTAs to the generic kernel unless it was forced).
+ * fd_plan_kernel_for: family an apply of `nbands` bands will launch.
  * fd_plan_launches: kernels launched by this plan so far (for bench.py's gpu_launches).
  * fd_plan_get_weights: the 3*(nn+1) doubles w_d[j] = -1/2 c_j / h_d^2 (d-major) the kernels use. */
 FD_API int fd_plan_set_kernel(fd_plan *plan, int32_t kernel, int32_t param);
 FD_API int fd_plan_get_kernel(const fd_plan *plan);
+FD_API int fd_plan_kernel_for(const fd_plan *plan, int64_t nbands);
 FD_API int64_t fd_plan_launches(const fd_plan *plan);
 FD_API int fd_plan_get_weights(const fd_plan *plan, double *w, int32_t capacity);
 

@@ -42,7 +42,8 @@ struct fd_plan {
     FdGeom g;
     int device;
     int sm_count;
-    int kernel;        // FD_KERNEL_GENERIC | FD_KERNEL_SWEEP actually used
+    int kernel;        // FD_KERNEL_GENERIC | FD_KERNEL_SWEEP: family of the plan
+    int forced;        // 1: set explicitly (fd_plan_set_kernel / FDHAM_TUNE), no per-batch choice
     FdSweepCfg sweep;
     double h[3];
     double k[3];

@@ -24,7 +24,7 @@ LIB_PATH = os.path.join(_HERE, "libfdham.so")
 
 EXPORTED_SYMBOLS = [
     "fd_create", "fd_apply_kinetic", "fd_apply_hamiltonian", "fd_apply_hamiltonian_host",
-    "fd_destroy", "fd_strerror", "fd_plan_set_kernel", "fd_plan_get_kernel", "fd_plan_launches",
+    "fd_destroy", "fd_strerror", "fd_plan_set_kernel", "fd_plan_get_kernel", "fd_plan_kernel_for", "fd_plan_launches",
     "fd_plan_get_weights",
 ]
 
@@ -66,6 +66,8 @@ def load_library() -> ctypes.CDLL:
     lib.fd_plan_set_kernel.restype = ctypes.c_int
     lib.fd_plan_get_kernel.argtypes = [vp]
     lib.fd_plan_get_kernel.restype = ctypes.c_int
+    lib.fd_plan_kernel_for.argtypes = [vp, i64]
+    lib.fd_plan_kernel_for.restype = ctypes.c_int
     lib.fd_plan_launches.argtypes = [vp]
     lib.fd_plan_launches.restype = ctypes.c_int64
     lib.fd_plan_get_weights.argtypes = [vp, f64p, i32]
@@ -156,6 +158,10 @@ def fd_plan_set_kernel(plan, kernel: int, param: int = 0) -> None:
 
 def fd_plan_get_kernel(plan) -> int:
     return int(load_library().fd_plan_get_kernel(plan))
+
+
+def fd_plan_kernel_for(plan, nbands: int) -> int:
+    return int(load_library().fd_plan_kernel_for(plan, int(nbands)))
 
 
 def fd_plan_launches(plan) -> int:

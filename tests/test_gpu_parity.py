@@ -30,11 +30,20 @@ def fd():
 
 
 def gpu_apply(fd, cfg, psi, v, kernel=None, kinetic=False, tyc=0):
-    """psi, v: numpy arrays; returns numpy H psi computed by libfdham on cuda:0."""
+    """psi, v: numpy arrays; returns numpy H psi computed by libfdham on cuda:0.
+
+    kernel: a FD_KERNEL_* family to force, "auto" for the plan's own per-batch choice, or None =
+    the sweep kernel wherever the plan supports it (the kernel under test; small batches would
+    otherwise be handed to the generic kernel), else the generic one."""
     plan = fd.fd_create(cfg.shape, cfg.h, cfg.nn, cfg.bc, cfg.k if cfg.complex else None,
                         fd.FD_C128 if cfg.complex else fd.FD_F64, 0)
     try:
-        if kernel is not None:
+        if kernel is None:
+            try:
+                fd.fd_plan_set_kernel(plan, fd.FD_KERNEL_SWEEP, tyc)
+            except fd.FDError:
+                fd.fd_plan_set_kernel(plan, fd.FD_KERNEL_GENERIC, 0)
+        elif kernel != "auto":
             fd.fd_plan_set_kernel(plan, kernel, tyc)
         d_psi = torch.from_numpy(psi).cuda()
         d_out = torch.full_like(d_psi, float("nan"))
@@ -43,7 +52,7 @@ def gpu_apply(fd, cfg, psi, v, kernel=None, kinetic=False, tyc=0):
         else:
             fd.fd_apply_hamiltonian(plan, d_psi, torch.from_numpy(v).cuda(), d_out)
         torch.cuda.synchronize()
-        used = fd.fd_plan_get_kernel(plan)
+        used = fd.fd_plan_kernel_for(plan, psi.shape[0])
         return d_out.cpu().numpy(), used
     finally:
         fd.fd_destroy(plan)
@@ -62,13 +71,17 @@ def check(oracle, fd, cfg, psi, v, kernel=None, tyc=0):
 # ------------------------------------------------------------------------------ BASELINE configs
 
 @pytest.mark.parametrize("idx", [1, 2])
-@pytest.mark.parametrize("kernel", ["auto", "generic"])
+@pytest.mark.parametrize("kernel", ["auto", "sweep", "generic"])
 def test_small_configs_full_compare(oracle, fd, idx, kernel):
     cfg = W.get(idx)
     psi, v = W.make_psi(cfg), W.make_veff(cfg)
-    used = check(oracle, fd, cfg, psi, v, None if kernel == "auto" else fd.FD_KERNEL_GENERIC)
+    forced = {"auto": "auto", "sweep": fd.FD_KERNEL_SWEEP, "generic": fd.FD_KERNEL_GENERIC}[kernel]
+    used = check(oracle, fd, cfg, psi, v, forced)
     if kernel == "auto":
-        assert used == fd.FD_KERNEL_SWEEP     # the bandwidth kernel is the one under test
+        # 24^3 x 8 bands cannot fill the persistent teams: the plan hands it to the generic kernel
+        assert used == (fd.FD_KERNEL_GENERIC if idx == 1 else fd.FD_KERNEL_SWEEP)
+    else:
+        assert used == forced
 
 
 def _big_config_check(oracle, fd, cfg, full_bands, chunk=32, nsample=4000):
@@ -144,7 +157,8 @@ SWEEP_SHAPES = [(8, 8, 8), (9, 8, 10), (8, 17, 12), (33, 10, 8), (12, 50, 14), (
 def test_shape_sweep_all_bc_combinations_real(oracle, fd, shape):
     for bc in itertools.product((0, 1), repeat=3):
         cfg = W.custom(shape, (0.2, 0.23, 0.17), bc, nbands=3)
-        check(oracle, fd, cfg, W.make_psi(cfg), W.make_veff(cfg))
+        used = check(oracle, fd, cfg, W.make_psi(cfg), W.make_veff(cfg), fd.FD_KERNEL_SWEEP)
+        assert used == fd.FD_KERNEL_SWEEP
 
 
 @pytest.mark.parametrize("shape", [(8, 8, 8), (9, 12, 10), (8, 23, 12), (20, 10, 36)])
@@ -152,7 +166,8 @@ def test_shape_sweep_complex_bloch(oracle, fd, shape):
     for bc in [(1, 1, 1), (1, 0, 1), (0, 1, 1), (1, 1, 0), (0, 0, 0)]:
         k = tuple(kk if b else 0.0 for kk, b in zip((0.25, 0.125, -0.3), bc))
         cfg = W.custom(shape, (0.2, 0.23, 0.17), bc, k=k, complex_=True, nbands=3)
-        check(oracle, fd, cfg, W.make_psi(cfg), W.make_veff(cfg))
+        used = check(oracle, fd, cfg, W.make_psi(cfg), W.make_veff(cfg), fd.FD_KERNEL_SWEEP)
+        assert used == fd.FD_KERNEL_SWEEP
 
 
 @pytest.mark.parametrize("shape", [(3, 4, 5), (7, 7, 7), (6, 6, 6), (5, 9, 11), (3, 3, 3)])
@@ -160,7 +175,7 @@ def test_generic_fallback_shapes(oracle, fd, shape):
     """odd nz / tiny axes / n = nn / n = 2nn (double hit) run on the generic kernel."""
     for bc in [(1, 1, 1), (0, 1, 0), (0, 0, 0)]:
         cfg = W.custom(shape, (0.2, 0.23, 0.17), bc, nbands=2)
-        used = check(oracle, fd, cfg, W.make_psi(cfg), W.make_veff(cfg))
+        used = check(oracle, fd, cfg, W.make_psi(cfg), W.make_veff(cfg), "auto")
         assert used == fd.FD_KERNEL_GENERIC
         ck = W.custom(shape, (0.2, 0.23, 0.17), bc, complex_=True, nbands=2,
                       k=tuple(0.3 * b for b in bc))
@@ -258,7 +273,7 @@ def test_plane_waves_on_device_closed_form(fd):
                  ((0.25, 0.125, -0.4), (0, 0, 0))]:
         cfg = W.custom(n, h_ang, (1, 1, 1), k=k, complex_=True, nbands=1)
         psi = planewave(n, k, m)[None]
-        got, used = gpu_apply(fd, cfg, psi, None, kinetic=True)
+        got, used = gpu_apply(fd, cfg, psi, None, fd.FD_KERNEL_SWEEP, kinetic=True)
         assert used == fd.FD_KERNEL_SWEEP
         lam = planewave_eig(n, cfg.h, k, m)
         assert np.max(np.abs(got - lam * psi)) <= 1e-12 * kinetic_row_sum(cfg.h)
