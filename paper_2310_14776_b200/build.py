@@ -12,12 +12,13 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 ROOT = os.path.dirname(_HERE)
 LIB = os.path.join(_HERE, "libfdham.so")
-SOURCES = ["fd_api.cu", "fd_generic.cu", "fd_sweep.cu"]
-HEADERS = [os.path.join(CSRC, "fd_internal.h"), os.path.join(ROOT, "include", "fdham.h")]
+SOURCES = ["fd_api.cu", "fd_generic.cu", "fd_sweep.cu", "fd_sweep_inst_real.cu",
+           "fd_sweep_inst_cplx_ph0.cu", "fd_sweep_inst_cplx_ph1.cu", "fd_sweep_inst_cplx_ph3.cu"]
+HEADERS = [os.path.join(CSRC, "fd_internal.h"), os.path.join(CSRC, "fd_sweep_kernel.cuh"),
+           os.path.join(ROOT, "include", "fdham.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-              "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "--use_fast_math"]
-# --use_fast_math only affects single-precision intrinsics; the path is float64 throughout
-NVCC_FLAGS.remove("--use_fast_math")
+              "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden"]
+OBJDIR = os.path.join(_HERE, "build")
 
 
 def _nvcc() -> str:
@@ -36,18 +37,43 @@ def _stale() -> bool:
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
+    """Compile every translation unit (in parallel) and link libfdham.so; no-op when up to date."""
     if not force and not _stale():
         return LIB
-    tmp = LIB + f".tmp{os.getpid()}"
-    cmd = [_nvcc(), *NVCC_FLAGS, "-shared", "-o", tmp, *[os.path.join(CSRC, s) for s in SOURCES]]
-    if verbose:
-        cmd[1:1] = ["-Xptxas", "-v"]
-    res = subprocess.run(cmd, capture_output=True, text=True)
-    if verbose or res.returncode != 0:
-        sys.stderr.write(res.stdout + res.stderr)
-    if res.returncode != 0:
-        raise RuntimeError("nvcc failed building libfdham.so")
-    os.replace(tmp, LIB)
+    from concurrent.futures import ThreadPoolExecutor
+    os.makedirs(OBJDIR, exist_ok=True)
+    nvcc = _nvcc()
+    tag = f".tmp{os.getpid()}"
+
+    def compile_one(src: str):
+        obj = os.path.join(OBJDIR, tag[1:] + "_" + src.replace(".cu", ".o"))
+        cmd = [nvcc, *NVCC_FLAGS, "-c", "-o", obj, os.path.join(CSRC, src)]
+        if verbose:
+            cmd[1:1] = ["-Xptxas", "-v"]
+        return obj, subprocess.run(cmd, capture_output=True, text=True)
+
+    with ThreadPoolExecutor(max_workers=min(len(SOURCES), os.cpu_count() or 1)) as pool:
+        results = list(pool.map(compile_one, SOURCES))
+    failed = False
+    for _, res in results:
+        if verbose or res.returncode != 0:
+            sys.stderr.write(res.stdout + res.stderr)
+        failed |= res.returncode != 0
+    objs = [o for o, _ in results]
+    try:
+        if failed:
+            raise RuntimeError("nvcc failed building libfdham.so")
+        tmp = LIB + tag
+        res = subprocess.run([nvcc, *NVCC_FLAGS, "-shared", "-o", tmp, *objs],
+                             capture_output=True, text=True)
+        if res.returncode != 0:
+            sys.stderr.write(res.stdout + res.stderr)
+            raise RuntimeError("nvcc failed linking libfdham.so")
+        os.replace(tmp, LIB)
+    finally:
+        for o in objs:
+            if os.path.exists(o):
+                os.remove(o)
     return LIB
 
 

@@ -1,0 +1,609 @@
+// fd_sweep_kernel.cuh -- the sweep kernel template (included by the fd_sweep_inst_*.cu translation
+// units, which instantiate it, so that they compile in parallel).
+//
+// Sweep kernel: the bandwidth path of libfdham (nn = 3, i.e. GPAW's default 19-point star).
+//
+// Operation: include/fdham.h -- out = -1/2 lap_FD psi + v_eff psi (Eq. 6 first two terms,
+// PAPER.md:187-188; FD kinetic operator PAPER.md:232; the stencil hot spot PAPER.md:150).
+// Steps a2..a6 of SURVEY 8(a) are all fused here: halo/boundary resolution, the 19 taps, the
+// v_eff multiply-add, the store, and the band-batched tiling.
+//
+// Design:
+//   * A CTA owns one y-tile (tyc rows x the full z row) and sweeps along x.  The y-z tile of each
+//     x plane, with 3 halo rows on either side, and the matching v_eff rows are staged in shared
+//     memory by the TMA unit (cp.async.bulk, completion on an mbarrier) through a ring of
+//     `stages` slots, so HBM reads are deep, asynchronous and fully coalesced (whole rows), and
+//     each psi value crosses HBM once.
+//   * The whole schedule of a CTA (which plane to load, which output plane completes, which
+//     v_eff plane, which Bloch factor, which L2 policy) is a table in shared memory built once at
+//     kernel start: the sweep itself is one flat loop over table entries with no index
+//     arithmetic; the next entry is fetched one step ahead.
+//   * x direction: scatter form.  When plane xl arrives its value u adds w_x[|j|] u to the seven
+//     in-flight output accumulators xl-3..xl+3 held in REGISTERS; output xl-3 is then complete
+//     and is stored (streaming store).  The accumulator slots rotate by compile-time index
+//     (loop unrolled x7).
+//   * y and z directions: read from the shared-memory tile of the centre plane.  Each thread owns
+//     a micro tile of 4 rows x one 16-byte chunk (real: 2 points, complex: 1 point) to amortise
+//     the y-halo reads; consecutive lanes own consecutive chunks, so every 16-byte shared-memory
+//     access of a warp is conflict free (the shared-memory data pipe is what bounds this kernel).
+//   * The row length is a template parameter for the common grids (ROWD doubles per z row; 0 =
+//     run time), so every shared-memory and store address of a step is base register + immediate.
+//   * The warp that is last to release a ring slot refills it (election by a shared-memory
+//     counter whose result is consumed only at the end of the step), so no warp ever waits for
+//     the others in order to issue a load.
+//   * Boundaries are resolved while staging / addressing, never by a padded copy:
+//       periodic y  -> the wrapped halo rows are a separate bulk copy from the other end;
+//       zero y      -> those shared-memory rows are zeroed once and never overwritten;
+//       periodic z  -> per-thread precomputed wrapped chunk offsets inside the row;
+//       zero z      -> the out-of-range chunk address points at a zero block of the stage;
+//       periodic x  -> the table's prologue/epilogue entries load planes from the other end;
+//       zero x      -> those entries carry no load (the value is taken as zero);
+//       Bloch phase -> multiply only wrapped rows / chunks / planes (complex128 only).
+//   * Persistent teams: the (band, x) planes are split evenly over sm_count / nytiles teams of
+//     nytiles CTAs (one CTA per SM, plain launch, no cluster: 147 of 148 SMs for 3 tiles).  The
+//     CTAs of a team sweep the same planes for adjacent y-tiles; the y-halo rows they share are
+//     fetched from HBM once and hit L2 the second time.  Nothing synchronises the CTAs of a
+//     team: a CTA that falls behind finds its halo rows in L2 (its neighbours loaded them), runs
+//     faster and catches up, so the drift stays far below what the 126 MB L2 retains (measured:
+//     DRAM reads 1.92 GB against 1.82 GB algorithmic on the 96^3 x 256 workload).  A progress
+//     throttle through global memory was tried and removed: its polls sit behind the bulk
+//     traffic in the memory system and cost more than 2x (profiles/r1c notes).
+//   * L2 policy: planes that the periodic x wrap reads twice (the first and last three of a band)
+//     are loaded evict_last the first time, as is v_eff (shared by all bands).
+#pragma once
+#include "fd_internal.h"
+
+namespace {
+
+constexpr int kMaxThreads = 384;
+constexpr int kMaxStages = 8;
+constexpr int kCtlBytes = 256;   // full[8] + empty[8] mbarriers, 8 election counters, misc
+constexpr int kSmemMax = 227 * 1024;
+
+// Step-table entry (8 bytes): .x = plane to load (band*nx + x, low kPlaneBits bits) | flags,
+// .y = output plane completed by the step (band*nx + x) or ~0.
+constexpr int kPlaneBits = 26;
+constexpr unsigned kPlaneMask = (1u << kPlaneBits) - 1u;
+constexpr unsigned kWrapLo = 1u << 26;   // plane wrapped from below 0: Bloch factor conj(ph_x)
+constexpr unsigned kWrapHi = 1u << 27;   // plane wrapped from past nx-1: Bloch factor ph_x
+constexpr unsigned kKeepL2 = 1u << 28;   // load evict_last: the x wrap reads this plane again
+constexpr unsigned kZero = 1u << 29;     // no load: the plane lies outside a zero-BC x axis
+constexpr unsigned kCentre = 1u << 30;   // centre plane: y/z taps, diagonal and v_eff this step
+constexpr unsigned kNoPlane = 0xffffffffu;
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p)
+{
+    return static_cast<uint32_t>(__cvta_generic_to_shared(p));
+}
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity)
+{
+    uint32_t ok;
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n"
+        : "=r"(ok)
+        : "r"(bar), "r"(parity)
+        : "memory");
+    return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
+{
+    while (!mbar_try_wait(bar, parity)) {
+    }
+}
+// TMA 1-D bulk copy global -> shared, completion counted in bytes on an mbarrier (SASS: UBLKCP).
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar)
+{
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+        ::"r"(dst), "l"(src), "r"(bytes), "r"(bar)
+        : "memory");
+}
+__device__ __forceinline__ void bulk_g2s_hint(uint32_t dst, const void *src, uint32_t bytes,
+                                              uint32_t bar, unsigned long long policy)
+{
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint "
+        "[%0], [%1], %2, [%3], %4;"
+        ::"r"(dst), "l"(src), "r"(bytes), "r"(bar), "l"(policy)
+        : "memory");
+}
+__device__ __forceinline__ unsigned long long policy_evict_last()
+{
+    unsigned long long p;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+// one lane of the (converged) warp
+__device__ __forceinline__ bool elect_one()
+{
+    uint32_t p;
+    asm volatile(
+        "{\n"
+        ".reg .pred P;\n"
+        "elect.sync _|P, 0xffffffff;\n"
+        "selp.u32 %0, 1, 0, P;\n"
+        "}\n"
+        : "=r"(p));
+    return p != 0;
+}
+
+__device__ __forceinline__ double2 lds128(const unsigned char *p)
+{
+    return *reinterpret_cast<const double2 *>(p);
+}
+__device__ __forceinline__ double lds64(const unsigned char *p)
+{
+    return *reinterpret_cast<const double *>(p);
+}
+__device__ __forceinline__ void fma2(double2 &a, double w, const double2 &x)
+{
+    a.x = fma(w, x.x, a.x);
+    a.y = fma(w, x.y, a.y);
+}
+__device__ __forceinline__ double2 mul2(double w, const double2 &x)
+{
+    return make_double2(w * x.x, w * x.y);
+}
+__device__ __forceinline__ double2 cmul(const double2 &a, double pr, double pi)
+{
+    return make_double2(a.x * pr - a.y * pi, a.x * pi + a.y * pr);
+}
+
+// The linear (band, x) plane range [L0, L1) of a team, cut into segments of one band each:
+// segment 0 = (b0, [x00, x00+len0)), segment k >= 1 = (b0+k, [0, len_k)).  A segment of `len`
+// output planes takes len + 6 steps s = 0..len+5; step s brings in plane xl = x0 - 3 + s.
+struct TeamRange {
+    long long L0, L1;
+    int nx;
+    int b0, x00, len0;
+    int nsteps;
+    __device__ void init(long long l0, long long l1, int nx_)
+    {
+        L0 = l0;
+        L1 = l1;
+        nx = nx_;
+        b0 = (int)(l0 / nx_);
+        x00 = (int)(l0 - (long long)b0 * nx_);
+        const long long n = l1 - l0;
+        len0 = (n < (long long)(nx_ - x00)) ? (int)n : (nx_ - x00);
+        const long long rest = n - len0;
+        const int nseg = 1 + (int)((rest + nx_ - 1) / nx_);
+        nsteps = (int)n + 6 * nseg;
+    }
+    // Table entry of step e (layout above).
+    __device__ uint2 entry(int e, int per_x) const
+    {
+        int band, x0, len, s;
+        if (e < len0 + 6) {
+            band = b0;
+            x0 = x00;
+            len = len0;
+            s = e;
+        } else {
+            const int e2 = e - (len0 + 6);
+            const int k = e2 / (nx + 6);
+            s = e2 - k * (nx + 6);
+            band = b0 + 1 + k;
+            x0 = 0;
+            const long long rem = L1 - (L0 + len0 + (long long)k * nx);
+            len = (rem < (long long)nx) ? (int)rem : nx;
+        }
+        const int xl = x0 - 3 + s;
+        uint2 m;
+        if (xl < 0) {
+            m.x = per_x ? ((unsigned)(band * nx + xl + nx) | kWrapLo) : kZero;
+        } else if (xl >= nx) {
+            m.x = per_x ? ((unsigned)(band * nx + xl - nx) | kWrapHi) : kZero;
+        } else {
+            m.x = (unsigned)(band * nx + xl);
+        }
+        // a whole periodic band: its last three planes (read first, as the wrap) and its first
+        // three come round again ~nx steps later
+        if (per_x && x0 == 0 && len == nx && s < 6) m.x |= kKeepL2;
+        if (s >= 3 && s < len + 3) m.x |= kCentre;
+        m.y = (s >= 6) ? (unsigned)(band * nx + x0 + s - 6) : kNoPlane;
+        return m;
+    }
+};
+
+// PH (complex only): which Bloch-phase code is compiled in -- bit 0: x and y wraps, bit 1: z wraps.
+template <bool CPLX, bool HAS_V, int ROWD, int PH>
+__global__ void __launch_bounds__(kMaxThreads, 1)
+fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSweepCfg cfg,
+                const double *__restrict__ psi, const double *__restrict__ v_eff,
+                double *__restrict__ out, const long long total_planes, const int quota)
+{
+    constexpr int TY = 4;              // rows per thread
+    constexpr int TC = 1;              // 16-byte chunks per thread per row (lane stride 16 B)
+    constexpr int ZH = CPLX ? 3 : 2;   // halo chunks per side along z
+    constexpr int NP = TY * TC;
+
+    extern __shared__ __align__(128) unsigned char smem[];
+    const uint32_t smem_base = smem_u32(smem);
+    const uint32_t full_bar = smem_base;         // kMaxStages x 8 bytes
+    const uint32_t empty_bar = smem_base + 64;   // kMaxStages x 8 bytes
+    unsigned int *const elect_cnt = reinterpret_cast<unsigned int *>(smem + 128);
+    unsigned long long *const l2pol = reinterpret_cast<unsigned long long *>(smem + 168);
+    const uint2 *const tabp = reinterpret_cast<const uint2 *>(smem + cfg.tab_off);
+    const unsigned char *const stage0p = smem + cfg.stage_off;
+    const uint32_t stage0 = smem_base + (uint32_t)cfg.stage_off;
+    const uint32_t stage_bytes = (uint32_t)cfg.stage_bytes;
+    const int K = cfg.stages;
+
+    const int nx = g.n[0], ny = g.n[1], nz = g.n[2];
+    const int rowd = ROWD ? ROWD : nz * (CPLX ? 2 : 1);  // doubles per z row of psi
+    const int pitch = rowd * 8;                          // bytes per z row of psi
+    const int pitchv = CPLX ? pitch / 2 : pitch;         // bytes per z row of v_eff
+    const int cpr = rowd >> 1;                           // 16-byte chunks per row
+    const int tid = threadIdx.x;
+    const unsigned nwarps = blockDim.x >> 5;
+
+    const int yt = (int)(blockIdx.x % (unsigned)cfg.nytiles);
+    const long long team = blockIdx.x / (unsigned)cfg.nytiles;
+    const int y0 = yt * cfg.tyc;
+    const int rows_valid = min(cfg.tyc, ny - y0);
+    const long long L0 = team * (long long)quota;
+    const long long L1 = (L0 + quota < total_planes) ? (L0 + quota) : total_planes;
+    if (L0 >= L1) return;
+
+    // ---- y segments of the staged tile: smem row R <-> global row y0 - 3 + R ------------------
+    const int per_y = g.bc[1], per_x = g.bc[0], per_z = g.bc[2];
+    const int nlo = max(0, 3 - y0);                     // rows below row 0
+    const int nhi = max(0, y0 + rows_valid + 3 - ny);   // rows past row ny-1
+    const int nmid = rows_valid + 6 - nlo - nhi;
+    const uint32_t zb = (uint32_t)cfg.zb_bytes;
+    const uint32_t tx_psi = (uint32_t)((nmid + (per_y ? nlo + nhi : 0)) * pitch);
+    const uint32_t tx_v = (uint32_t)(rows_valid * pitchv);
+    const long long plane_d = (long long)ny * rowd;  // doubles per x plane of psi / out
+
+    TeamRange tr;
+    tr.init(L0, L1, nx);
+    const int nsteps = tr.nsteps;
+
+    // ---- one-time shared memory setup ------------------------------------------------------
+    if (tid == 0) {
+        for (int i = 0; i < K; ++i) {
+            mbar_init(full_bar + 8 * i, 1);
+            mbar_init(empty_bar + 8 * i, nwarps);
+            elect_cnt[i] = 0;
+        }
+        l2pol[0] = policy_evict_last();
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    for (int e = tid; e <= nsteps; e += blockDim.x)  // one entry past the end: prefetched, unused
+        reinterpret_cast<uint2 *>(smem + cfg.tab_off)[e] =
+            (e < nsteps) ? tr.entry(e, per_x) : make_uint2(kZero, kNoPlane);
+    for (int st = 0; st < K; ++st) {
+        unsigned char *sb = smem + cfg.stage_off + (size_t)st * stage_bytes;
+        for (int i = tid; i < (int)(zb >> 3); i += blockDim.x)  // the zero block
+            reinterpret_cast<double *>(sb)[i] = 0.0;
+        double *rows = reinterpret_cast<double *>(sb + zb);
+        if (!per_y) {  // zero halo rows, written once
+            for (int i = tid; i < nlo * rowd; i += blockDim.x) rows[i] = 0.0;
+            for (int i = tid; i < nhi * rowd; i += blockDim.x)
+                rows[(size_t)(nlo + nmid) * rowd + i] = 0.0;
+        }
+        // rows past the ragged end of the last tile are never loaded: define them
+        for (int i = tid; i < (cfg.tyc - rows_valid) * rowd; i += blockDim.x)
+            rows[(size_t)(rows_valid + 6) * rowd + i] = 0.0;
+    }
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    __syncthreads();
+
+    // ---- the load of table entry e into ring slot s (one thread) --------------------------------
+    auto issue = [&](int e, uint32_t s) {
+        const unsigned mx = tabp[e].x;
+        const uint32_t bar = full_bar + 8 * s;
+        if (mx & kZero) {
+            mbar_arrive(bar);
+            return;
+        }
+        const uint32_t dst = stage0 + s * stage_bytes + zb;
+        const double *src = psi + (long long)(mx & kPlaneMask) * plane_d;
+        const bool with_v = HAS_V && (mx & kCentre);
+        mbar_expect_tx(bar, tx_psi + (with_v ? tx_v : 0u));
+        if (mx & kKeepL2) {
+            const unsigned long long pol = l2pol[0];
+            if (per_y && nlo > 0)
+                bulk_g2s_hint(dst, src + (long long)(ny - nlo) * rowd, (uint32_t)(nlo * pitch), bar,
+                              pol);
+            bulk_g2s_hint(dst + nlo * pitch, src + (long long)(y0 - 3 + nlo) * rowd,
+                          (uint32_t)(nmid * pitch), bar, pol);
+            if (per_y && nhi > 0)
+                bulk_g2s_hint(dst + (nlo + nmid) * pitch, src, (uint32_t)(nhi * pitch), bar, pol);
+        } else {
+            if (per_y && nlo > 0)
+                bulk_g2s(dst, src + (long long)(ny - nlo) * rowd, (uint32_t)(nlo * pitch), bar);
+            bulk_g2s(dst + nlo * pitch, src + (long long)(y0 - 3 + nlo) * rowd,
+                     (uint32_t)(nmid * pitch), bar);
+            if (per_y && nhi > 0)
+                bulk_g2s(dst + (nlo + nmid) * pitch, src, (uint32_t)(nhi * pitch), bar);
+        }
+        if (with_v) {
+            const int xc = (int)((mx & kPlaneMask) % (unsigned)nx);
+            bulk_g2s_hint(stage0 + s * stage_bytes + (uint32_t)cfg.v_off,
+                          v_eff + ((long long)xc * ny + y0) * nz, tx_v, bar, l2pol[0]);
+        }
+    };
+    if (tid == 0)
+        for (int i = 0; i < K && i < nsteps; ++i) issue(i, (uint32_t)i);
+
+    // ---- thread -> micro tile ---------------------------------------------------------------
+    int rg = tid / cfg.lanes;
+    const int lz = tid - rg * cfg.lanes;
+    const bool tactive = rg < cfg.rowgroups;
+    if (!tactive) rg = cfg.rowgroups - 1;  // surplus threads shadow the last row group, never store
+    const int r0 = rg * TY;                // first halo row (smem row index) of this thread
+    const int zc0 = lz * TC;               // first own chunk in the row
+    const int own_off = (int)zb + r0 * pitch + zc0 * 16;
+    const int v_off = cfg.v_off + r0 * pitchv + lz * (CPLX ? 8 : 16);
+
+    // halo chunks along z: k < ZH left of the own chunks, k >= ZH right of them; an out-of-range
+    // chunk on a zero-BC axis reads the zero block at the start of the stage (offset 0).
+    int hb[2 * ZH];
+    int zwrap = 0;  // 2 bits per halo chunk: 1 = wrapped below 0, 2 = wrapped past nz (complex only)
+#pragma unroll
+    for (int k = 0; k < 2 * ZH; ++k) {
+        int cz = zc0 + ((k < ZH) ? (k - ZH) : (k - ZH + TC));
+        bool valid = true;
+        if (cz < 0) {
+            if (per_z) { cz += cpr; zwrap |= 1 << (2 * k); } else valid = false;
+        } else if (cz >= cpr) {
+            if (per_z) { cz -= cpr; zwrap |= 2 << (2 * k); } else valid = false;
+        }
+        hb[k] = valid ? (int)zb + (r0 + 3) * pitch + cz * 16 : 0;
+    }
+    // real: lanes of odd 8-lane groups fetch z+4 first and z-3 second (see the z taps)
+    const bool swp = !CPLX && (tid & 8) != 0;
+    const int off8a = swp ? hb[2 * ZH - 1] : hb[0] + 8;
+    const int off8b = swp ? hb[0] + 8 : hb[2 * ZH - 1];
+    const bool zphase = CPLX && (PH & 2) && per_z && (g.ph_re[2] != 1.0 || g.ph_im[2] != 0.0) && zwrap != 0;
+    const bool yphase = CPLX && (PH & 1) && per_y && (g.ph_re[1] != 1.0 || g.ph_im[1] != 0.0);
+    const bool xphase = CPLX && (PH & 1) && per_x && (g.ph_re[0] != 1.0 || g.ph_im[0] != 0.0);
+
+    // only the first row group of tile 0 has wrapped rows below, only row groups reaching past the
+    // last valid row of the last tile have wrapped rows above
+    const bool ylo = yphase && r0 < nlo;
+    const bool yhi = yphase && r0 + TY + 6 > nlo + nmid;
+
+    // store addressing: row i of the micro tile is global row y0 + r0 + i
+    unsigned row_ok = 0;
+#pragma unroll
+    for (int i = 0; i < TY; ++i)
+        if (tactive && (r0 + i) < rows_valid) row_ok |= 1u << i;
+    double *const obase = out + (long long)(y0 + r0) * rowd + zc0 * 2;
+
+    const double wx1 = g.w[0][1], wx2 = g.w[0][2], wx3 = g.w[0][3];
+    const double wy1 = g.w[1][1], wy2 = g.w[1][2], wy3 = g.w[1][3];
+    const double wz1 = g.w[2][1], wz2 = g.w[2][2], wz3 = g.w[2][3];
+    const double wdiag = g.wdiag;
+
+    // ---- the sweep: one flat loop over the step table ------------------------------------------
+    double2 acc[7][NP];
+#pragma unroll
+    for (int a = 0; a < 7; ++a)
+#pragma unroll
+        for (int p = 0; p < NP; ++p) acc[a][p] = make_double2(0.0, 0.0);
+
+    uint32_t st = 0, par = 0;  // ring slot and mbarrier phase parity of the current step
+    uint2 m = tabp[0];         // .x flags (| load plane), .y out plane of the current step
+    for (int q7 = 0; q7 < nsteps; q7 += 7) {
+#pragma unroll
+        for (int J = 0; J < 7; ++J) {
+            const int q = q7 + J;
+            if (q < nsteps) {
+                const uint2 mn = tabp[q + 1];
+                mbar_wait(full_bar + 8 * st, par);
+                const unsigned char *const sb = stage0p + st * stage_bytes;
+                const unsigned char *const ub = sb + own_off;
+
+                // ---- own values of the incoming plane
+                double2 u[NP];
+                if (!(m.x & kZero)) {
+#pragma unroll
+                    for (int i = 0; i < TY; ++i)
+#pragma unroll
+                        for (int t = 0; t < TC; ++t)
+                            u[i * TC + t] = lds128(ub + (3 + i) * pitch + t * 16);
+                    if (CPLX && (PH & 1) && yhi) {
+                        // rows past a ragged tile end are wrapped rows: neighbours of the last
+                        // valid rows, so they carry the y Bloch factor like any halo row
+#pragma unroll
+                        for (int i = 0; i < TY; ++i)
+                            if (r0 + 3 + i >= nlo + nmid) {
+#pragma unroll
+                                for (int t = 0; t < TC; ++t)
+                                    u[i * TC + t] = cmul(u[i * TC + t], g.ph_re[1], g.ph_im[1]);
+                            }
+                    }
+                    if (CPLX && (PH & 1) && xphase && (m.x & (kWrapLo | kWrapHi))) {
+                        const double pi_ = (m.x & kWrapLo) ? -g.ph_im[0] : g.ph_im[0];
+#pragma unroll
+                        for (int p = 0; p < NP; ++p) u[p] = cmul(u[p], g.ph_re[0], pi_);
+                    }
+                } else {
+#pragma unroll
+                    for (int p = 0; p < NP; ++p) u[p] = make_double2(0.0, 0.0);
+                }
+
+                // ---- x taps, oldest output first: it is complete after this and leaves
+#pragma unroll
+                for (int p = 0; p < NP; ++p) fma2(acc[(J + 4) % 7][p], wx3, u[p]);
+                if (m.y != kNoPlane) {
+                    double *o = obase + (long long)m.y * plane_d;
+#pragma unroll
+                    for (int i = 0; i < TY; ++i)
+                        if (row_ok & (1u << i)) {
+#pragma unroll
+                            for (int t = 0; t < TC; ++t)
+                                __stcs(reinterpret_cast<double2 *>(o + i * rowd) + t,
+                                       acc[(J + 4) % 7][i * TC + t]);
+                        }
+                }
+#pragma unroll
+                for (int p = 0; p < NP; ++p) {
+                    fma2(acc[(J + 5) % 7][p], wx2, u[p]);
+                    fma2(acc[(J + 6) % 7][p], wx1, u[p]);
+                    fma2(acc[(J + 1) % 7][p], wx1, u[p]);
+                    fma2(acc[(J + 2) % 7][p], wx2, u[p]);
+                }
+
+                if (m.x & kCentre) {
+                    // ---- diagonal (+ v_eff)
+#pragma unroll
+                    for (int i = 0; i < TY; ++i) {
+                        double d0 = wdiag, d1 = wdiag;
+                        if (HAS_V) {
+                            if constexpr (CPLX) {
+                                d0 += lds64(sb + v_off + i * pitchv);
+                                d1 = d0;
+                            } else {
+                                const double2 vv = lds128(sb + v_off + i * pitchv);
+                                d0 += vv.x;
+                                d1 += vv.y;
+                            }
+                        }
+                        acc[J][i].x = fma(d0, u[i].x, acc[J][i].x);
+                        acc[J][i].y = fma(d1, u[i].y, acc[J][i].y);
+                    }
+                    // ---- y taps: stream the TY + 6 rows of the thread's column through
+#pragma unroll
+                    for (int rr = 0; rr < TY + 6; ++rr) {
+                        if (rr >= 3 && rr < 3 + TY) continue;  // own rows: already in u
+                        double2 c[TC];
+#pragma unroll
+                        for (int t = 0; t < TC; ++t) c[t] = lds128(ub + rr * pitch + t * 16);
+                        if (CPLX && (PH & 1)) {
+                            if (rr < 3) {
+                                if (ylo && r0 + rr < nlo) {
+#pragma unroll
+                                    for (int t = 0; t < TC; ++t)
+                                        c[t] = cmul(c[t], g.ph_re[1], -g.ph_im[1]);
+                                }
+                            } else if (yhi && r0 + rr >= nlo + nmid) {
+#pragma unroll
+                                for (int t = 0; t < TC; ++t) c[t] = cmul(c[t], g.ph_re[1], g.ph_im[1]);
+                            }
+                        }
+#pragma unroll
+                        for (int i = 0; i < TY; ++i) {
+                            const int d = rr - 3 - i;
+                            const int ad = d < 0 ? -d : d;
+                            if (ad >= 1 && ad <= 3) {
+                                const double w = (ad == 1) ? wy1 : (ad == 2) ? wy2 : wy3;
+#pragma unroll
+                                for (int t = 0; t < TC; ++t) fma2(acc[J][i * TC + t], w, c[t]);
+                            }
+                        }
+                    }
+                    // own rows are y neighbours of each other
+#pragma unroll
+                    for (int i = 0; i < TY; ++i)
+#pragma unroll
+                        for (int i2 = 0; i2 < TY; ++i2) {
+                            const int ad = i2 > i ? i2 - i : i - i2;
+                            if (ad >= 1 && ad <= 3) {
+                                const double w = (ad == 1) ? wy1 : (ad == 2) ? wy2 : wy3;
+#pragma unroll
+                                for (int t = 0; t < TC; ++t)
+                                    fma2(acc[J][i * TC + t], w, u[i2 * TC + t]);
+                            }
+                        }
+                    // ---- z taps
+#pragma unroll
+                    for (int i = 0; i < TY; ++i) {
+                        if constexpr (CPLX) {
+                            // chunk = one complex point; hz = L3,L2,L1,R1,R2,R3
+                            double2 hz[2 * ZH];
+#pragma unroll
+                            for (int k = 0; k < 2 * ZH; ++k) hz[k] = lds128(sb + hb[k] + i * pitch);
+                            if ((PH & 2) && zphase) {
+#pragma unroll
+                                for (int k = 0; k < 2 * ZH; ++k) {
+                                    const int wbits = (zwrap >> (2 * k)) & 3;
+                                    if (wbits == 1) hz[k] = cmul(hz[k], g.ph_re[2], -g.ph_im[2]);
+                                    if (wbits == 2) hz[k] = cmul(hz[k], g.ph_re[2], g.ph_im[2]);
+                                }
+                            }
+                            double2 &a = acc[J][i];
+                            fma2(a, wz1, hz[2]);
+                            fma2(a, wz1, hz[3]);
+                            fma2(a, wz2, hz[1]);
+                            fma2(a, wz2, hz[4]);
+                            fma2(a, wz3, hz[0]);
+                            fma2(a, wz3, hz[5]);
+                        } else {
+                            // chunk = points (z, z+1); halo = z-3 | z-2,z-1 | z+2,z+3 | z+4.
+                            // The two 8-byte halo words come in two loads whose lanes alternate
+                            // (by groups of 8) between z-3 and z+4, so each half warp touches 32
+                            // distinct banks (an 8-byte load at a 16-byte lane stride would be a
+                            // 2-way bank conflict).
+                            const double e0 = lds64(sb + off8a + i * pitch);
+                            const double e1 = lds64(sb + off8b + i * pitch);
+                            const double l3 = swp ? e1 : e0;
+                            const double r4 = swp ? e0 : e1;
+                            const double2 l21 = lds128(sb + hb[1] + i * pitch);
+                            const double2 r23 = lds128(sb + hb[2] + i * pitch);
+                            double2 &a = acc[J][i];
+                            const double2 o = u[i];
+                            a.x = fma(wz1, l21.y, a.x);
+                            a.x = fma(wz1, o.y, a.x);
+                            a.x = fma(wz2, l21.x, a.x);
+                            a.x = fma(wz2, r23.x, a.x);
+                            a.x = fma(wz3, l3, a.x);
+                            a.x = fma(wz3, r23.y, a.x);
+                            a.y = fma(wz1, o.x, a.y);
+                            a.y = fma(wz1, r23.x, a.y);
+                            a.y = fma(wz2, l21.y, a.y);
+                            a.y = fma(wz2, r23.y, a.y);
+                            a.y = fma(wz3, l21.x, a.y);
+                            a.y = fma(wz3, r4, a.y);
+                        }
+                    }
+                }
+
+                // ---- release the slot; the last warp to do so will refill it with step q + K
+                bool last = false;
+                __syncwarp();
+                if (elect_one()) {
+                    mbar_arrive(empty_bar + 8 * st);
+                    last = atomicInc(&elect_cnt[st], nwarps - 1) == nwarps - 1;
+                }
+
+                // ---- the output three planes ahead is born
+#pragma unroll
+                for (int p = 0; p < NP; ++p) acc[(J + 3) % 7][p] = mul2(wx3, u[p]);
+
+                if (last && q + K < nsteps) {
+                    const int e = q + K;
+                    mbar_wait(empty_bar + 8 * st, par);
+                    issue(e, st);
+                }
+                if (++st == (uint32_t)K) {
+                    st = 0;
+                    par ^= 1u;
+                }
+                m = mn;
+            }
+        }
+    }
+}
+
+}  // namespace
