@@ -349,3 +349,42 @@ def test_host_buffer_apply(oracle, fd):
             assert np.max(np.abs(p_out.numpy() - want_t)) <= tol
         finally:
             fd.fd_destroy(plan)
+
+
+@pytest.mark.parametrize("xchunk", [3, 5, 11])
+def test_many_short_teams_more_ctas_than_sms(oracle, fd, monkeypatch, xchunk):
+    """FDHAM_TUNE=xchunk=n cuts the (band, x) planes into teams of n planes: every team seam, band
+    seam and wrap entry of the step table is exercised, with more CTAs than SMs (several waves)."""
+    monkeypatch.setenv("FDHAM_TUNE", f"xchunk={xchunk},kernel=2")
+    for bc, cplx, k in [((1, 1, 1), False, (0, 0, 0)), ((0, 1, 0), False, (0, 0, 0)),
+                        ((1, 1, 1), True, (0.25, 0.125, -0.3))]:
+        cfg = W.custom((24, 40, 16), (0.2, 0.21, 0.18), bc, k=k, complex_=cplx, nbands=37)
+        psi, v = W.make_psi(cfg), W.make_veff(cfg)
+        got, used = gpu_apply(fd, cfg, psi, v, "auto")
+        assert used == fd.FD_KERNEL_SWEEP
+        want = oracle.apply(cfg.shape, cfg.h, 3, cfg.bc, cfg.k if cplx else None, psi, v)
+        assert np.max(np.abs(got - want)) <= parity_tol(cfg.h, 3, psi, v)
+
+def test_one_plan_two_streams_concurrently(oracle, fd):
+    """A plan is immutable: applies of the same plan on two streams may overlap."""
+    cfg = W.custom((32, 32, 32), (0.2,) * 3, (1, 1, 1), nbands=24)
+    psi, v = W.make_psi(cfg), W.make_veff(cfg)
+    plan = fd.fd_create(cfg.shape, cfg.h, 3, cfg.bc)
+    try:
+        fd.fd_plan_set_kernel(plan, fd.FD_KERNEL_SWEEP)
+        s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+        a = torch.from_numpy(psi).cuda()
+        b = torch.from_numpy(psi[::-1].copy()).cuda()
+        d_v = torch.from_numpy(v).cuda()
+        oa, ob = torch.empty_like(a), torch.empty_like(b)
+        torch.cuda.synchronize()
+        for _ in range(5):
+            fd.fd_apply_hamiltonian(plan, a, d_v, oa, stream=s1)
+            fd.fd_apply_hamiltonian(plan, b, d_v, ob, stream=s2)
+        torch.cuda.synchronize()
+        want = oracle.apply(cfg.shape, cfg.h, 3, cfg.bc, None, psi, v)
+        tol = parity_tol(cfg.h, 3, psi, v)
+        assert np.max(np.abs(oa.cpu().numpy() - want)) <= tol
+        assert np.max(np.abs(ob.cpu().numpy() - want[::-1])) <= tol
+    finally:
+        fd.fd_destroy(plan)
