@@ -36,8 +36,9 @@ DEFAULT_WORKLOAD = "cfg3"
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the sweep kernel from the committed
 # `ncu --set full` capture (profiles/), keyed by workload; None until a capture exists.
 NCU_TRAFFIC_BYTES = {
-    # profiles/r1f_sweep_cfg3_ncu_full.md: 1.928 GB read + 1.774 GB written per launch
-    "cfg3_96c_periodic_f64": 3702005000,
+    # profiles/r1i_sweep_ncu_full.md: dram__bytes_read.sum + dram__bytes_write.sum per launch
+    "cfg3_96c_periodic_f64": 3698447000,
+    "cfg5_slab_128x128x192_f64": 22225838000,
 }
 
 
