@@ -87,6 +87,8 @@ typedef struct {
     int bc[3];
     double k[3];
     double c[FDO_MAX_NN + 1];
+    double scale; /* prefactor of the FD Laplacian: -1/2 (kinetic operator, Eq. 6) unless the
+                     caller of fd_oracle_apply_scaled asks for another one */
 } fdo_geom;
 
 static int fdo_fill_geom(fdo_geom *g, const int32_t shape[3], const double h[3], int nn,
@@ -95,6 +97,7 @@ static int fdo_fill_geom(fdo_geom *g, const int32_t shape[3], const double h[3],
     if (!shape || !h || !bc) return -1;
     if (fd_oracle_coeffs(nn, g->c) != 0) return -1;
     g->nn = nn;
+    g->scale = -0.5;
     for (int d = 0; d < 3; ++d) {
         if (shape[d] < 1 || !(h[d] > 0.0)) return -1;
         if (bc[d] != FDO_BC_ZERO && bc[d] != FDO_BC_PERIODIC) return -1;
@@ -145,7 +148,7 @@ static inline double fdo_point_real(const fdo_geom *g, const double *psi, const 
         double s = g->c[0] * psi[lin];
         for (int j = 1; j <= g->nn; ++j)
             s += g->c[j] * (fdo_hat_real(g, psi, idx, d, +j) + fdo_hat_real(g, psi, idx, d, -j));
-        acc += (-0.5 / (g->h[d] * g->h[d])) * s;
+        acc += (g->scale / (g->h[d] * g->h[d])) * s;
     }
     if (v) acc += v[lin] * psi[lin];
     return acc;
@@ -160,7 +163,7 @@ static inline double complex fdo_point_cplx(const fdo_geom *g, const double comp
         double complex s = g->c[0] * psi[lin];
         for (int j = 1; j <= g->nn; ++j)
             s += g->c[j] * (fdo_hat_cplx(g, psi, idx, d, +j) + fdo_hat_cplx(g, psi, idx, d, -j));
-        acc += (-0.5 / (g->h[d] * g->h[d])) * s;
+        acc += (g->scale / (g->h[d] * g->h[d])) * s;
     }
     if (v) acc += v[lin] * psi[lin];
     return acc;
@@ -178,6 +181,51 @@ int fd_oracle_apply(const int32_t shape[3], const double h[3], int32_t nn, const
 {
     fdo_geom g;
     if (fdo_fill_geom(&g, shape, h, nn, bc, k_reduced) != 0) return -1;
+    if (!psi || !out || nbands < 0) return -1;
+    if (!is_complex)
+        for (int d = 0; d < 3; ++d)
+            if (g.k[d] != 0.0) return -1;
+    const int64_t P = g.n[0] * g.n[1] * g.n[2];
+#ifdef _OPENMP
+    if (nthreads > 0) omp_set_num_threads(nthreads);
+#else
+    (void)nthreads;
+#endif
+#pragma omp parallel for schedule(static)
+    for (int64_t b = 0; b < nbands; ++b) {
+        for (int64_t ix = 0; ix < g.n[0]; ++ix)
+            for (int64_t iy = 0; iy < g.n[1]; ++iy)
+                for (int64_t iz = 0; iz < g.n[2]; ++iz) {
+                    const int64_t idx[3] = { ix, iy, iz };
+                    const int64_t lin = (ix * g.n[1] + iy) * g.n[2] + iz;
+                    if (is_complex) {
+                        const double complex *pb = (const double complex *)psi + b * P;
+                        ((double complex *)out)[b * P + lin] = fdo_point_cplx(&g, pb, v_eff, idx);
+                    } else {
+                        const double *pb = (const double *)psi + b * P;
+                        ((double *)out)[b * P + lin] = fdo_point_real(&g, pb, v_eff, idx);
+                    }
+                }
+    }
+    return 0;
+}
+
+/*
+ * Same definition evaluated only at npoints sampled outputs: points[4*s + {0,1,2,3}] =
+ * (band, ix, iy, iz); out[s] (double or double complex).  psi is the whole batch
+ * [nbands, nx, ny, nz].  Used for full-size parity where the whole oracle would be too slow.
+ */
+/* Same as fd_oracle_apply with `scale` in place of the -1/2 of Eq. 6: out = scale lap_FD psi
+ * (+ v_eff psi).  scale = 1 is the plain FD Laplacian of the Poisson problem (PAPER.md:248 names
+ * the solvers that use it). */
+int fd_oracle_apply_scaled(const int32_t shape[3], const double h[3], int32_t nn, const int32_t bc[3],
+                    const double *k_reduced, int32_t is_complex, const void *psi,
+                    const double *v_eff, void *out, int64_t nbands, int32_t nthreads, double scale)
+{
+    fdo_geom g;
+    if (fdo_fill_geom(&g, shape, h, nn, bc, k_reduced) != 0) return -1;
+    if (!isfinite(scale)) return -1;
+    g.scale = scale;
     if (!psi || !out || nbands < 0) return -1;
     if (!is_complex)
         for (int d = 0; d < 3; ++d)
@@ -256,7 +304,7 @@ int fd_oracle_dense(const int32_t shape[3], const double h[3], int32_t nn, const
                 const int64_t row = (ix * g.n[1] + iy) * g.n[2] + iz;
                 if (v_eff) M[row * P + row] += v_eff[row];
                 for (int d = 0; d < 3; ++d) {
-                    const double pref = -0.5 / (g.h[d] * g.h[d]);
+                    const double pref = g.scale / (g.h[d] * g.h[d]);
                     M[row * P + row] += pref * g.c[0];
                     for (int j = 1; j <= g.nn; ++j)
                         for (int sgn = -1; sgn <= 1; sgn += 2) {

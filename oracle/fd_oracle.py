@@ -35,6 +35,10 @@ def _load():
         lib.fd_oracle_apply.argtypes = [i32p, f64p, ctypes.c_int32, i32p, f64p, ctypes.c_int32,
                                         vp, f64p, vp, ctypes.c_int64, ctypes.c_int32]
         lib.fd_oracle_apply.restype = ctypes.c_int
+        lib.fd_oracle_apply_scaled.argtypes = [i32p, f64p, ctypes.c_int32, i32p, f64p,
+                                               ctypes.c_int32, vp, f64p, vp, ctypes.c_int64,
+                                               ctypes.c_int32, ctypes.c_double]
+        lib.fd_oracle_apply_scaled.restype = ctypes.c_int
         lib.fd_oracle_points.argtypes = [i32p, f64p, ctypes.c_int32, i32p, f64p, ctypes.c_int32,
                                          vp, f64p, ctypes.c_int64, i64p, ctypes.c_int64, vp]
         lib.fd_oracle_points.restype = ctypes.c_int
@@ -92,15 +96,21 @@ def _check_inputs(shape, psi, v_eff):
 
 def apply(shape: Sequence[int], h: Sequence[float], nn: int, bc: Sequence[int],
           k: Optional[Sequence[float]], psi: np.ndarray, v_eff: Optional[np.ndarray] = None,
-          nthreads: int = 0) -> np.ndarray:
-    """H psi (v_eff given) or T psi (v_eff None) for psi[nbands,nx,ny,nz]; returns a new array."""
+          nthreads: int = 0, scale: Optional[float] = None) -> np.ndarray:
+    """H psi (v_eff given) or T psi (v_eff None) for psi[nbands,nx,ny,nz]; returns a new array.
+    scale: prefactor of the FD Laplacian instead of -1/2 (None = the kinetic operator of Eq. 6)."""
     shape, psi, v_eff = _check_inputs(shape, psi, v_eff)
     out = np.empty_like(psi)
     is_c = psi.dtype == np.complex128
     kk = _f64(k) if k is not None else None
-    rc = _load().fd_oracle_apply(_i32(shape), _f64(h), int(nn), _i32(bc), kk, int(is_c),
-                                 _ptr(psi), _f64ptr(v_eff), _ptr(out), psi.shape[0],
-                                 int(nthreads))
+    if scale is None:
+        rc = _load().fd_oracle_apply(_i32(shape), _f64(h), int(nn), _i32(bc), kk, int(is_c),
+                                     _ptr(psi), _f64ptr(v_eff), _ptr(out), psi.shape[0],
+                                     int(nthreads))
+    else:
+        rc = _load().fd_oracle_apply_scaled(_i32(shape), _f64(h), int(nn), _i32(bc), kk,
+                                            int(is_c), _ptr(psi), _f64ptr(v_eff), _ptr(out),
+                                            psi.shape[0], int(nthreads), float(scale))
     if rc != 0:
         raise ValueError("fd_oracle_apply: invalid argument")
     return out

@@ -29,16 +29,17 @@ def coeffs_f64(nn: int) -> np.ndarray:
     return np.array([float(c) for c in golden_coeffs()[nn]], dtype=np.float64)
 
 
-def kinetic_row_sum(h, nn: int = 3) -> float:
-    """S = 1/2 sum_d (|c_0| + 2 sum_j |c_j|) / h_d^2 : absolute row sum of T (R10)."""
+def kinetic_row_sum(h, nn: int = 3, scale: float = -0.5) -> float:
+    """S = |scale| sum_d (|c_0| + 2 sum_j |c_j|) / h_d^2 : absolute row sum of scale * lap_FD; for
+    the kinetic operator (scale = -1/2) this is DESIGN.md reading R10."""
     c = golden_coeffs()[nn]
     a = float(abs(c[0]) + 2 * sum(abs(x) for x in c[1:]))
-    return 0.5 * sum(a / (hd * hd) for hd in h)
+    return abs(scale) * sum(a / (hd * hd) for hd in h)
 
 
-def parity_tol(h, nn, psi: np.ndarray, v_eff) -> float:
+def parity_tol(h, nn, psi: np.ndarray, v_eff, scale: float = -0.5) -> float:
     """north_star: max|d| <= 1e-12 (max|psi| * S + max|v_eff psi|)."""
-    s = kinetic_row_sum(h, nn)
+    s = kinetic_row_sum(h, nn, scale)
     mp = float(np.max(np.abs(psi))) if psi.size else 0.0
     mv = 0.0
     if v_eff is not None and psi.size:
