@@ -86,6 +86,17 @@ FD_API int fd_create(fd_plan **plan, const int32_t shape[3], const double h[3], 
               const int32_t bc[3], const double k_reduced[3], int32_t dtype, int32_t device);
 
 /*
+ * fd_create_scaled -- fd_create with `scale` in place of the -1/2 of Eq. 6: the plan's applies
+ * compute out = scale lap_FD psi (+ v_eff psi), weights w_d[j] = scale c_j / h_d^2.  scale = 1 gives
+ * the plain FD Laplacian of the Poisson problem (the paper's grid Poisson solvers, PAPER.md:248,
+ * use the same stencil).  fd_create(...) == fd_create_scaled(..., -0.5).
+ * Extra error: FD_ERR_INVALID for a non-finite scale.
+ */
+FD_API int fd_create_scaled(fd_plan **plan, const int32_t shape[3], const double h[3], int32_t nn,
+                     const int32_t bc[3], const double k_reduced[3], int32_t dtype, int32_t device,
+                     double scale);
+
+/*
  * fd_apply_kinetic -- out = T psi = -1/2 lap_FD psi  (steps a2+a3+a5+a6 of SURVEY 8(a); Eq. 6
  * first term).
  *   psi, out   device pointers, [nbands,nx,ny,nz] of the plan's dtype, 16-byte aligned

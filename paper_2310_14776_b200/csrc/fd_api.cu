@@ -111,7 +111,14 @@ extern "C" {
 int fd_create(fd_plan **plan_out, const int32_t shape[3], const double h[3], int32_t nn,
               const int32_t bc[3], const double k_reduced[3], int32_t dtype, int32_t device)
 {
-    if (!plan_out || !shape || !h || !bc) return FD_ERR_INVALID;
+    return fd_create_scaled(plan_out, shape, h, nn, bc, k_reduced, dtype, device, -0.5);
+}
+
+int fd_create_scaled(fd_plan **plan_out, const int32_t shape[3], const double h[3], int32_t nn,
+                     const int32_t bc[3], const double k_reduced[3], int32_t dtype, int32_t device,
+                     double scale)
+{
+    if (!plan_out || !shape || !h || !bc || !isfinite(scale)) return FD_ERR_INVALID;
     if (nn < 1 || nn > FD_MAX_NN) return FD_ERR_INVALID;
     if (dtype != FD_F64 && dtype != FD_C128) return FD_ERR_INVALID;
     for (int d = 0; d < 3; ++d) {
@@ -150,7 +157,7 @@ int fd_create(fd_plan **plan_out, const int32_t shape[3], const double h[3], int
         g.bc[d] = bc[d];
         p->h[d] = h[d];
         p->k[d] = k_reduced ? k_reduced[d] : 0.0;
-        for (int j = 0; j <= nn; ++j) g.w[d][j] = (-0.5 * c[j]) / (h[d] * h[d]);
+        for (int j = 0; j <= nn; ++j) g.w[d][j] = (scale * c[j]) / (h[d] * h[d]);
         g.wdiag += g.w[d][0];
         // exp(+2 pi i k_d); exact 1 at Gamma so real-valued data stays phase free
         if (p->k[d] == 0.0) {

@@ -23,7 +23,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libfdham.so")
 
 EXPORTED_SYMBOLS = [
-    "fd_create", "fd_apply_kinetic", "fd_apply_hamiltonian", "fd_apply_hamiltonian_host",
+    "fd_create", "fd_create_scaled", "fd_apply_kinetic", "fd_apply_hamiltonian",
+    "fd_apply_hamiltonian_host",
     "fd_destroy", "fd_strerror", "fd_plan_set_kernel", "fd_plan_get_kernel", "fd_plan_kernel_for", "fd_plan_launches",
     "fd_plan_get_weights",
 ]
@@ -52,6 +53,9 @@ def load_library() -> ctypes.CDLL:
     i32p, f64p = ctypes.POINTER(ctypes.c_int32), ctypes.POINTER(ctypes.c_double)
     lib.fd_create.argtypes = [ctypes.POINTER(vp), i32p, f64p, i32, i32p, f64p, i32, i32]
     lib.fd_create.restype = ctypes.c_int
+    lib.fd_create_scaled.argtypes = [ctypes.POINTER(vp), i32p, f64p, i32, i32p, f64p, i32, i32,
+                                     ctypes.c_double]
+    lib.fd_create_scaled.restype = ctypes.c_int
     lib.fd_apply_kinetic.argtypes = [vp, vp, vp, i64, vp]
     lib.fd_apply_kinetic.restype = ctypes.c_int
     lib.fd_apply_hamiltonian.argtypes = [vp, vp, vp, vp, i64, vp]
@@ -96,6 +100,21 @@ def fd_create(shape: Sequence[int], h: Sequence[float], nn: int = 3,
                        (ctypes.c_double * 3)(*[float(x) for x in h]), int(nn),
                        (ctypes.c_int32 * 3)(*[int(b) for b in bc]), kk, int(dtype), int(device))
     _check(rc, "fd_create")
+    return plan
+
+
+def fd_create_scaled(shape: Sequence[int], h: Sequence[float], nn: int = 3,
+                     bc: Sequence[int] = (1, 1, 1), k: Optional[Sequence[float]] = None,
+                     dtype: int = FD_F64, device: int = 0, scale: float = -0.5) -> ctypes.c_void_p:
+    """fd_create with `scale` in place of -1/2 (include/fdham.h: fd_create_scaled)."""
+    lib = load_library()
+    plan = ctypes.c_void_p()
+    kk = (ctypes.c_double * 3)(*[float(x) for x in k]) if k is not None else None
+    rc = lib.fd_create_scaled(ctypes.byref(plan), (ctypes.c_int32 * 3)(*[int(s) for s in shape]),
+                              (ctypes.c_double * 3)(*[float(x) for x in h]), int(nn),
+                              (ctypes.c_int32 * 3)(*[int(b) for b in bc]), kk, int(dtype),
+                              int(device), float(scale))
+    _check(rc, "fd_create_scaled")
     return plan
 
 

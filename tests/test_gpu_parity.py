@@ -388,3 +388,30 @@ def test_one_plan_two_streams_concurrently(oracle, fd):
         assert np.max(np.abs(ob.cpu().numpy() - want[::-1])) <= tol
     finally:
         fd.fd_destroy(plan)
+
+
+@pytest.mark.parametrize("scale", [1.0, -2.25])
+def test_scaled_laplacian_plans(oracle, fd, scale):
+    """fd_create_scaled: scale * lap_FD psi + v psi on both kernel families, real
+    and complex with Bloch phases, against the oracle's scaled apply."""
+    for bc, cplx, k in [((1, 1, 1), False, None), ((1, 0, 1), False, None),
+                        ((1, 1, 0), True, (0.25, 0.125, 0.0))]:
+        cfg = W.custom((16, 20, 24), (0.2, 0.23, 0.17), bc, k=k or (0, 0, 0), complex_=cplx,
+                       nbands=5)
+        psi, v = W.make_psi(cfg), W.make_veff(cfg)
+        want = oracle.apply(cfg.shape, cfg.h, 3, cfg.bc, k, psi, v, scale=scale)
+        tol = parity_tol(cfg.h, 3, psi, v, scale)
+        for kern in (fd.FD_KERNEL_SWEEP, fd.FD_KERNEL_GENERIC):
+            plan = fd.fd_create_scaled(cfg.shape, cfg.h, 3, cfg.bc, k,
+                                       fd.FD_C128 if cplx else fd.FD_F64, 0, scale)
+            try:
+                fd.fd_plan_set_kernel(plan, kern)
+                d_psi = torch.from_numpy(psi).cuda()
+                d_out = torch.full_like(d_psi, float("nan"))
+                fd.fd_apply_hamiltonian(plan, d_psi, torch.from_numpy(v).cuda(), d_out)
+                torch.cuda.synchronize()
+                assert np.max(np.abs(d_out.cpu().numpy() - want)) <= tol
+            finally:
+                fd.fd_destroy(plan)
+    with pytest.raises(fd.FDError):
+        fd.fd_create_scaled((8, 8, 8), (0.2,) * 3, 3, (1, 1, 1), None, fd.FD_F64, 0, float("inf"))
