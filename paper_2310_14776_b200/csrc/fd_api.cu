@@ -57,7 +57,7 @@ int check_apply_args(const fd_plan *plan, const void *psi, const double *v_eff, 
 // Kernel family for a batch of `nbands`.  The sweep kernel pays ~1.2 us per x plane of a team's
 // share plus 6 halo planes per band segment whatever the grid size, so a batch that is far too
 // small to fill the persistent teams goes to the one-thread-per-point kernel (measured on B200:
-// 24^3 x 8 bands takes 7 us there against 27 us; 48^3 x 64 bands 166 us against 39 us).
+// 24^3 x 8 bands takes 8 us there against 27 us; 48^3 x 64 bands 115 us against 39 us).
 int kernel_for_batch(const fd_plan *plan, int64_t nbands)
 {
     if (plan->kernel != FD_KERNEL_SWEEP || plan->forced) return plan->kernel;
@@ -69,7 +69,7 @@ int kernel_for_batch(const fd_plan *plan, int64_t nbands)
     if (quota < min_quota) quota = min_quota;
     const double nseg = 1.0 + floor(quota / g.n[0]);
     const double t_sweep_us = 5.0 + 1.2 * (quota + 6.0 * nseg + 4.0);
-    const double t_generic_us = 4.0 + units / 40.0e3;
+    const double t_generic_us = 4.0 + units / 60.0e3;
     return t_generic_us < t_sweep_us ? FD_KERNEL_GENERIC : FD_KERNEL_SWEEP;
 }
 

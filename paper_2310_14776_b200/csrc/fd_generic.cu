@@ -60,30 +60,39 @@ __device__ __forceinline__ void store<true>(double *p, long long idx, const Val<
     reinterpret_cast<double2 *>(p)[idx] = make_double2(v.x, v.y);
 }
 
-template <bool CPLX, bool HAS_V>
-__global__ void __launch_bounds__(256)
-fd_generic_kernel(const FdGeom g, const double *__restrict__ psi, const double *__restrict__ v_eff,
-                  double *__restrict__ out, long long nbands)
+// Block = 64 z-points x 4 rows of one x plane (neighbours along z and y share L1 lines); the
+// stencil half width is a template parameter so the tap loops unroll and the weights come
+// straight from the constant bank.  blockIdx.z = x plane * band groups + band group.
+constexpr int kBx = 64, kBy = 4;
+
+template <bool CPLX, bool HAS_V, int NN>
+__global__ void __launch_bounds__(kBx * kBy)
+fd_generic_kernel(const __grid_constant__ FdGeom g, const double *__restrict__ psi,
+                  const double *__restrict__ v_eff, double *__restrict__ out, long long nbands,
+                  int bgroups)
 {
+    const int iz = blockIdx.x * kBx + threadIdx.x;
+    const int iy = blockIdx.y * kBy + threadIdx.y;
+    const int ix = blockIdx.z / bgroups;
+    const int bg = blockIdx.z - ix * bgroups;
+    if (iz >= g.n[2] || iy >= g.n[1]) return;
     const long long P = (long long)g.n[0] * g.n[1] * g.n[2];
-    const long long lin = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (lin >= P) return;
-    const int iz = (int)(lin % g.n[2]);
-    const int iy = (int)((lin / g.n[2]) % g.n[1]);
-    const int ix = (int)(lin / ((long long)g.n[2] * g.n[1]));
+    const long long lin = ((long long)ix * g.n[1] + iy) * g.n[2] + iz;
     const int idx[3] = {ix, iy, iz};
     const long long stride[3] = {(long long)g.n[1] * g.n[2], (long long)g.n[2], 1};
     double diag = g.wdiag;
     if (HAS_V) diag += __ldg(v_eff + lin);
 
-    for (long long b = blockIdx.y; b < nbands; b += gridDim.y) {
+    for (long long b = bg; b < nbands; b += bgroups) {
         const double *pb = psi + (CPLX ? 2 : 1) * b * P;
         const Val<CPLX> c = load<CPLX>(pb, lin);
         Val<CPLX> acc = Val<CPLX>::zero();
         acc.fma(diag, c);
+#pragma unroll
         for (int d = 0; d < 3; ++d) {
             const int n = g.n[d];
-            for (int j = 1; j <= g.nn; ++j) {
+#pragma unroll
+            for (int j = 1; j <= NN; ++j) {
                 const double w = g.w[d][j];
                 // upper tap i + j
                 int p = idx[d] + j;
@@ -107,27 +116,44 @@ fd_generic_kernel(const FdGeom g, const double *__restrict__ psi, const double *
     }
 }
 
+template <bool CPLX, bool HAS_V>
+cudaError_t launch_nn(const FdGeom &g, const double *p, const double *v_eff, double *o,
+                      long long nbands, cudaStream_t stream)
+{
+    // band groups: enough CTAs to fill the device, blockIdx.z <= 65535
+    long long bgroups = nbands;
+    const long long cap = 65535 / g.n[0];
+    if (bgroups > cap) bgroups = cap;
+    if (bgroups < 1) return cudaErrorInvalidConfiguration;
+    const dim3 block(kBx, kBy);
+    const dim3 grid((unsigned)((g.n[2] + kBx - 1) / kBx), (unsigned)((g.n[1] + kBy - 1) / kBy),
+                    (unsigned)(g.n[0] * bgroups));
+    if (grid.y > 65535) return cudaErrorInvalidConfiguration;
+    const int bgi = (int)bgroups;
+    switch (g.nn) {
+    case 1: fd_generic_kernel<CPLX, HAS_V, 1><<<grid, block, 0, stream>>>(g, p, v_eff, o, nbands, bgi); break;
+    case 2: fd_generic_kernel<CPLX, HAS_V, 2><<<grid, block, 0, stream>>>(g, p, v_eff, o, nbands, bgi); break;
+    case 3: fd_generic_kernel<CPLX, HAS_V, 3><<<grid, block, 0, stream>>>(g, p, v_eff, o, nbands, bgi); break;
+    case 4: fd_generic_kernel<CPLX, HAS_V, 4><<<grid, block, 0, stream>>>(g, p, v_eff, o, nbands, bgi); break;
+    case 5: fd_generic_kernel<CPLX, HAS_V, 5><<<grid, block, 0, stream>>>(g, p, v_eff, o, nbands, bgi); break;
+    case 6: fd_generic_kernel<CPLX, HAS_V, 6><<<grid, block, 0, stream>>>(g, p, v_eff, o, nbands, bgi); break;
+    default: return cudaErrorInvalidConfiguration;
+    }
+    return cudaPeekAtLastError();
+}
+
 }  // namespace
 
 cudaError_t fd_launch_generic(const fd_plan *plan, const void *psi, const double *v_eff, void *out,
                               int64_t nbands, cudaStream_t stream)
 {
     const FdGeom &g = plan->g;
-    const long long P = (long long)g.n[0] * g.n[1] * g.n[2];
-    dim3 block(256);
-    dim3 grid((unsigned)((P + 255) / 256), (unsigned)(nbands < 32768 ? nbands : 32768));
+    if (g.n[0] > 65535) return cudaErrorInvalidConfiguration;
     const double *p = static_cast<const double *>(psi);
     double *o = static_cast<double *>(out);
-    if (g.cplx) {
-        if (v_eff)
-            fd_generic_kernel<true, true><<<grid, block, 0, stream>>>(g, p, v_eff, o, nbands);
-        else
-            fd_generic_kernel<true, false><<<grid, block, 0, stream>>>(g, p, nullptr, o, nbands);
-    } else {
-        if (v_eff)
-            fd_generic_kernel<false, true><<<grid, block, 0, stream>>>(g, p, v_eff, o, nbands);
-        else
-            fd_generic_kernel<false, false><<<grid, block, 0, stream>>>(g, p, nullptr, o, nbands);
-    }
-    return cudaPeekAtLastError();
+    if (g.cplx)
+        return v_eff ? launch_nn<true, true>(g, p, v_eff, o, nbands, stream)
+                     : launch_nn<true, false>(g, p, nullptr, o, nbands, stream);
+    return v_eff ? launch_nn<false, true>(g, p, v_eff, o, nbands, stream)
+                 : launch_nn<false, false>(g, p, nullptr, o, nbands, stream);
 }
