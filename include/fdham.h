@@ -64,7 +64,7 @@ enum {
 enum {
     FD_KERNEL_AUTO = 0,    /* pick the fastest supported kernel for the plan (default)            */
     FD_KERNEL_GENERIC = 1, /* one thread per grid point, any nn / shape / bc                      */
-    FD_KERNEL_SWEEP = 2    /* TMA-staged y-z tiles + register sweep along x (nn = 3 only)          */
+    FD_KERNEL_SWEEP = 2    /* TMA-staged y-z tiles + register sweep along x (nn = 1..3)            */
 };
 
 /*

@@ -68,7 +68,7 @@ int kernel_for_batch(const fd_plan *plan, int64_t nbands)
     const double min_quota = g.n[0] < 16 ? g.n[0] : 16;
     if (quota < min_quota) quota = min_quota;
     const double nseg = 1.0 + floor(quota / g.n[0]);
-    const double t_sweep_us = 5.0 + 1.2 * (quota + 6.0 * nseg + 4.0);
+    const double t_sweep_us = 5.0 + 1.2 * (quota + 2.0 * g.nn * nseg + 4.0);
     const double t_generic_us = 4.0 + units / 60.0e3;
     return t_generic_us < t_sweep_us ? FD_KERNEL_GENERIC : FD_KERNEL_SWEEP;
 }

@@ -56,15 +56,15 @@ cudaError_t fd_launch_generic(const fd_plan *plan, const void *psi, const double
 // fd_sweep_inst_*.cu: instantiations of the sweep kernel template (fd_sweep_kernel.cuh)
 typedef void (*FdSweepKernelFn)(const FdGeom, const FdSweepCfg, const double *, const double *,
                                 double *, const long long, const int);
-FdSweepKernelFn fd_sweep_pick_real(int rowd, int has_v);
-FdSweepKernelFn fd_sweep_pick_cplx_ph0(int rowd, int has_v);
-FdSweepKernelFn fd_sweep_pick_cplx_ph1(int rowd, int has_v);
-FdSweepKernelFn fd_sweep_pick_cplx_ph3(int rowd, int has_v);
-inline FdSweepKernelFn fd_sweep_pick_cplx(int rowd, int has_v, int ph)
+FdSweepKernelFn fd_sweep_pick_real(int rowd, int has_v, int nn);
+FdSweepKernelFn fd_sweep_pick_cplx_ph0(int rowd, int has_v, int nn);
+FdSweepKernelFn fd_sweep_pick_cplx_ph1(int rowd, int has_v, int nn);
+FdSweepKernelFn fd_sweep_pick_cplx_ph3(int rowd, int has_v, int nn);
+inline FdSweepKernelFn fd_sweep_pick_cplx(int rowd, int has_v, int ph, int nn)
 {
-    if (ph == 0) return fd_sweep_pick_cplx_ph0(rowd, has_v);
-    if (ph == 1) return fd_sweep_pick_cplx_ph1(rowd, has_v);
-    return fd_sweep_pick_cplx_ph3(rowd, has_v);
+    if (ph == 0) return fd_sweep_pick_cplx_ph0(rowd, has_v, nn);
+    if (ph == 1) return fd_sweep_pick_cplx_ph1(rowd, has_v, nn);
+    return fd_sweep_pick_cplx_ph3(rowd, has_v, nn);
 }
 // fd_sweep.cu
 void fd_sweep_configure(fd_plan *plan, int tyc_override, int xchunk_override);

@@ -19,7 +19,8 @@ void fd_sweep_configure(fd_plan *plan, int tyc_override, int xchunk_override)
     const FdGeom &g = plan->g;
     c = FdSweepCfg{};
     c.xchunk = xchunk_override;  // 0 = automatic (persistent teams), else planes per team
-    if (g.nn != 3) return;
+    if (g.nn > 3) return;  // 2 nn + 1 accumulator planes: the register budget ends at nn = 3
+    const int halo = 2 * g.nn;
     if (g.n[0] < 8 || g.n[1] < 8 || g.n[2] < 8 || (g.n[2] & 1)) return;
     c.ty = 4;
     c.tc = 1;
@@ -30,7 +31,7 @@ void fd_sweep_configure(fd_plan *plan, int tyc_override, int xchunk_override)
     c.zb_bytes = (g.bc[2] == 0) ? (c.ty * pitch + 127) / 128 * 128 : 0;
     const int max_rg = kMaxThreads / c.lanes;
     auto stage_bytes = [&](int tyc) {
-        return (c.zb_bytes + (tyc + 6) * pitch + tyc * pitchv + 127) / 128 * 128;
+        return (c.zb_bytes + (tyc + halo) * pitch + tyc * pitchv + 127) / 128 * 128;
     };
     // fewest y tiles whose stage fits a ring of >= 3 slots beside a 4 KiB (512-step) table
     int tyc = 0;
@@ -54,7 +55,7 @@ void fd_sweep_configure(fd_plan *plan, int tyc_override, int xchunk_override)
     c.nytiles = ceil_div(g.n[1], tyc);
     c.threads = ceil_div(c.rowgroups * c.lanes, 32) * 32;
     c.stage_bytes = stage_bytes(tyc);
-    c.v_off = c.zb_bytes + (tyc + 6) * pitch;
+    c.v_off = c.zb_bytes + (tyc + halo) * pitch;
     int tab_bytes = 16384;
     int stages = (kSmemMax - kCtlBytes - tab_bytes) / c.stage_bytes;
     if (stages < 3) {
@@ -81,12 +82,12 @@ FdSweepKernelFn kernel_for(const fd_plan *plan, bool has_v)
 {
     const FdGeom &g = plan->g;
     const int rowd = g.n[2] * (g.cplx ? 2 : 1);
-    if (!g.cplx) return fd_sweep_pick_real(rowd, has_v);
+    if (!g.cplx) return fd_sweep_pick_real(rowd, has_v, g.nn);
     // which Bloch-phase code the kernel needs: bit 0 = x or y, bit 1 = z
     int ph = 0;
     for (int d = 0; d < 3; ++d)
         if (g.bc[d] && (g.ph_re[d] != 1.0 || g.ph_im[d] != 0.0)) ph |= (d == 2) ? 2 : 1;
-    return fd_sweep_pick_cplx(rowd, has_v, ph);
+    return fd_sweep_pick_cplx(rowd, has_v, ph, g.nn);
 }
 
 }  // namespace
@@ -121,11 +122,12 @@ cudaError_t fd_launch_sweep(const fd_plan *plan, const void *psi, const double *
             quota = c.xchunk;
         } else {
             quota = (total + c.max_teams - 1) / c.max_teams;
-            const int min_quota = g.n[0] < 16 ? g.n[0] : 16;  // below this the 6 halo planes dominate
+            const int min_quota = g.n[0] < 16 ? g.n[0] : 16;  // below this the halo planes dominate
             if (quota < min_quota) quota = min_quota;
         }
-        // the team's steps (quota + 6 per band touched, + 1 prefetched entry) must fit the table
-        const long long quota_cap = ((long long)(c.tab_cap - 13) * g.n[0]) / (g.n[0] + 6);
+        // the team's steps (quota + 2 nn per band touched, + 1 prefetched entry) must fit the table
+        const long long quota_cap =
+            ((long long)(c.tab_cap - 4 * g.nn - 1) * g.n[0]) / (g.n[0] + 2 * g.nn);
         if (quota > quota_cap) quota = quota_cap;
         if (quota < 1) return cudaErrorInvalidConfiguration;
         const long long nteams = (total + quota - 1) / quota;

@@ -1,7 +1,8 @@
 // fd_sweep_kernel.cuh -- the sweep kernel template (included by the fd_sweep_inst_*.cu translation
 // units, which instantiate it, so that they compile in parallel).
 //
-// Sweep kernel: the bandwidth path of libfdham (nn = 3, i.e. GPAW's default 19-point star).
+// Sweep kernel: the bandwidth path of libfdham (nn = 1..3; nn = 3 is GPAW's default 19-point star,
+// which the comments below use for concreteness: halo 3, seven accumulators).
 //
 // Operation: include/fdham.h -- out = -1/2 lap_FD psi + v_eff psi (Eq. 6 first two terms,
 // PAPER.md:187-188; FD kinetic operator PAPER.md:232; the stencil hot spot PAPER.md:150).
@@ -168,14 +169,16 @@ __device__ __forceinline__ double2 cmul(const double2 &a, double pr, double pi)
 
 // The linear (band, x) plane range [L0, L1) of a team, cut into segments of one band each:
 // segment 0 = (b0, [x00, x00+len0)), segment k >= 1 = (b0+k, [0, len_k)).  A segment of `len`
-// output planes takes len + 6 steps s = 0..len+5; step s brings in plane xl = x0 - 3 + s.
+// output planes takes len + 2 nn steps s = 0..len+2nn-1; step s brings in plane xl = x0 - nn + s.
 struct TeamRange {
     long long L0, L1;
     int nx;
     int b0, x00, len0;
     int nsteps;
-    __device__ void init(long long l0, long long l1, int nx_)
+    int hn;  // stencil half width nn: a segment has 2 nn halo steps
+    __device__ void init(long long l0, long long l1, int nx_, int nn_)
     {
+        hn = nn_;
         L0 = l0;
         L1 = l1;
         nx = nx_;
@@ -185,27 +188,27 @@ struct TeamRange {
         len0 = (n < (long long)(nx_ - x00)) ? (int)n : (nx_ - x00);
         const long long rest = n - len0;
         const int nseg = 1 + (int)((rest + nx_ - 1) / nx_);
-        nsteps = (int)n + 6 * nseg;
+        nsteps = (int)n + 2 * hn * nseg;
     }
     // Table entry of step e (layout above).
     __device__ uint2 entry(int e, int per_x) const
     {
         int band, x0, len, s;
-        if (e < len0 + 6) {
+        if (e < len0 + 2 * hn) {
             band = b0;
             x0 = x00;
             len = len0;
             s = e;
         } else {
-            const int e2 = e - (len0 + 6);
-            const int k = e2 / (nx + 6);
-            s = e2 - k * (nx + 6);
+            const int e2 = e - (len0 + 2 * hn);
+            const int k = e2 / (nx + 2 * hn);
+            s = e2 - k * (nx + 2 * hn);
             band = b0 + 1 + k;
             x0 = 0;
             const long long rem = L1 - (L0 + len0 + (long long)k * nx);
             len = (rem < (long long)nx) ? (int)rem : nx;
         }
-        const int xl = x0 - 3 + s;
+        const int xl = x0 - hn + s;
         uint2 m;
         if (xl < 0) {
             m.x = per_x ? ((unsigned)(band * nx + xl + nx) | kWrapLo) : kZero;
@@ -216,15 +219,16 @@ struct TeamRange {
         }
         // a whole periodic band: its last three planes (read first, as the wrap) and its first
         // three come round again ~nx steps later
-        if (per_x && x0 == 0 && len == nx && s < 6) m.x |= kKeepL2;
-        if (s >= 3 && s < len + 3) m.x |= kCentre;
-        m.y = (s >= 6) ? (unsigned)(band * nx + x0 + s - 6) : kNoPlane;
+        if (per_x && x0 == 0 && len == nx && s < 2 * hn) m.x |= kKeepL2;
+        if (s >= hn && s < len + hn) m.x |= kCentre;
+        m.y = (s >= 2 * hn) ? (unsigned)(band * nx + x0 + s - 2 * hn) : kNoPlane;
         return m;
     }
 };
 
 // PH (complex only): which Bloch-phase code is compiled in -- bit 0: x and y wraps, bit 1: z wraps.
-template <bool CPLX, bool HAS_V, int ROWD, int PH>
+// NN: stencil half width (1..3); 2 NN + 1 register accumulators per point, unrolled 2 NN + 1 times.
+template <bool CPLX, bool HAS_V, int ROWD, int PH, int NN>
 __global__ void __launch_bounds__(kMaxThreads, 1)
 fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSweepCfg cfg,
                 const double *__restrict__ psi, const double *__restrict__ v_eff,
@@ -232,7 +236,8 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
 {
     constexpr int TY = 4;              // rows per thread
     constexpr int TC = 1;              // 16-byte chunks per thread per row (lane stride 16 B)
-    constexpr int ZH = CPLX ? 3 : 2;   // halo chunks per side along z
+    constexpr int ZH = CPLX ? NN : (NN + 1) / 2;   // halo chunks per side along z
+    constexpr int NS = 2 * NN + 1;     // in-flight output planes (accumulator slots)
     constexpr int NP = TY * TC;
 
     extern __shared__ __align__(128) unsigned char smem[];
@@ -265,16 +270,16 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
 
     // ---- y segments of the staged tile: smem row R <-> global row y0 - 3 + R ------------------
     const int per_y = g.bc[1], per_x = g.bc[0], per_z = g.bc[2];
-    const int nlo = max(0, 3 - y0);                     // rows below row 0
-    const int nhi = max(0, y0 + rows_valid + 3 - ny);   // rows past row ny-1
-    const int nmid = rows_valid + 6 - nlo - nhi;
+    const int nlo = max(0, NN - y0);                     // rows below row 0
+    const int nhi = max(0, y0 + rows_valid + NN - ny);   // rows past row ny-1
+    const int nmid = rows_valid + 2 * NN - nlo - nhi;
     const uint32_t zb = (uint32_t)cfg.zb_bytes;
     const uint32_t tx_psi = (uint32_t)((nmid + (per_y ? nlo + nhi : 0)) * pitch);
     const uint32_t tx_v = (uint32_t)(rows_valid * pitchv);
     const long long plane_d = (long long)ny * rowd;  // doubles per x plane of psi / out
 
     TeamRange tr;
-    tr.init(L0, L1, nx);
+    tr.init(L0, L1, nx, NN);
     const int nsteps = tr.nsteps;
 
     // ---- one-time shared memory setup ------------------------------------------------------
@@ -302,7 +307,7 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
         }
         // rows past the ragged end of the last tile are never loaded: define them
         for (int i = tid; i < (cfg.tyc - rows_valid) * rowd; i += blockDim.x)
-            rows[(size_t)(rows_valid + 6) * rowd + i] = 0.0;
+            rows[(size_t)(rows_valid + 2 * NN) * rowd + i] = 0.0;
     }
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     __syncthreads();
@@ -324,14 +329,14 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
             if (per_y && nlo > 0)
                 bulk_g2s_hint(dst, src + (long long)(ny - nlo) * rowd, (uint32_t)(nlo * pitch), bar,
                               pol);
-            bulk_g2s_hint(dst + nlo * pitch, src + (long long)(y0 - 3 + nlo) * rowd,
+            bulk_g2s_hint(dst + nlo * pitch, src + (long long)(y0 - NN + nlo) * rowd,
                           (uint32_t)(nmid * pitch), bar, pol);
             if (per_y && nhi > 0)
                 bulk_g2s_hint(dst + (nlo + nmid) * pitch, src, (uint32_t)(nhi * pitch), bar, pol);
         } else {
             if (per_y && nlo > 0)
                 bulk_g2s(dst, src + (long long)(ny - nlo) * rowd, (uint32_t)(nlo * pitch), bar);
-            bulk_g2s(dst + nlo * pitch, src + (long long)(y0 - 3 + nlo) * rowd,
+            bulk_g2s(dst + nlo * pitch, src + (long long)(y0 - NN + nlo) * rowd,
                      (uint32_t)(nmid * pitch), bar);
             if (per_y && nhi > 0)
                 bulk_g2s(dst + (nlo + nmid) * pitch, src, (uint32_t)(nhi * pitch), bar);
@@ -368,7 +373,7 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
         } else if (cz >= cpr) {
             if (per_z) { cz -= cpr; zwrap |= 2 << (2 * k); } else valid = false;
         }
-        hb[k] = valid ? (int)zb + (r0 + 3) * pitch + cz * 16 : 0;
+        hb[k] = valid ? (int)zb + (r0 + NN) * pitch + cz * 16 : 0;
     }
     // real: lanes of odd 8-lane groups fetch z+4 first and z-3 second (see the z taps)
     const bool swp = !CPLX && (tid & 8) != 0;
@@ -381,7 +386,7 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
     // only the first row group of tile 0 has wrapped rows below, only row groups reaching past the
     // last valid row of the last tile have wrapped rows above
     const bool ylo = yphase && r0 < nlo;
-    const bool yhi = yphase && r0 + TY + 6 > nlo + nmid;
+    const bool yhi = yphase && r0 + TY + 2 * NN > nlo + nmid;
 
     // store addressing: row i of the micro tile is global row y0 + r0 + i
     unsigned row_ok = 0;
@@ -390,23 +395,27 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
         if (tactive && (r0 + i) < rows_valid) row_ok |= 1u << i;
     double *const obase = out + (long long)(y0 + r0) * rowd + zc0 * 2;
 
-    const double wx1 = g.w[0][1], wx2 = g.w[0][2], wx3 = g.w[0][3];
-    const double wy1 = g.w[1][1], wy2 = g.w[1][2], wy3 = g.w[1][3];
-    const double wz1 = g.w[2][1], wz2 = g.w[2][2], wz3 = g.w[2][3];
+    double wx[NN + 1], wy[NN + 1], wz[NN + 1];  // w[j] = scale c_j / h_d^2, j = 1..NN
+#pragma unroll
+    for (int j = 1; j <= NN; ++j) {
+        wx[j] = g.w[0][j];
+        wy[j] = g.w[1][j];
+        wz[j] = g.w[2][j];
+    }
     const double wdiag = g.wdiag;
 
     // ---- the sweep: one flat loop over the step table ------------------------------------------
-    double2 acc[7][NP];
+    double2 acc[NS][NP];
 #pragma unroll
-    for (int a = 0; a < 7; ++a)
+    for (int a = 0; a < NS; ++a)
 #pragma unroll
         for (int p = 0; p < NP; ++p) acc[a][p] = make_double2(0.0, 0.0);
 
     uint32_t st = 0, par = 0;  // ring slot and mbarrier phase parity of the current step
     uint2 m = tabp[0];         // .x flags (| load plane), .y out plane of the current step
-    for (int q7 = 0; q7 < nsteps; q7 += 7) {
+    for (int q7 = 0; q7 < nsteps; q7 += NS) {
 #pragma unroll
-        for (int J = 0; J < 7; ++J) {
+        for (int J = 0; J < NS; ++J) {
             const int q = q7 + J;
             if (q < nsteps) {
                 const uint2 mn = tabp[q + 1];
@@ -421,13 +430,13 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
                     for (int i = 0; i < TY; ++i)
 #pragma unroll
                         for (int t = 0; t < TC; ++t)
-                            u[i * TC + t] = lds128(ub + (3 + i) * pitch + t * 16);
+                            u[i * TC + t] = lds128(ub + (NN + i) * pitch + t * 16);
                     if (CPLX && (PH & 1) && yhi) {
                         // rows past a ragged tile end are wrapped rows: neighbours of the last
                         // valid rows, so they carry the y Bloch factor like any halo row
 #pragma unroll
                         for (int i = 0; i < TY; ++i)
-                            if (r0 + 3 + i >= nlo + nmid) {
+                            if (r0 + NN + i >= nlo + nmid) {
 #pragma unroll
                                 for (int t = 0; t < TC; ++t)
                                     u[i * TC + t] = cmul(u[i * TC + t], g.ph_re[1], g.ph_im[1]);
@@ -445,7 +454,7 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
 
                 // ---- x taps, oldest output first: it is complete after this and leaves
 #pragma unroll
-                for (int p = 0; p < NP; ++p) fma2(acc[(J + 4) % 7][p], wx3, u[p]);
+                for (int p = 0; p < NP; ++p) fma2(acc[(J + NN + 1) % NS][p], wx[NN], u[p]);
                 if (m.y != kNoPlane) {
                     double *o = obase + (long long)m.y * plane_d;
 #pragma unroll
@@ -454,15 +463,16 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
 #pragma unroll
                             for (int t = 0; t < TC; ++t)
                                 __stcs(reinterpret_cast<double2 *>(o + i * rowd) + t,
-                                       acc[(J + 4) % 7][i * TC + t]);
+                                       acc[(J + NN + 1) % NS][i * TC + t]);
                         }
                 }
 #pragma unroll
                 for (int p = 0; p < NP; ++p) {
-                    fma2(acc[(J + 5) % 7][p], wx2, u[p]);
-                    fma2(acc[(J + 6) % 7][p], wx1, u[p]);
-                    fma2(acc[(J + 1) % 7][p], wx1, u[p]);
-                    fma2(acc[(J + 2) % 7][p], wx2, u[p]);
+#pragma unroll
+                    for (int d = 1; d < NN; ++d) {  // outputs xl - d and xl + d
+                        fma2(acc[(J + NS - d) % NS][p], wx[d], u[p]);
+                        fma2(acc[(J + d) % NS][p], wx[d], u[p]);
+                    }
                 }
 
                 if (m.x & kCentre) {
@@ -485,13 +495,13 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
                     }
                     // ---- y taps: stream the TY + 6 rows of the thread's column through
 #pragma unroll
-                    for (int rr = 0; rr < TY + 6; ++rr) {
-                        if (rr >= 3 && rr < 3 + TY) continue;  // own rows: already in u
+                    for (int rr = 0; rr < TY + 2 * NN; ++rr) {
+                        if (rr >= NN && rr < NN + TY) continue;  // own rows: already in u
                         double2 c[TC];
 #pragma unroll
                         for (int t = 0; t < TC; ++t) c[t] = lds128(ub + rr * pitch + t * 16);
                         if (CPLX && (PH & 1)) {
-                            if (rr < 3) {
+                            if (rr < NN) {
                                 if (ylo && r0 + rr < nlo) {
 #pragma unroll
                                     for (int t = 0; t < TC; ++t)
@@ -504,12 +514,11 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
                         }
 #pragma unroll
                         for (int i = 0; i < TY; ++i) {
-                            const int d = rr - 3 - i;
+                            const int d = rr - NN - i;
                             const int ad = d < 0 ? -d : d;
-                            if (ad >= 1 && ad <= 3) {
-                                const double w = (ad == 1) ? wy1 : (ad == 2) ? wy2 : wy3;
+                            if (ad >= 1 && ad <= NN) {
 #pragma unroll
-                                for (int t = 0; t < TC; ++t) fma2(acc[J][i * TC + t], w, c[t]);
+                                for (int t = 0; t < TC; ++t) fma2(acc[J][i * TC + t], wy[ad], c[t]);
                             }
                         }
                     }
@@ -519,18 +528,17 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
 #pragma unroll
                         for (int i2 = 0; i2 < TY; ++i2) {
                             const int ad = i2 > i ? i2 - i : i - i2;
-                            if (ad >= 1 && ad <= 3) {
-                                const double w = (ad == 1) ? wy1 : (ad == 2) ? wy2 : wy3;
+                            if (ad >= 1 && ad <= NN) {
 #pragma unroll
                                 for (int t = 0; t < TC; ++t)
-                                    fma2(acc[J][i * TC + t], w, u[i2 * TC + t]);
+                                    fma2(acc[J][i * TC + t], wy[ad], u[i2 * TC + t]);
                             }
                         }
                     // ---- z taps
 #pragma unroll
                     for (int i = 0; i < TY; ++i) {
                         if constexpr (CPLX) {
-                            // chunk = one complex point; hz = L3,L2,L1,R1,R2,R3
+                            // chunk = one complex point; hz = L_NN .. L_1, R_1 .. R_NN
                             double2 hz[2 * ZH];
 #pragma unroll
                             for (int k = 0; k < 2 * ZH; ++k) hz[k] = lds128(sb + hb[k] + i * pitch);
@@ -543,38 +551,61 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
                                 }
                             }
                             double2 &a = acc[J][i];
-                            fma2(a, wz1, hz[2]);
-                            fma2(a, wz1, hz[3]);
-                            fma2(a, wz2, hz[1]);
-                            fma2(a, wz2, hz[4]);
-                            fma2(a, wz3, hz[0]);
-                            fma2(a, wz3, hz[5]);
+#pragma unroll
+                            for (int j = 1; j <= NN; ++j) {
+                                fma2(a, wz[j], hz[NN - j]);
+                                fma2(a, wz[j], hz[NN + j - 1]);
+                            }
                         } else {
-                            // chunk = points (z, z+1); halo = z-3 | z-2,z-1 | z+2,z+3 | z+4.
-                            // The two 8-byte halo words come in two loads whose lanes alternate
-                            // (by groups of 8) between z-3 and z+4, so each half warp touches 32
-                            // distinct banks (an 8-byte load at a 16-byte lane stride would be a
-                            // 2-way bank conflict).
-                            const double e0 = lds64(sb + off8a + i * pitch);
-                            const double e1 = lds64(sb + off8b + i * pitch);
-                            const double l3 = swp ? e1 : e0;
-                            const double r4 = swp ? e0 : e1;
-                            const double2 l21 = lds128(sb + hb[1] + i * pitch);
-                            const double2 r23 = lds128(sb + hb[2] + i * pitch);
                             double2 &a = acc[J][i];
                             const double2 o = u[i];
-                            a.x = fma(wz1, l21.y, a.x);
-                            a.x = fma(wz1, o.y, a.x);
-                            a.x = fma(wz2, l21.x, a.x);
-                            a.x = fma(wz2, r23.x, a.x);
-                            a.x = fma(wz3, l3, a.x);
-                            a.x = fma(wz3, r23.y, a.x);
-                            a.y = fma(wz1, o.x, a.y);
-                            a.y = fma(wz1, r23.x, a.y);
-                            a.y = fma(wz2, l21.y, a.y);
-                            a.y = fma(wz2, r23.y, a.y);
-                            a.y = fma(wz3, l21.x, a.y);
-                            a.y = fma(wz3, r4, a.y);
+                            if constexpr (NN == 3) {
+                                // chunk = points (z, z+1); halo = z-3 | z-2,z-1 | z+2,z+3 | z+4.
+                                // The two 8-byte halo words come in two loads whose lanes
+                                // alternate (by groups of 8) between z-3 and z+4, so each half
+                                // warp touches 32 distinct banks (an 8-byte load at a 16-byte
+                                // lane stride would be a 2-way bank conflict).
+                                const double e0 = lds64(sb + off8a + i * pitch);
+                                const double e1 = lds64(sb + off8b + i * pitch);
+                                const double l3 = swp ? e1 : e0;
+                                const double r4 = swp ? e0 : e1;
+                                const double2 l21 = lds128(sb + hb[1] + i * pitch);
+                                const double2 r23 = lds128(sb + hb[2] + i * pitch);
+                                a.x = fma(wz[1], l21.y, a.x);
+                                a.x = fma(wz[1], o.y, a.x);
+                                a.x = fma(wz[2], l21.x, a.x);
+                                a.x = fma(wz[2], r23.x, a.x);
+                                a.x = fma(wz[3], l3, a.x);
+                                a.x = fma(wz[3], r23.y, a.x);
+                                a.y = fma(wz[1], o.x, a.y);
+                                a.y = fma(wz[1], r23.x, a.y);
+                                a.y = fma(wz[2], l21.y, a.y);
+                                a.y = fma(wz[2], r23.y, a.y);
+                                a.y = fma(wz[3], l21.x, a.y);
+                                a.y = fma(wz[3], r4, a.y);
+                            } else if constexpr (NN == 2) {
+                                // halo = z-2,z-1 | z+2,z+3: the two neighbouring chunks
+                                const double2 l21 = lds128(sb + hb[0] + i * pitch);
+                                const double2 r23 = lds128(sb + hb[1] + i * pitch);
+                                a.x = fma(wz[1], l21.y, a.x);
+                                a.x = fma(wz[1], o.y, a.x);
+                                a.x = fma(wz[2], l21.x, a.x);
+                                a.x = fma(wz[2], r23.x, a.x);
+                                a.y = fma(wz[1], o.x, a.y);
+                                a.y = fma(wz[1], r23.x, a.y);
+                                a.y = fma(wz[2], l21.y, a.y);
+                                a.y = fma(wz[2], r23.y, a.y);
+                            } else {
+                                // halo = z-1 | z+2: two 8-byte words, fetched pairwise as above
+                                const double e0 = lds64(sb + off8a + i * pitch);
+                                const double e1 = lds64(sb + off8b + i * pitch);
+                                const double l1 = swp ? e1 : e0;
+                                const double r2 = swp ? e0 : e1;
+                                a.x = fma(wz[1], l1, a.x);
+                                a.x = fma(wz[1], o.y, a.x);
+                                a.y = fma(wz[1], o.x, a.y);
+                                a.y = fma(wz[1], r2, a.y);
+                            }
                         }
                     }
                 }
@@ -589,7 +620,7 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
 
                 // ---- the output three planes ahead is born
 #pragma unroll
-                for (int p = 0; p < NP; ++p) acc[(J + 3) % 7][p] = mul2(wx3, u[p]);
+                for (int p = 0; p < NP; ++p) acc[(J + NN) % NS][p] = mul2(wx[NN], u[p]);
 
                 if (last && q + K < nsteps) {
                     const int e = q + K;

@@ -185,7 +185,27 @@ def test_generic_fallback_shapes(oracle, fd, shape):
 @pytest.mark.parametrize("nn", [1, 2, 4, 5, 6])
 def test_other_stencil_orders(oracle, fd, nn):
     cfg = W.custom((12, 10, 14), (0.2, 0.23, 0.17), (1, 0, 1), nbands=2, nn=nn)
-    check(oracle, fd, cfg, W.make_psi(cfg), W.make_veff(cfg))
+    used = check(oracle, fd, cfg, W.make_psi(cfg), W.make_veff(cfg), fd.FD_KERNEL_GENERIC)
+    assert used == fd.FD_KERNEL_GENERIC
+
+
+@pytest.mark.parametrize("nn", [1, 2])
+def test_sweep_kernel_lower_orders(oracle, fd, nn):
+    """the sweep kernel for nn = 1, 2 (3- and 5-slot accumulator rotation, nn
+    halo rows / planes / z points): all BC mixes, several tiles with a ragged one, real and
+    complex with Bloch phases on every axis, several bands per team and several teams."""
+    for bc in itertools.product((0, 1), repeat=3):
+        cfg = W.custom((9, 26, 12), (0.2, 0.23, 0.17), bc, nbands=7, nn=nn)
+        used = check(oracle, fd, cfg, W.make_psi(cfg), W.make_veff(cfg), fd.FD_KERNEL_SWEEP, tyc=8)
+        assert used == fd.FD_KERNEL_SWEEP
+    for bc in [(1, 1, 1), (0, 1, 1), (1, 1, 0)]:
+        k = tuple(kk if b else 0.0 for kk, b in zip((0.25, 0.125, -0.3), bc))
+        cfg = W.custom((10, 20, 8), (0.2, 0.23, 0.17), bc, k=k, complex_=True, nbands=5, nn=nn)
+        used = check(oracle, fd, cfg, W.make_psi(cfg), W.make_veff(cfg), fd.FD_KERNEL_SWEEP, tyc=8)
+        assert used == fd.FD_KERNEL_SWEEP
+    cfg = W.custom((40, 48, 64), (0.2, 0.2, 0.18), (1, 1, 0), nbands=40, nn=nn)
+    used = check(oracle, fd, cfg, W.make_psi(cfg), W.make_veff(cfg), fd.FD_KERNEL_SWEEP)
+    assert used == fd.FD_KERNEL_SWEEP
 
 
 @pytest.mark.parametrize("tyc", [4, 8, 12, 20])
