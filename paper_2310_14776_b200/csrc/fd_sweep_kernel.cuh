@@ -423,191 +423,237 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
                 const unsigned char *const sb = stage0p + st * stage_bytes;
                 const unsigned char *const ub = sb + own_off;
 
-                // ---- own values of the incoming plane
-                double2 u[NP];
-                if (!(m.x & kZero)) {
+                double2 u[NP];  // float64 path: own values of the incoming plane
+                if constexpr (CPLX) {
+                    // complex128: the rows of the thread's column stream through one register
+                    // pair (no copy of the own values is kept: at 168 registers that is what
+                    // lets the loads run ahead; measured +8 % on cfg4, -9 % for float64)
+                    double *const o = obase + (long long)m.y * plane_d;  // used only if m.y is a plane
+                    const bool store_now = m.y != kNoPlane;
+
+                    // One own row of the incoming plane: its value c adds w_x[|d|] c to the outputs
+                    // xl + d in flight (d = -NN: complete after this, stored and gone; d = +NN: born).
+                    auto x_taps_row = [&](int i, const double2 c) {
+                        double2 &lv = acc[(J + NN + 1) % NS][i];
+                        fma2(lv, wx[NN], c);
+                        if (store_now && (row_ok & (1u << i)))
+                            __stcs(reinterpret_cast<double2 *>(o + i * rowd), lv);
 #pragma unroll
-                    for (int i = 0; i < TY; ++i)
+                        for (int d = 1; d < NN; ++d) {
+                            fma2(acc[(J + NS - d) % NS][i], wx[d], c);
+                            fma2(acc[(J + d) % NS][i], wx[d], c);
+                        }
+                        acc[(J + NN) % NS][i] = mul2(wx[NN], c);
+                    };
+
+                    if (!(m.x & kCentre)) {
+                        // ---- halo step (prologue / epilogue of a band segment): x taps only
 #pragma unroll
-                        for (int t = 0; t < TC; ++t)
-                            u[i * TC + t] = lds128(ub + (NN + i) * pitch + t * 16);
-                    if (CPLX && (PH & 1) && yhi) {
-                        // rows past a ragged tile end are wrapped rows: neighbours of the last
-                        // valid rows, so they carry the y Bloch factor like any halo row
+                        for (int i = 0; i < TY; ++i) {
+                            double2 c = make_double2(0.0, 0.0);
+                            if (!(m.x & kZero)) {
+                                c = lds128(ub + (NN + i) * pitch);
+                                if (CPLX && (PH & 1)) {
+                                    // rows past a ragged tile end are wrapped rows: neighbours of the
+                                    // last valid rows, so they carry the y Bloch factor
+                                    if (yhi && r0 + NN + i >= nlo + nmid) c = cmul(c, g.ph_re[1], g.ph_im[1]);
+                                    if (xphase && (m.x & (kWrapLo | kWrapHi)))
+                                        c = cmul(c, g.ph_re[0], (m.x & kWrapLo) ? -g.ph_im[0] : g.ph_im[0]);
+                                }
+                            }
+                            x_taps_row(i, c);
+                        }
+                    } else {
+                        // ---- centre step: the TY + 2 NN rows of the thread's column stream through
+                        // one register pair; a halo row feeds the y taps, an own row also the x taps,
+                        // the diagonal (+ v_eff) and the z taps of its output
+#pragma unroll
+                        for (int rr = 0; rr < TY + 2 * NN; ++rr) {
+                            double2 c = lds128(ub + rr * pitch);
+                            if (CPLX && (PH & 1)) {
+                                if (rr < NN) {
+                                    if (ylo && r0 + rr < nlo) c = cmul(c, g.ph_re[1], -g.ph_im[1]);
+                                } else if (yhi && r0 + rr >= nlo + nmid) {
+                                    c = cmul(c, g.ph_re[1], g.ph_im[1]);
+                                }
+                            }
+#pragma unroll
+                            for (int i = 0; i < TY; ++i) {  // y taps into the other rows
+                                const int d = rr - NN - i;
+                                const int ad = d < 0 ? -d : d;
+                                if (ad >= 1 && ad <= NN) fma2(acc[J][i], wy[ad], c);
+                            }
+                            if (rr >= NN && rr < NN + TY) {
+                                const int i = rr - NN;
+                                x_taps_row(i, c);
+                                double2 &a = acc[J][i];
+                                // diagonal (+ v_eff)
+                                double d0 = wdiag, d1 = wdiag;
+                                if (HAS_V) {
+                                    d0 += lds64(sb + v_off + i * pitchv);
+                                    d1 = d0;
+                                }
+                                a.x = fma(d0, c.x, a.x);
+                                a.y = fma(d1, c.y, a.y);
+                                // z taps
+                                {
+                                    // chunk = one complex point; hz = L_NN .. L_1, R_1 .. R_NN
+                                    double2 hz[2 * ZH];
+#pragma unroll
+                                    for (int k = 0; k < 2 * ZH; ++k) hz[k] = lds128(sb + hb[k] + i * pitch);
+                                    if ((PH & 2) && zphase) {
+#pragma unroll
+                                        for (int k = 0; k < 2 * ZH; ++k) {
+                                            const int wbits = (zwrap >> (2 * k)) & 3;
+                                            if (wbits == 1) hz[k] = cmul(hz[k], g.ph_re[2], -g.ph_im[2]);
+                                            if (wbits == 2) hz[k] = cmul(hz[k], g.ph_re[2], g.ph_im[2]);
+                                        }
+                                    }
+#pragma unroll
+                                    for (int j = 1; j <= NN; ++j) {
+                                        fma2(a, wz[j], hz[NN - j]);
+                                        fma2(a, wz[j], hz[NN + j - 1]);
+                                    }
+                                }
+                            }
+                        }
+                    }
+
+                } else {
+                    // ---- own values of the incoming plane
+                    if (!(m.x & kZero)) {
 #pragma unroll
                         for (int i = 0; i < TY; ++i)
-                            if (r0 + NN + i >= nlo + nmid) {
-#pragma unroll
-                                for (int t = 0; t < TC; ++t)
-                                    u[i * TC + t] = cmul(u[i * TC + t], g.ph_re[1], g.ph_im[1]);
-                            }
-                    }
-                    if (CPLX && (PH & 1) && xphase && (m.x & (kWrapLo | kWrapHi))) {
-                        const double pi_ = (m.x & kWrapLo) ? -g.ph_im[0] : g.ph_im[0];
-#pragma unroll
-                        for (int p = 0; p < NP; ++p) u[p] = cmul(u[p], g.ph_re[0], pi_);
-                    }
-                } else {
-#pragma unroll
-                    for (int p = 0; p < NP; ++p) u[p] = make_double2(0.0, 0.0);
-                }
-
-                // ---- x taps, oldest output first: it is complete after this and leaves
-#pragma unroll
-                for (int p = 0; p < NP; ++p) fma2(acc[(J + NN + 1) % NS][p], wx[NN], u[p]);
-                if (m.y != kNoPlane) {
-                    double *o = obase + (long long)m.y * plane_d;
-#pragma unroll
-                    for (int i = 0; i < TY; ++i)
-                        if (row_ok & (1u << i)) {
 #pragma unroll
                             for (int t = 0; t < TC; ++t)
-                                __stcs(reinterpret_cast<double2 *>(o + i * rowd) + t,
-                                       acc[(J + NN + 1) % NS][i * TC + t]);
-                        }
-                }
+                                u[i * TC + t] = lds128(ub + (NN + i) * pitch + t * 16);
+                    } else {
 #pragma unroll
-                for (int p = 0; p < NP; ++p) {
-#pragma unroll
-                    for (int d = 1; d < NN; ++d) {  // outputs xl - d and xl + d
-                        fma2(acc[(J + NS - d) % NS][p], wx[d], u[p]);
-                        fma2(acc[(J + d) % NS][p], wx[d], u[p]);
+                        for (int p = 0; p < NP; ++p) u[p] = make_double2(0.0, 0.0);
                     }
-                }
 
-                if (m.x & kCentre) {
-                    // ---- diagonal (+ v_eff)
+                    // ---- x taps, oldest output first: it is complete after this and leaves
 #pragma unroll
-                    for (int i = 0; i < TY; ++i) {
-                        double d0 = wdiag, d1 = wdiag;
-                        if (HAS_V) {
-                            if constexpr (CPLX) {
-                                d0 += lds64(sb + v_off + i * pitchv);
-                                d1 = d0;
-                            } else {
+                    for (int p = 0; p < NP; ++p) fma2(acc[(J + NN + 1) % NS][p], wx[NN], u[p]);
+                    if (m.y != kNoPlane) {
+                        double *o = obase + (long long)m.y * plane_d;
+#pragma unroll
+                        for (int i = 0; i < TY; ++i)
+                            if (row_ok & (1u << i)) {
+#pragma unroll
+                                for (int t = 0; t < TC; ++t)
+                                    __stcs(reinterpret_cast<double2 *>(o + i * rowd) + t,
+                                           acc[(J + NN + 1) % NS][i * TC + t]);
+                            }
+                    }
+#pragma unroll
+                    for (int p = 0; p < NP; ++p) {
+#pragma unroll
+                        for (int d = 1; d < NN; ++d) {  // outputs xl - d and xl + d
+                            fma2(acc[(J + NS - d) % NS][p], wx[d], u[p]);
+                            fma2(acc[(J + d) % NS][p], wx[d], u[p]);
+                        }
+                    }
+
+                    if (m.x & kCentre) {
+                        // ---- diagonal (+ v_eff)
+#pragma unroll
+                        for (int i = 0; i < TY; ++i) {
+                            double d0 = wdiag, d1 = wdiag;
+                            if (HAS_V) {
                                 const double2 vv = lds128(sb + v_off + i * pitchv);
                                 d0 += vv.x;
                                 d1 += vv.y;
                             }
+                            acc[J][i].x = fma(d0, u[i].x, acc[J][i].x);
+                            acc[J][i].y = fma(d1, u[i].y, acc[J][i].y);
                         }
-                        acc[J][i].x = fma(d0, u[i].x, acc[J][i].x);
-                        acc[J][i].y = fma(d1, u[i].y, acc[J][i].y);
-                    }
-                    // ---- y taps: stream the TY + 6 rows of the thread's column through
+                        // ---- y taps: stream the TY + 6 rows of the thread's column through
 #pragma unroll
-                    for (int rr = 0; rr < TY + 2 * NN; ++rr) {
-                        if (rr >= NN && rr < NN + TY) continue;  // own rows: already in u
-                        double2 c[TC];
+                        for (int rr = 0; rr < TY + 2 * NN; ++rr) {
+                            if (rr >= NN && rr < NN + TY) continue;  // own rows: already in u
+                            double2 c[TC];
 #pragma unroll
-                        for (int t = 0; t < TC; ++t) c[t] = lds128(ub + rr * pitch + t * 16);
-                        if (CPLX && (PH & 1)) {
-                            if (rr < NN) {
-                                if (ylo && r0 + rr < nlo) {
+                            for (int t = 0; t < TC; ++t) c[t] = lds128(ub + rr * pitch + t * 16);
+#pragma unroll
+                            for (int i = 0; i < TY; ++i) {
+                                const int d = rr - NN - i;
+                                const int ad = d < 0 ? -d : d;
+                                if (ad >= 1 && ad <= NN) {
+#pragma unroll
+                                    for (int t = 0; t < TC; ++t) fma2(acc[J][i * TC + t], wy[ad], c[t]);
+                                }
+                            }
+                        }
+                        // own rows are y neighbours of each other
+#pragma unroll
+                        for (int i = 0; i < TY; ++i)
+#pragma unroll
+                            for (int i2 = 0; i2 < TY; ++i2) {
+                                const int ad = i2 > i ? i2 - i : i - i2;
+                                if (ad >= 1 && ad <= NN) {
 #pragma unroll
                                     for (int t = 0; t < TC; ++t)
-                                        c[t] = cmul(c[t], g.ph_re[1], -g.ph_im[1]);
+                                        fma2(acc[J][i * TC + t], wy[ad], u[i2 * TC + t]);
                                 }
-                            } else if (yhi && r0 + rr >= nlo + nmid) {
-#pragma unroll
-                                for (int t = 0; t < TC; ++t) c[t] = cmul(c[t], g.ph_re[1], g.ph_im[1]);
                             }
-                        }
+                        // ---- z taps
 #pragma unroll
                         for (int i = 0; i < TY; ++i) {
-                            const int d = rr - NN - i;
-                            const int ad = d < 0 ? -d : d;
-                            if (ad >= 1 && ad <= NN) {
-#pragma unroll
-                                for (int t = 0; t < TC; ++t) fma2(acc[J][i * TC + t], wy[ad], c[t]);
-                            }
-                        }
-                    }
-                    // own rows are y neighbours of each other
-#pragma unroll
-                    for (int i = 0; i < TY; ++i)
-#pragma unroll
-                        for (int i2 = 0; i2 < TY; ++i2) {
-                            const int ad = i2 > i ? i2 - i : i - i2;
-                            if (ad >= 1 && ad <= NN) {
-#pragma unroll
-                                for (int t = 0; t < TC; ++t)
-                                    fma2(acc[J][i * TC + t], wy[ad], u[i2 * TC + t]);
-                            }
-                        }
-                    // ---- z taps
-#pragma unroll
-                    for (int i = 0; i < TY; ++i) {
-                        if constexpr (CPLX) {
-                            // chunk = one complex point; hz = L_NN .. L_1, R_1 .. R_NN
-                            double2 hz[2 * ZH];
-#pragma unroll
-                            for (int k = 0; k < 2 * ZH; ++k) hz[k] = lds128(sb + hb[k] + i * pitch);
-                            if ((PH & 2) && zphase) {
-#pragma unroll
-                                for (int k = 0; k < 2 * ZH; ++k) {
-                                    const int wbits = (zwrap >> (2 * k)) & 3;
-                                    if (wbits == 1) hz[k] = cmul(hz[k], g.ph_re[2], -g.ph_im[2]);
-                                    if (wbits == 2) hz[k] = cmul(hz[k], g.ph_re[2], g.ph_im[2]);
+                            {
+                                double2 &a = acc[J][i];
+                                const double2 o = u[i];
+                                if constexpr (NN == 3) {
+                                    // chunk = points (z, z+1); halo = z-3 | z-2,z-1 | z+2,z+3 | z+4.
+                                    // The two 8-byte halo words come in two loads whose lanes
+                                    // alternate (by groups of 8) between z-3 and z+4, so each half
+                                    // warp touches 32 distinct banks (an 8-byte load at a 16-byte
+                                    // lane stride would be a 2-way bank conflict).
+                                    const double e0 = lds64(sb + off8a + i * pitch);
+                                    const double e1 = lds64(sb + off8b + i * pitch);
+                                    const double l3 = swp ? e1 : e0;
+                                    const double r4 = swp ? e0 : e1;
+                                    const double2 l21 = lds128(sb + hb[1] + i * pitch);
+                                    const double2 r23 = lds128(sb + hb[2] + i * pitch);
+                                    a.x = fma(wz[1], l21.y, a.x);
+                                    a.x = fma(wz[1], o.y, a.x);
+                                    a.x = fma(wz[2], l21.x, a.x);
+                                    a.x = fma(wz[2], r23.x, a.x);
+                                    a.x = fma(wz[3], l3, a.x);
+                                    a.x = fma(wz[3], r23.y, a.x);
+                                    a.y = fma(wz[1], o.x, a.y);
+                                    a.y = fma(wz[1], r23.x, a.y);
+                                    a.y = fma(wz[2], l21.y, a.y);
+                                    a.y = fma(wz[2], r23.y, a.y);
+                                    a.y = fma(wz[3], l21.x, a.y);
+                                    a.y = fma(wz[3], r4, a.y);
+                                } else if constexpr (NN == 2) {
+                                    // halo = z-2,z-1 | z+2,z+3: the two neighbouring chunks
+                                    const double2 l21 = lds128(sb + hb[0] + i * pitch);
+                                    const double2 r23 = lds128(sb + hb[1] + i * pitch);
+                                    a.x = fma(wz[1], l21.y, a.x);
+                                    a.x = fma(wz[1], o.y, a.x);
+                                    a.x = fma(wz[2], l21.x, a.x);
+                                    a.x = fma(wz[2], r23.x, a.x);
+                                    a.y = fma(wz[1], o.x, a.y);
+                                    a.y = fma(wz[1], r23.x, a.y);
+                                    a.y = fma(wz[2], l21.y, a.y);
+                                    a.y = fma(wz[2], r23.y, a.y);
+                                } else {
+                                    // halo = z-1 | z+2: two 8-byte words, fetched pairwise as above
+                                    const double e0 = lds64(sb + off8a + i * pitch);
+                                    const double e1 = lds64(sb + off8b + i * pitch);
+                                    const double l1 = swp ? e1 : e0;
+                                    const double r2 = swp ? e0 : e1;
+                                    a.x = fma(wz[1], l1, a.x);
+                                    a.x = fma(wz[1], o.y, a.x);
+                                    a.y = fma(wz[1], o.x, a.y);
+                                    a.y = fma(wz[1], r2, a.y);
                                 }
                             }
-                            double2 &a = acc[J][i];
-#pragma unroll
-                            for (int j = 1; j <= NN; ++j) {
-                                fma2(a, wz[j], hz[NN - j]);
-                                fma2(a, wz[j], hz[NN + j - 1]);
-                            }
-                        } else {
-                            double2 &a = acc[J][i];
-                            const double2 o = u[i];
-                            if constexpr (NN == 3) {
-                                // chunk = points (z, z+1); halo = z-3 | z-2,z-1 | z+2,z+3 | z+4.
-                                // The two 8-byte halo words come in two loads whose lanes
-                                // alternate (by groups of 8) between z-3 and z+4, so each half
-                                // warp touches 32 distinct banks (an 8-byte load at a 16-byte
-                                // lane stride would be a 2-way bank conflict).
-                                const double e0 = lds64(sb + off8a + i * pitch);
-                                const double e1 = lds64(sb + off8b + i * pitch);
-                                const double l3 = swp ? e1 : e0;
-                                const double r4 = swp ? e0 : e1;
-                                const double2 l21 = lds128(sb + hb[1] + i * pitch);
-                                const double2 r23 = lds128(sb + hb[2] + i * pitch);
-                                a.x = fma(wz[1], l21.y, a.x);
-                                a.x = fma(wz[1], o.y, a.x);
-                                a.x = fma(wz[2], l21.x, a.x);
-                                a.x = fma(wz[2], r23.x, a.x);
-                                a.x = fma(wz[3], l3, a.x);
-                                a.x = fma(wz[3], r23.y, a.x);
-                                a.y = fma(wz[1], o.x, a.y);
-                                a.y = fma(wz[1], r23.x, a.y);
-                                a.y = fma(wz[2], l21.y, a.y);
-                                a.y = fma(wz[2], r23.y, a.y);
-                                a.y = fma(wz[3], l21.x, a.y);
-                                a.y = fma(wz[3], r4, a.y);
-                            } else if constexpr (NN == 2) {
-                                // halo = z-2,z-1 | z+2,z+3: the two neighbouring chunks
-                                const double2 l21 = lds128(sb + hb[0] + i * pitch);
-                                const double2 r23 = lds128(sb + hb[1] + i * pitch);
-                                a.x = fma(wz[1], l21.y, a.x);
-                                a.x = fma(wz[1], o.y, a.x);
-                                a.x = fma(wz[2], l21.x, a.x);
-                                a.x = fma(wz[2], r23.x, a.x);
-                                a.y = fma(wz[1], o.x, a.y);
-                                a.y = fma(wz[1], r23.x, a.y);
-                                a.y = fma(wz[2], l21.y, a.y);
-                                a.y = fma(wz[2], r23.y, a.y);
-                            } else {
-                                // halo = z-1 | z+2: two 8-byte words, fetched pairwise as above
-                                const double e0 = lds64(sb + off8a + i * pitch);
-                                const double e1 = lds64(sb + off8b + i * pitch);
-                                const double l1 = swp ? e1 : e0;
-                                const double r2 = swp ? e0 : e1;
-                                a.x = fma(wz[1], l1, a.x);
-                                a.x = fma(wz[1], o.y, a.x);
-                                a.y = fma(wz[1], o.x, a.y);
-                                a.y = fma(wz[1], r2, a.y);
-                            }
                         }
                     }
+
                 }
 
                 // ---- release the slot; the last warp to do so will refill it with step q + K
@@ -618,9 +664,11 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
                     last = atomicInc(&elect_cnt[st], nwarps - 1) == nwarps - 1;
                 }
 
-                // ---- the output three planes ahead is born
+                // ---- float64 path: the output NN planes ahead is born
+                if constexpr (!CPLX) {
 #pragma unroll
-                for (int p = 0; p < NP; ++p) acc[(J + NN) % NS][p] = mul2(wx[NN], u[p]);
+                    for (int p = 0; p < NP; ++p) acc[(J + NN) % NS][p] = mul2(wx[NN], u[p]);
+                }
 
                 if (last && q + K < nsteps) {
                     const int e = q + K;
