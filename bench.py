@@ -36,8 +36,10 @@ DEFAULT_WORKLOAD = "cfg3"
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the sweep kernel from the committed
 # `ncu --set full` capture (profiles/), keyed by workload; None until a capture exists.
 NCU_TRAFFIC_BYTES = {
-    # profiles/r1i_sweep_ncu_full.md: dram__bytes_read.sum + dram__bytes_write.sum per launch
-    "cfg3_96c_periodic_f64": 3698447000,
+    # profiles/r1n_sweep_ncu_full.md (cfg3, cfg4), r1i_sweep_ncu_full.md (cfg5):
+    # dram__bytes_read.sum + dram__bytes_write.sum per launch
+    "cfg3_96c_periodic_f64": 3698254000,
+    "cfg4_72c_bloch_c128": 1547743000,
     "cfg5_slab_128x128x192_f64": 22225838000,
 }
 
