@@ -301,9 +301,9 @@ const char *fd_strerror(int status)
 int fd_plan_set_kernel(fd_plan *plan, int32_t kernel, int32_t param)
 {
     if (!plan) return FD_ERR_INVALID;
-    plan->forced = (kernel != FD_KERNEL_AUTO);
     if (kernel == FD_KERNEL_GENERIC) {
         plan->kernel = FD_KERNEL_GENERIC;
+        plan->forced = 1;
         return FD_OK;
     }
     if (kernel != FD_KERNEL_AUTO && kernel != FD_KERNEL_SWEEP) return FD_ERR_INVALID;
@@ -314,12 +314,10 @@ int fd_plan_set_kernel(fd_plan *plan, int32_t kernel, int32_t param)
             return FD_ERR_CUDA;
         }
     }
-    if (plan->sweep.supported) {
-        plan->kernel = FD_KERNEL_SWEEP;
-        return FD_OK;
-    }
-    if (kernel == FD_KERNEL_SWEEP) return FD_ERR_UNSUPPORTED;
-    plan->kernel = FD_KERNEL_GENERIC;
+    if (!plan->sweep.supported && kernel == FD_KERNEL_SWEEP) return FD_ERR_UNSUPPORTED;
+    // a failed request above leaves the family and the per-batch choice as they were
+    plan->kernel = plan->sweep.supported ? FD_KERNEL_SWEEP : FD_KERNEL_GENERIC;
+    plan->forced = (kernel != FD_KERNEL_AUTO);
     return FD_OK;
 }
 
