@@ -17,6 +17,13 @@ struct FdGeom {
     double ph_re[3], ph_im[3];   // exp(+2 pi i k_d): factor when a tap runs past the UPPER end
 };
 
+// Limits shared by the sweep kernel (fd_sweep_kernel.cuh) and its host side (fd_sweep.cu)
+constexpr int kFdSweepMaxThreads = 384;      // CTA size bound (168 registers per thread)
+constexpr int kFdSweepMaxStages = 8;         // mbarrier slots reserved per ring
+constexpr int kFdSweepCtlBytes = 256;        // full[8] + empty[8] mbarriers, 8 election counters, misc
+constexpr int kFdSweepSmemMax = 227 * 1024;  // dynamic shared memory per CTA on sm_100
+constexpr int kFdSweepPlaneBits = 26;        // bits of a (band, x) plane index in a step-table entry
+
 // Launch description of the sweep kernel, fixed at plan time (tile choice) -- see fd_sweep.cu.
 struct FdSweepCfg {
     int supported;     // 0: plan cannot use the sweep kernel

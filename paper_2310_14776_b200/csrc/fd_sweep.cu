@@ -4,10 +4,10 @@
 
 namespace {
 
-constexpr int kMaxThreads = 384;
-constexpr int kCtlBytes = 256;   // must match fd_sweep_kernel.cuh
-constexpr int kSmemMax = 227 * 1024;
-constexpr int kPlaneBits = 26;   // must match fd_sweep_kernel.cuh
+constexpr int kMaxThreads = kFdSweepMaxThreads;
+constexpr int kCtlBytes = kFdSweepCtlBytes;
+constexpr int kSmemMax = kFdSweepSmemMax;
+constexpr int kPlaneBits = kFdSweepPlaneBits;
 
 inline int ceil_div(int a, int b) { return (a + b - 1) / b; }
 

@@ -56,14 +56,14 @@
 
 namespace {
 
-constexpr int kMaxThreads = 384;
-constexpr int kMaxStages = 8;
-constexpr int kCtlBytes = 256;   // full[8] + empty[8] mbarriers, 8 election counters, misc
-constexpr int kSmemMax = 227 * 1024;
+constexpr int kMaxThreads = kFdSweepMaxThreads;
+constexpr int kMaxStages = kFdSweepMaxStages;
+constexpr int kCtlBytes = kFdSweepCtlBytes;
+constexpr int kSmemMax = kFdSweepSmemMax;
 
 // Step-table entry (8 bytes): .x = plane to load (band*nx + x, low kPlaneBits bits) | flags,
 // .y = output plane completed by the step (band*nx + x) or ~0.
-constexpr int kPlaneBits = 26;
+constexpr int kPlaneBits = kFdSweepPlaneBits;
 constexpr unsigned kPlaneMask = (1u << kPlaneBits) - 1u;
 constexpr unsigned kWrapLo = 1u << 26;   // plane wrapped from below 0: Bloch factor conj(ph_x)
 constexpr unsigned kWrapHi = 1u << 27;   // plane wrapped from past nx-1: Bloch factor ph_x
