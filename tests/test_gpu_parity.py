@@ -385,6 +385,7 @@ def test_many_short_teams_more_ctas_than_sms(oracle, fd, monkeypatch, xchunk):
         want = oracle.apply(cfg.shape, cfg.h, 3, cfg.bc, cfg.k if cplx else None, psi, v)
         assert np.max(np.abs(got - want)) <= parity_tol(cfg.h, 3, psi, v)
 
+
 def test_one_plan_two_streams_concurrently(oracle, fd):
     """A plan is immutable: applies of the same plan on two streams may overlap."""
     cfg = W.custom((32, 32, 32), (0.2,) * 3, (1, 1, 1), nbands=24)
