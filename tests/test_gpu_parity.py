@@ -436,3 +436,44 @@ def test_scaled_laplacian_plans(oracle, fd, scale):
                 fd.fd_destroy(plan)
     with pytest.raises(fd.FDError):
         fd.fd_create_scaled((8, 8, 8), (0.2,) * 3, 3, (1, 1, 1), None, fd.FD_F64, 0, float("inf"))
+
+
+def test_guard_bands_no_out_of_bounds_access(oracle, fd):
+    """psi, v_eff and out sit inside larger buffers whose surroundings are NaN (inputs) or a
+    sentinel (output): an out-of-bounds read would poison the result, an out-of-bounds write would
+    change the guard band.  Ragged y tiles, all boundary mixes, both kernels, both dtypes."""
+    pad = 4096  # elements of the buffer's dtype on either side
+    for shape, bc, cplx, k, nn in [((12, 26, 16), (1, 1, 1), False, None, 3),
+                                   ((9, 22, 12), (0, 1, 0), False, None, 3),
+                                   ((10, 18, 8), (1, 1, 1), True, (0.25, 0.125, -0.3), 3),
+                                   ((9, 26, 12), (1, 0, 1), False, None, 2),
+                                   ((8, 8, 8), (0, 0, 0), False, None, 3)]:
+        cfg = W.custom(shape, (0.2, 0.21, 0.18), bc, k=k or (0, 0, 0), complex_=cplx, nbands=5,
+                       nn=nn)
+        psi, v = W.make_psi(cfg), W.make_veff(cfg)
+        want = oracle.apply(cfg.shape, cfg.h, nn, cfg.bc, k, psi, v)
+        tol = parity_tol(cfg.h, nn, psi, v)
+        tdt = torch.complex128 if cplx else torch.float64
+        n = psi.size
+        big_in = torch.full((n + 2 * pad,), float("nan"), dtype=tdt, device="cuda")
+        big_v = torch.full((v.size + 2 * pad,), float("nan"), dtype=torch.float64, device="cuda")
+        d_psi = big_in[pad:pad + n].view(psi.shape)
+        d_v = big_v[pad:pad + v.size].view(v.shape)
+        d_psi.copy_(torch.from_numpy(psi))
+        d_v.copy_(torch.from_numpy(v))
+        for kern in (fd.FD_KERNEL_SWEEP, fd.FD_KERNEL_GENERIC):
+            plan = fd.fd_create(cfg.shape, cfg.h, nn, cfg.bc, k,
+                                fd.FD_C128 if cplx else fd.FD_F64, 0)
+            try:
+                fd.fd_plan_set_kernel(plan, kern, 8 if kern == fd.FD_KERNEL_SWEEP else 0)
+                big_out = torch.full((n + 2 * pad,), 12345.0, dtype=tdt, device="cuda")
+                d_out = big_out[pad:pad + n].view(psi.shape)
+                fd.fd_apply_hamiltonian(plan, d_psi, d_v, d_out)
+                torch.cuda.synchronize()
+                got = d_out.cpu().numpy()
+                assert np.isfinite(got).all(), f"{shape} {bc} kernel {kern}: read outside psi/v_eff"
+                assert np.max(np.abs(got - want)) <= tol
+                guards = torch.cat([big_out[:pad], big_out[pad + n:]])
+                assert bool((guards == 12345.0).all()), f"{shape} {bc} kernel {kern}: wrote outside out"
+            finally:
+                fd.fd_destroy(plan)
