@@ -264,24 +264,30 @@ def run_ours(args):
     value, ms_step = aggregate(ms_local, units, world, reduce_max)
 
     # ---- end to end: pinned HOST buffers through fd_apply_hamiltonian_host ------------------
-    e2e_steps = max(1, min(3, args.steps))
+    e2e_steps = max(1, min(7, args.steps))
     h_psi = torch.empty(d_psi.shape, dtype=tdt).pin_memory()
     h_psi.copy_(d_psi)
     h_v = torch.from_numpy(v_host).pin_memory()
     h_out = torch.empty(d_psi.shape, dtype=tdt).pin_memory()
     fd.fd_apply_hamiltonian_host(plan, h_psi, h_v, h_out)      # warm-up
     sync_all()
-    t0 = time.perf_counter()
+    per_step = []
     for _ in range(e2e_steps):
+        t0 = time.perf_counter()
         fd.fd_apply_hamiltonian_host(plan, h_psi, h_v, h_out)  # blocks until out is on the host
-    e2e_ms_local = (time.perf_counter() - t0) * 1e3 / e2e_steps
+        per_step.append((time.perf_counter() - t0) * 1e3)
+    # the host side of the box is shared: an occasional call takes 2-3x as long (PCIe / host
+    # memory traffic of other tenants), so the median step is reported and the mean kept beside it
+    e2e_ms_local = sorted(per_step)[len(per_step) // 2]
+    e2e_ms_mean = sum(per_step) / len(per_step)
     e2e_value, _ = aggregate(e2e_ms_local, units, world, reduce_max)
     ok = bool(torch.equal(h_out[:2], d_out[:2].cpu()))
     band_bytes = cfg.npoints * cfg.elem_bytes
     e2e = {"value": e2e_value, "unit": UNIT,
            "h2d_bytes_per_step": cfg.nbands * band_bytes + cfg.npoints * 8,
            "d2h_bytes_per_step": cfg.nbands * band_bytes,
-           "steps": e2e_steps, "ms_per_step": e2e_ms_local, "matches_device_path": ok,
+           "steps": e2e_steps, "ms_per_step": e2e_ms_local, "ms_per_step_mean": e2e_ms_mean,
+           "stat": "median step", "matches_device_path": ok,
            "api": "fd_apply_hamiltonian_host (pinned host buffers, 3-slot H2D/kernel/D2H ring)"}
 
     if rank == 0:
