@@ -89,8 +89,10 @@ int apply_device(const fd_plan *plan, const void *psi, const double *v_eff, void
     return FD_OK;
 }
 
+}  // namespace
+
 // "tyc=24,xchunk=32,kernel=1": debugging / tuning knob read once at fd_create.
-int tune_value(const char *key)
+int fd_tune_value(const char *key)
 {
     const char *env = getenv("FDHAM_TUNE");
     if (!env) return 0;
@@ -104,6 +106,8 @@ int tune_value(const char *key)
     return 0;
 }
 
+namespace {
+int tune_value(const char *key) { return fd_tune_value(key); }
 }  // namespace
 
 extern "C" {
@@ -169,7 +173,7 @@ int fd_create_scaled(fd_plan **plan_out, const int32_t shape[3], const double h[
         }
     }
 
-    fd_sweep_configure(p, tune_value("tyc"), tune_value("xchunk"));
+    fd_sweep_configure(p, tune_value("tyc"), tune_value("xchunk"), tune_value("stages"));
     p->kernel = p->sweep.supported ? FD_KERNEL_SWEEP : FD_KERNEL_GENERIC;
     if (tune_value("kernel") == FD_KERNEL_GENERIC) p->kernel = FD_KERNEL_GENERIC;
     if (tune_value("kernel") != 0) p->forced = 1;
@@ -308,7 +312,7 @@ int fd_plan_set_kernel(fd_plan *plan, int32_t kernel, int32_t param)
     }
     if (kernel != FD_KERNEL_AUTO && kernel != FD_KERNEL_SWEEP) return FD_ERR_INVALID;
     if (param != 0 || kernel == FD_KERNEL_SWEEP) {
-        fd_sweep_configure(plan, param, plan->sweep.xchunk);
+        fd_sweep_configure(plan, param, plan->sweep.xchunk, plan->sweep.stages_req);
         if (plan->sweep.supported && fd_sweep_prepare(plan) != cudaSuccess) {
             cudaGetLastError();
             return FD_ERR_CUDA;

@@ -18,7 +18,8 @@ struct FdGeom {
 };
 
 // Limits shared by the sweep kernel (fd_sweep_kernel.cuh) and its host side (fd_sweep.cu)
-constexpr int kFdSweepMaxThreads = 384;      // CTA size bound (168 registers per thread)
+constexpr int kFdSweepMaxThreads = 384;      // compute threads per CTA (160 registers each)
+constexpr int kFdSweepProducerThreads = 128; // + one warpgroup whose first lane issues the TMA loads
 constexpr int kFdSweepMaxStages = 8;         // mbarrier slots reserved per ring
 constexpr int kFdSweepCtlBytes = 256;        // full[8] + empty[8] mbarriers, 8 election counters, misc
 constexpr int kFdSweepSmemMax = 227 * 1024;  // dynamic shared memory per CTA on sm_100
@@ -32,7 +33,8 @@ struct FdSweepCfg {
     int rowgroups;     // row groups per CTA; tile rows tyc = rowgroups * ty
     int tyc;           // y rows per CTA tile
     int nytiles;       // ceil(ny / tyc)
-    int threads;       // CTA size (multiple of 32)
+    int threads;       // compute threads (multiple of 32)
+    int threads_wg;    // the same rounded up to whole warpgroups: first thread of the producer group
     int stages;        // smem ring depth
     int zb_bytes;      // zero block at the start of every stage (zero-BC z halo source), else 0
     int v_off;         // offset of the v_eff rows inside a stage
@@ -43,6 +45,7 @@ struct FdSweepCfg {
     int smem_bytes;    // dynamic shared memory per CTA
     int max_teams;     // teams of nytiles CTAs resident at once (one CTA per SM)
     int xchunk;        // 0 = persistent teams, else x planes per team (tuning knob)
+    int stages_req;    // 0 = as many ring slots as fit, else an upper bound (tuning knob)
 };
 
 struct fd_plan {
@@ -73,8 +76,10 @@ inline FdSweepKernelFn fd_sweep_pick_cplx(int rowd, int has_v, int ph, int nn)
     if (ph == 1) return fd_sweep_pick_cplx_ph1(rowd, has_v, nn);
     return fd_sweep_pick_cplx_ph3(rowd, has_v, nn);
 }
+// fd_api.cu: integer value of `key` in the FDHAM_TUNE environment variable (0 if absent)
+int fd_tune_value(const char *key);
 // fd_sweep.cu
-void fd_sweep_configure(fd_plan *plan, int tyc_override, int xchunk_override);
+void fd_sweep_configure(fd_plan *plan, int tyc_override, int xchunk_override, int stages_override);
 cudaError_t fd_sweep_prepare(fd_plan *plan);  // shared-memory opt-in of the plan's kernels
 cudaError_t fd_launch_sweep(const fd_plan *plan, const void *psi, const double *v_eff, void *out,
                             int64_t nbands, cudaStream_t stream, int *nlaunches);

@@ -13,15 +13,17 @@ inline int ceil_div(int a, int b) { return (a + b - 1) / b; }
 
 }  // namespace
 
-void fd_sweep_configure(fd_plan *plan, int tyc_override, int xchunk_override)
+void fd_sweep_configure(fd_plan *plan, int tyc_override, int xchunk_override, int stages_override)
 {
     FdSweepCfg &c = plan->sweep;
     const FdGeom &g = plan->g;
     c = FdSweepCfg{};
     c.xchunk = xchunk_override;  // 0 = automatic (persistent teams), else planes per team
+    c.stages_req = stages_override;
     if (g.nn > 3) return;  // 2 nn + 1 accumulator planes: the register budget ends at nn = 3
     const int halo = 2 * g.nn;
     if (g.n[0] < 8 || g.n[1] < 8 || g.n[2] < 8 || (g.n[2] & 1)) return;
+    if (g.n[0] > 65536) return;  // x index + 2 nn in 17 bits of a step-table entry
     c.ty = 4;
     c.tc = 1;
     const int pitch = g.n[2] * (g.cplx ? 16 : 8);
@@ -54,6 +56,7 @@ void fd_sweep_configure(fd_plan *plan, int tyc_override, int xchunk_override)
     c.rowgroups = tyc / c.ty;
     c.nytiles = ceil_div(g.n[1], tyc);
     c.threads = ceil_div(c.rowgroups * c.lanes, 32) * 32;
+    c.threads_wg = ceil_div(c.threads, 128) * 128;
     c.stage_bytes = stage_bytes(tyc);
     c.v_off = c.zb_bytes + (tyc + halo) * pitch;
     int tab_bytes = 16384;
@@ -64,6 +67,7 @@ void fd_sweep_configure(fd_plan *plan, int tyc_override, int xchunk_override)
     }
     if (stages < 2) return;
     if (stages > 6) stages = 6;
+    if (stages_override >= 2 && stages_override < stages) stages = stages_override;
     c.stages = stages;
     tab_bytes = (kSmemMax - kCtlBytes - stages * c.stage_bytes) / 128 * 128;
     if (tab_bytes > 65536) tab_bytes = 65536;
@@ -92,13 +96,15 @@ FdSweepKernelFn kernel_for(const fd_plan *plan, bool has_v)
 
 }  // namespace
 
+// The shared-memory opt-in belongs to the kernel instantiation, not to the plan (plans of different
+// shapes share the run-time-pitch instantiations): always the architectural maximum, so that a later
+// plan with a smaller footprint never lowers the limit under an earlier one.
 cudaError_t fd_sweep_prepare(fd_plan *plan)
 {
-    const FdSweepCfg &c = plan->sweep;
     for (int has_v = 0; has_v < 2; ++has_v) {
         cudaError_t e = cudaFuncSetAttribute(reinterpret_cast<const void *>(kernel_for(plan, has_v)),
                                              cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             c.smem_bytes);
+                                             kSmemMax);
         if (e != cudaSuccess) return e;
     }
     return cudaSuccess;
@@ -135,7 +141,8 @@ cudaError_t fd_launch_sweep(const fd_plan *plan, const void *psi, const double *
         if (nblocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
         const double *p = static_cast<const double *>(psi) + b0 * band_d;
         double *o = static_cast<double *>(out) + b0 * band_d;
-        kern<<<dim3((unsigned)nblocks), dim3((unsigned)c.threads), (size_t)c.smem_bytes, stream>>>(
+        kern<<<dim3((unsigned)nblocks), dim3((unsigned)(c.threads_wg + kFdSweepProducerThreads)), (size_t)c.smem_bytes,
+               stream>>>(
             g, c, p, v_eff, o, total, (int)quota);
         cudaError_t e = cudaPeekAtLastError();
         if (e != cudaSuccess) return e;

@@ -56,21 +56,23 @@
 
 namespace {
 
-constexpr int kMaxThreads = kFdSweepMaxThreads;
+constexpr int kMaxThreads = kFdSweepMaxThreads;          // compute threads
+constexpr int kProducerThreads = kFdSweepProducerThreads;  // one more warpgroup: its first lane issues the loads
 constexpr int kMaxStages = kFdSweepMaxStages;
 constexpr int kCtlBytes = kFdSweepCtlBytes;
 constexpr int kSmemMax = kFdSweepSmemMax;
 
-// Step-table entry (8 bytes): .x = plane to load (band*nx + x, low kPlaneBits bits) | flags,
-// .y = output plane completed by the step (band*nx + x) or ~0.
-constexpr int kPlaneBits = kFdSweepPlaneBits;
-constexpr unsigned kPlaneMask = (1u << kPlaneBits) - 1u;
+// Step-table entry (8 bytes): .x = flags | (xl + nn), xl = x index of the plane the step brings in
+// (-nn .. nx+nn-1: the halo steps of a band segment lie outside the band), .y = band * nx (plane
+// index of the band's first plane).  Load plane = .y + xl (+- nx when wrapped), completed output
+// plane = .y + xl - nn (flag kOut), v_eff plane of a centre step = xl.
+constexpr unsigned kXMask = (1u << 17) - 1u;
 constexpr unsigned kWrapLo = 1u << 26;   // plane wrapped from below 0: Bloch factor conj(ph_x)
 constexpr unsigned kWrapHi = 1u << 27;   // plane wrapped from past nx-1: Bloch factor ph_x
 constexpr unsigned kKeepL2 = 1u << 28;   // load evict_last: the x wrap reads this plane again
 constexpr unsigned kZero = 1u << 29;     // no load: the plane lies outside a zero-BC x axis
 constexpr unsigned kCentre = 1u << 30;   // centre plane: y/z taps, diagonal and v_eff this step
-constexpr unsigned kNoPlane = 0xffffffffu;
+constexpr unsigned kOut = 1u << 31;      // the step completes output plane xl - nn
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p)
 {
@@ -210,18 +212,15 @@ struct TeamRange {
         }
         const int xl = x0 - hn + s;
         uint2 m;
-        if (xl < 0) {
-            m.x = per_x ? ((unsigned)(band * nx + xl + nx) | kWrapLo) : kZero;
-        } else if (xl >= nx) {
-            m.x = per_x ? ((unsigned)(band * nx + xl - nx) | kWrapHi) : kZero;
-        } else {
-            m.x = (unsigned)(band * nx + xl);
-        }
+        m.x = (unsigned)(xl + hn);
+        m.y = (unsigned)(band * nx);
+        if (xl < 0) m.x |= per_x ? kWrapLo : kZero;
+        if (xl >= nx) m.x |= per_x ? kWrapHi : kZero;
         // a whole periodic band: its last three planes (read first, as the wrap) and its first
         // three come round again ~nx steps later
         if (per_x && x0 == 0 && len == nx && s < 2 * hn) m.x |= kKeepL2;
         if (s >= hn && s < len + hn) m.x |= kCentre;
-        m.y = (s >= 2 * hn) ? (unsigned)(band * nx + x0 + s - 2 * hn) : kNoPlane;
+        if (s >= 2 * hn) m.x |= kOut;
         return m;
     }
 };
@@ -229,7 +228,7 @@ struct TeamRange {
 // PH (complex only): which Bloch-phase code is compiled in -- bit 0: x and y wraps, bit 1: z wraps.
 // NN: stencil half width (1..3); 2 NN + 1 register accumulators per point, unrolled 2 NN + 1 times.
 template <bool CPLX, bool HAS_V, int ROWD, int PH, int NN>
-__global__ void __launch_bounds__(kMaxThreads, 1)
+__global__ void __launch_bounds__(kMaxThreads + kProducerThreads, 1)
 fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSweepCfg cfg,
                 const double *__restrict__ psi, const double *__restrict__ v_eff,
                 double *__restrict__ out, const long long total_planes, const int quota)
@@ -244,8 +243,6 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
     const uint32_t smem_base = smem_u32(smem);
     const uint32_t full_bar = smem_base;         // kMaxStages x 8 bytes
     const uint32_t empty_bar = smem_base + 64;   // kMaxStages x 8 bytes
-    unsigned int *const elect_cnt = reinterpret_cast<unsigned int *>(smem + 128);
-    unsigned long long *const l2pol = reinterpret_cast<unsigned long long *>(smem + 168);
     const uint2 *const tabp = reinterpret_cast<const uint2 *>(smem + cfg.tab_off);
     const unsigned char *const stage0p = smem + cfg.stage_off;
     const uint32_t stage0 = smem_base + (uint32_t)cfg.stage_off;
@@ -258,7 +255,7 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
     const int pitchv = CPLX ? pitch / 2 : pitch;         // bytes per z row of v_eff
     const int cpr = rowd >> 1;                           // 16-byte chunks per row
     const int tid = threadIdx.x;
-    const unsigned nwarps = blockDim.x >> 5;
+    const unsigned nwarps = (unsigned)cfg.threads >> 5;  // compute warps (the empty barriers count them)
 
     const int yt = (int)(blockIdx.x % (unsigned)cfg.nytiles);
     const long long team = blockIdx.x / (unsigned)cfg.nytiles;
@@ -287,14 +284,12 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
         for (int i = 0; i < K; ++i) {
             mbar_init(full_bar + 8 * i, 1);
             mbar_init(empty_bar + 8 * i, nwarps);
-            elect_cnt[i] = 0;
         }
-        l2pol[0] = policy_evict_last();
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     for (int e = tid; e <= nsteps; e += blockDim.x)  // one entry past the end: prefetched, unused
         reinterpret_cast<uint2 *>(smem + cfg.tab_off)[e] =
-            (e < nsteps) ? tr.entry(e, per_x) : make_uint2(kZero, kNoPlane);
+            (e < nsteps) ? tr.entry(e, per_x) : make_uint2(kZero, 0u);
     for (int st = 0; st < K; ++st) {
         unsigned char *sb = smem + cfg.stage_off + (size_t)st * stage_bytes;
         for (int i = tid; i < (int)(zb >> 3); i += blockDim.x)  // the zero block
@@ -312,43 +307,58 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     __syncthreads();
 
-    // ---- the load of table entry e into ring slot s (one thread) --------------------------------
-    auto issue = [&](int e, uint32_t s) {
-        const unsigned mx = tabp[e].x;
-        const uint32_t bar = full_bar + 8 * s;
-        if (mx & kZero) {
-            mbar_arrive(bar);
-            return;
+    // ---- producer: the first lane of the extra warpgroup refills every slot as soon as the compute
+    // warps have released it.  (Issuing from a compute warp put ~10 % on the step: the warp that
+    // releases a slot last is the one every other warp is waiting for.)  The v_eff rows (L2 hits) go
+    // first: behind the psi rows (DRAM) they would arrive last and hold the stage back.
+    if (tid >= cfg.threads_wg) {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 24;");
+        if (tid != cfg.threads_wg) return;
+        const unsigned long long pol = policy_evict_last();
+        uint32_t s = 0, ph = 0;  // ring slot and pass parity: pass p waits for the release of pass p - 1
+        for (int e = 0; e < nsteps; ++e) {
+            if (e >= K) mbar_wait(empty_bar + 8 * s, ph ^ 1u);
+            const uint2 me = tabp[e];
+            const unsigned mx = me.x;
+            const uint32_t bar = full_bar + 8 * s;
+            if (mx & kZero) {
+                mbar_arrive(bar);
+            } else {
+                const uint32_t dst = stage0 + s * stage_bytes + zb;
+                const int xl = (int)(mx & kXMask) - NN;  // wrapped planes come from the other end
+                const int xs = xl + ((mx & kWrapLo) ? nx : 0) - ((mx & kWrapHi) ? nx : 0);
+                const double *src = psi + (long long)(me.y + (unsigned)xs) * plane_d;
+                const bool with_v = HAS_V && (mx & kCentre);
+                mbar_expect_tx(bar, tx_psi + (with_v ? tx_v : 0u));
+                if (with_v)
+                    bulk_g2s_hint(stage0 + s * stage_bytes + (uint32_t)cfg.v_off,
+                                  v_eff + ((long long)xl * ny + y0) * nz, tx_v, bar, pol);
+                if (mx & kKeepL2) {
+                    if (per_y && nlo > 0)
+                        bulk_g2s_hint(dst, src + (long long)(ny - nlo) * rowd, (uint32_t)(nlo * pitch),
+                                      bar, pol);
+                    bulk_g2s_hint(dst + nlo * pitch, src + (long long)(y0 - NN + nlo) * rowd,
+                                  (uint32_t)(nmid * pitch), bar, pol);
+                    if (per_y && nhi > 0)
+                        bulk_g2s_hint(dst + (nlo + nmid) * pitch, src, (uint32_t)(nhi * pitch), bar, pol);
+                } else {
+                    if (per_y && nlo > 0)
+                        bulk_g2s(dst, src + (long long)(ny - nlo) * rowd, (uint32_t)(nlo * pitch), bar);
+                    bulk_g2s(dst + nlo * pitch, src + (long long)(y0 - NN + nlo) * rowd,
+                             (uint32_t)(nmid * pitch), bar);
+                    if (per_y && nhi > 0)
+                        bulk_g2s(dst + (nlo + nmid) * pitch, src, (uint32_t)(nhi * pitch), bar);
+                }
+            }
+            if (++s == (uint32_t)K) {
+                s = 0;
+                ph ^= 1u;
+            }
         }
-        const uint32_t dst = stage0 + s * stage_bytes + zb;
-        const double *src = psi + (long long)(mx & kPlaneMask) * plane_d;
-        const bool with_v = HAS_V && (mx & kCentre);
-        mbar_expect_tx(bar, tx_psi + (with_v ? tx_v : 0u));
-        if (mx & kKeepL2) {
-            const unsigned long long pol = l2pol[0];
-            if (per_y && nlo > 0)
-                bulk_g2s_hint(dst, src + (long long)(ny - nlo) * rowd, (uint32_t)(nlo * pitch), bar,
-                              pol);
-            bulk_g2s_hint(dst + nlo * pitch, src + (long long)(y0 - NN + nlo) * rowd,
-                          (uint32_t)(nmid * pitch), bar, pol);
-            if (per_y && nhi > 0)
-                bulk_g2s_hint(dst + (nlo + nmid) * pitch, src, (uint32_t)(nhi * pitch), bar, pol);
-        } else {
-            if (per_y && nlo > 0)
-                bulk_g2s(dst, src + (long long)(ny - nlo) * rowd, (uint32_t)(nlo * pitch), bar);
-            bulk_g2s(dst + nlo * pitch, src + (long long)(y0 - NN + nlo) * rowd,
-                     (uint32_t)(nmid * pitch), bar);
-            if (per_y && nhi > 0)
-                bulk_g2s(dst + (nlo + nmid) * pitch, src, (uint32_t)(nhi * pitch), bar);
-        }
-        if (with_v) {
-            const int xc = (int)((mx & kPlaneMask) % (unsigned)nx);
-            bulk_g2s_hint(stage0 + s * stage_bytes + (uint32_t)cfg.v_off,
-                          v_eff + ((long long)xc * ny + y0) * nz, tx_v, bar, l2pol[0]);
-        }
-    };
-    if (tid == 0)
-        for (int i = 0; i < K && i < nsteps; ++i) issue(i, (uint32_t)i);
+        return;
+    }
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 160;");
+    if (tid >= cfg.threads) return;  // warps that only fill up the last compute warpgroup
 
     // ---- thread -> micro tile ---------------------------------------------------------------
     int rg = tid / cfg.lanes;
@@ -428,8 +438,9 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
                     // complex128: the rows of the thread's column stream through one register
                     // pair (no copy of the own values is kept: at 168 registers that is what
                     // lets the loads run ahead; measured +8 % on cfg4, -9 % for float64)
-                    double *const o = obase + (long long)m.y * plane_d;  // used only if m.y is a plane
-                    const bool store_now = m.y != kNoPlane;
+                    // used only if the step completes an output plane
+                    double *const o = obase + (long long)(m.y + (m.x & kXMask) - 2 * NN) * plane_d;
+                    const bool store_now = (m.x & kOut) != 0;
 
                     // One own row of the incoming plane: its value c adds w_x[|d|] c to the outputs
                     // xl + d in flight (d = -NN: complete after this, stored and gone; d = +NN: born).
@@ -535,8 +546,8 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
                     // ---- x taps, oldest output first: it is complete after this and leaves
 #pragma unroll
                     for (int p = 0; p < NP; ++p) fma2(acc[(J + NN + 1) % NS][p], wx[NN], u[p]);
-                    if (m.y != kNoPlane) {
-                        double *o = obase + (long long)m.y * plane_d;
+                    if (m.x & kOut) {
+                        double *o = obase + (long long)(m.y + (m.x & kXMask) - 2 * NN) * plane_d;
 #pragma unroll
                         for (int i = 0; i < TY; ++i)
                             if (row_ok & (1u << i)) {
@@ -656,24 +667,14 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
 
                 }
 
-                // ---- release the slot; the last warp to do so will refill it with step q + K
-                bool last = false;
+                // ---- release the slot (the producer refills it once every compute warp has)
                 __syncwarp();
-                if (elect_one()) {
-                    mbar_arrive(empty_bar + 8 * st);
-                    last = atomicInc(&elect_cnt[st], nwarps - 1) == nwarps - 1;
-                }
+                if (elect_one()) mbar_arrive(empty_bar + 8 * st);
 
                 // ---- float64 path: the output NN planes ahead is born
                 if constexpr (!CPLX) {
 #pragma unroll
                     for (int p = 0; p < NP; ++p) acc[(J + NN) % NS][p] = mul2(wx[NN], u[p]);
-                }
-
-                if (last && q + K < nsteps) {
-                    const int e = q + K;
-                    mbar_wait(empty_bar + 8 * st, par);
-                    issue(e, st);
                 }
                 if (++st == (uint32_t)K) {
                     st = 0;
