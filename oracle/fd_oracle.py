@@ -44,6 +44,27 @@ def _load():
         lib.fd_oracle_points.restype = ctypes.c_int
         lib.fd_oracle_dense.argtypes = [i32p, f64p, ctypes.c_int32, i32p, f64p, f64p, vp]
         lib.fd_oracle_dense.restype = ctypes.c_int
+        c128p = ctypes.c_void_p
+        lib.fd_oracle_expect.argtypes = [i32p, f64p, ctypes.c_int32, i32p, f64p, ctypes.c_int32,
+                                         vp, f64p, vp, ctypes.c_int64, ctypes.c_double, c128p, f64p]
+        lib.fd_oracle_expect.restype = ctypes.c_int
+        lib.fd_oracle_residual.argtypes = [ctypes.c_int64, ctypes.c_int32, vp, vp, f64p, vp,
+                                           ctypes.c_int64]
+        lib.fd_oracle_residual.restype = ctypes.c_int
+        lib.fd_oracle_jacobi.argtypes = [i32p, f64p, ctypes.c_int32, i32p, f64p, f64p, f64p,
+                                         ctypes.c_int64, ctypes.c_double, ctypes.c_double]
+        lib.fd_oracle_jacobi.restype = ctypes.c_int
+        lib.fd_oracle_transfer_weights.argtypes = [ctypes.c_int32, f64p]
+        lib.fd_oracle_transfer_weights.restype = ctypes.c_int
+        lib.fd_oracle_restrict.argtypes = [i32p, i32p, ctypes.c_int32, f64p, f64p, ctypes.c_int64]
+        lib.fd_oracle_restrict.restype = ctypes.c_int
+        lib.fd_oracle_interpolate.argtypes = [i32p, i32p, ctypes.c_int32, f64p, f64p,
+                                              ctypes.c_int64]
+        lib.fd_oracle_interpolate.restype = ctypes.c_int
+        lib.fd_oracle_paw_apply.argtypes = [i32p, f64p, i32p, f64p, ctypes.c_int32, ctypes.c_int32,
+                                            i32p, i32p, i32p, f64p, f64p, vp, vp, vp,
+                                            ctypes.c_int64, ctypes.c_int32]
+        lib.fd_oracle_paw_apply.restype = ctypes.c_int
         lib.fd_oracle_max_threads.argtypes = []
         lib.fd_oracle_max_threads.restype = ctypes.c_int
         _lib = lib
@@ -149,3 +170,114 @@ def dense(shape, h, nn, bc, k=None, v_eff: Optional[np.ndarray] = None) -> np.nd
     if rc != 0:
         raise ValueError("fd_oracle_dense: invalid argument")
     return M
+
+
+# ------------------------------------------------------------------------------ SURVEY 8(f) rows
+
+def expect(shape, h, nn, bc, k, psi: np.ndarray, v_eff: Optional[np.ndarray] = None,
+           scale: float = -0.5, want_out: bool = False):
+    """(eps[nbands] complex, norm[nbands]) = (sum conj(psi) H psi, sum |psi|^2) per band (plain grid
+    sums, fd_oracle.c: fd_oracle_expect); with want_out also H psi."""
+    shape, psi, v_eff = _check_inputs(shape, psi, v_eff)
+    nb = psi.shape[0]
+    eps = np.empty(nb, dtype=np.complex128)
+    norm = np.empty(nb, dtype=np.float64)
+    out = np.empty_like(psi) if want_out else None
+    kk = _f64(k) if k is not None else None
+    rc = _load().fd_oracle_expect(_i32(shape), _f64(h), int(nn), _i32(bc), kk,
+                                  int(psi.dtype == np.complex128), _ptr(psi), _f64ptr(v_eff),
+                                  _ptr(out) if out is not None else None, nb, float(scale),
+                                  _ptr(eps), _f64ptr(norm))
+    if rc != 0:
+        raise ValueError("fd_oracle_expect: invalid argument")
+    return (eps, norm, out) if want_out else (eps, norm)
+
+
+def residual(psi: np.ndarray, hpsi: np.ndarray, lam: np.ndarray) -> np.ndarray:
+    """r_b = hpsi_b - lam[b] psi_b."""
+    psi, hpsi = np.ascontiguousarray(psi), np.ascontiguousarray(hpsi)
+    lam = np.ascontiguousarray(lam, dtype=np.float64)
+    assert psi.shape == hpsi.shape and psi.dtype == hpsi.dtype and lam.shape == (psi.shape[0],)
+    out = np.empty_like(psi)
+    rc = _load().fd_oracle_residual(int(psi[0].size), int(psi.dtype == np.complex128), _ptr(psi),
+                                    _ptr(hpsi), _f64ptr(lam), _ptr(out), psi.shape[0])
+    if rc != 0:
+        raise ValueError("fd_oracle_residual: invalid argument")
+    return out
+
+
+def jacobi(shape, h, nn, bc, phi: np.ndarray, rhs: np.ndarray, omega: float,
+           scale: float = 1.0) -> np.ndarray:
+    """One weighted-Jacobi sweep for (scale lap_FD) phi = rhs (fd_oracle.c: fd_oracle_jacobi)."""
+    shape, phi, _ = _check_inputs(shape, phi, None)
+    rhs = np.ascontiguousarray(rhs, dtype=np.float64)
+    assert phi.dtype == np.float64 and rhs.shape == phi.shape
+    out = np.empty_like(phi)
+    rc = _load().fd_oracle_jacobi(_i32(shape), _f64(h), int(nn), _i32(bc), _f64ptr(phi),
+                                  _f64ptr(rhs), _f64ptr(out), phi.shape[0], float(omega),
+                                  float(scale))
+    if rc != 0:
+        raise ValueError("fd_oracle_jacobi: invalid argument")
+    return out
+
+
+def transfer_weights(p: int) -> np.ndarray:
+    """b[1..p] (b[0] = 0): midpoint Lagrange weights of the order-p grid transfer."""
+    b = (ctypes.c_double * (p + 1))()
+    if _load().fd_oracle_transfer_weights(int(p), b) != 0:
+        raise ValueError(f"bad transfer order p={p}")
+    return np.array(list(b), dtype=np.float64)
+
+
+def coarse_shape(shape_fine, bc):
+    """Coarse extents of a fine grid: n/2 on periodic axes (n even), (n-1)/2 on zero-BC axes."""
+    return tuple(int(n) // 2 if b else (int(n) - 1) // 2 for n, b in zip(shape_fine, bc))
+
+
+def restrict(shape_fine, bc, p: int, fine: np.ndarray) -> np.ndarray:
+    fine = np.ascontiguousarray(fine, dtype=np.float64)
+    assert fine.ndim == 4 and tuple(fine.shape[1:]) == tuple(shape_fine)
+    coarse = np.empty((fine.shape[0],) + coarse_shape(shape_fine, bc), dtype=np.float64)
+    rc = _load().fd_oracle_restrict(_i32(shape_fine), _i32(bc), int(p), _f64ptr(fine),
+                                    _f64ptr(coarse), fine.shape[0])
+    if rc != 0:
+        raise ValueError("fd_oracle_restrict: invalid argument")
+    return coarse
+
+
+def interpolate(shape_fine, bc, p: int, coarse: np.ndarray) -> np.ndarray:
+    coarse = np.ascontiguousarray(coarse, dtype=np.float64)
+    assert coarse.ndim == 4 and tuple(coarse.shape[1:]) == coarse_shape(shape_fine, bc)
+    fine = np.empty((coarse.shape[0],) + tuple(int(n) for n in shape_fine), dtype=np.float64)
+    rc = _load().fd_oracle_interpolate(_i32(shape_fine), _i32(bc), int(p), _f64ptr(coarse),
+                                       _f64ptr(fine), coarse.shape[0])
+    if rc != 0:
+        raise ValueError("fd_oracle_interpolate: invalid argument")
+    return fine
+
+
+def paw_apply(shape, h, bc, k, psi: np.ndarray, box_start, box_size, nproj, proj, dmat,
+              out: Optional[np.ndarray] = None, want_coef: bool = False):
+    """Non-local PAW term (fd_oracle.c: fd_oracle_paw_apply).  out None -> returns the term alone;
+    out given -> returns out + term (a copy).  With want_coef also the projections
+    P[nbands, sum n_i]."""
+    shape, psi, _ = _check_inputs(shape, psi, None)
+    is_c = psi.dtype == np.complex128
+    bs = np.ascontiguousarray(box_start, dtype=np.int32).reshape(-1, 3)
+    bz = np.ascontiguousarray(box_size, dtype=np.int32).reshape(-1, 3)
+    npj = np.ascontiguousarray(nproj, dtype=np.int32)
+    proj = np.ascontiguousarray(proj, dtype=np.float64)
+    dmat = np.ascontiguousarray(dmat, dtype=np.float64)
+    acc = out is not None
+    res = np.array(out, dtype=psi.dtype, copy=True, order="C") if acc else np.empty_like(psi)
+    coef = np.empty((psi.shape[0], int(npj.sum())), dtype=psi.dtype) if want_coef else None
+    i32p = ctypes.POINTER(ctypes.c_int32)
+    kk = _f64(k) if k is not None else None
+    rc = _load().fd_oracle_paw_apply(_i32(shape), _f64(h), _i32(bc), kk, int(is_c), len(npj),
+                                     bs.ctypes.data_as(i32p), bz.ctypes.data_as(i32p),
+                                     npj.ctypes.data_as(i32p), _f64ptr(proj), _f64ptr(dmat),
+                                     _ptr(psi), _ptr(res), _ptr(coef) if want_coef else None,
+                                     psi.shape[0], int(acc))
+    if rc != 0:
+        raise ValueError("fd_oracle_paw_apply: invalid argument")
+    return (res, coef) if want_coef else res
