@@ -29,7 +29,11 @@
  *   - psi and v_eff are read-only; out is fully overwritten (no accumulate) and must not overlap
  *     psi or v_eff;  the caller owns all three; the library owns only the plan;
  *   - applies are enqueued on `cuda_stream` (a cudaStream_t cast to void*, NULL = legacy default
- *     stream) and return immediately; a plan is immutable and may be used from several streams;
+ *     stream) and return immediately; a plan is immutable (the diagnostic fd_plan_set_kernel
+ *     excepted: call it before the plan is shared) and may be used from several streams;
+ *   - the plan's device must be the calling thread's current CUDA device in every call that
+ *     launches or copies (FD_ERR_INVALID otherwise); fd_create itself restores the caller's
+ *     current device before it returns;
  *   - there is no CPU fallback: without a usable CUDA device fd_create fails with FD_ERR_CUDA.
  */
 #ifndef FDHAM_H
@@ -79,7 +83,8 @@ enum {
  *   k_reduced  host: Bloch vector in reduced coordinates, NULL = Gamma; must be 0 on zero-BC axes
  *   dtype      FD_F64 (requires k = 0) or FD_C128
  *   device     CUDA device ordinal
- * Errors: FD_ERR_INVALID for any violated constraint above, FD_ERR_CUDA if the device cannot be
+ * Errors: FD_ERR_INVALID for any violated constraint above, FD_ERR_UNSUPPORTED for nx > 65535 or
+ * ny > 262140 (no kernel of this build launches such a grid), FD_ERR_CUDA if the device cannot be
  * used, FD_ERR_NOMEM.
  */
 FD_API int fd_create(fd_plan **plan, const int32_t shape[3], const double h[3], int32_t nn,
@@ -120,11 +125,59 @@ FD_API int fd_apply_hamiltonian(const fd_plan *plan, const void *psi, const doub
  * fd_apply_hamiltonian_host -- the same apply for HOST buffers (end-to-end path): copies psi and
  * v_eff to the device, applies, copies H psi back, in band chunks that overlap H2D, kernel and
  * D2H on internal streams.  v_eff may be NULL (kinetic only).  Blocks until `out` is complete.
- * Buffers may be pageable or pinned (pinned = faster).  Allocates and frees its own staging
- * device memory per call (FD_ERR_NOMEM if that fails).
+ * Buffers may be pageable or pinned (pinned = faster).  Creates and destroys a workspace per call
+ * (FD_ERR_NOMEM if that fails); a caller that applies repeatedly keeps one with the _ws form:
+ *
+ * fd_workspace_create -- device staging buffers (3 ring slots of `chunk_bytes` in + out, 0 = 64 MiB,
+ *   at least one band; plus one v_eff array) and the internal streams, for plans of this plan's
+ *   grid and dtype on its device.  Owned by the caller until fd_workspace_destroy (NULL = no-op).
+ * fd_apply_hamiltonian_host_ws -- fd_apply_hamiltonian_host on a workspace: no allocation, no
+ *   stream creation in the call.  One call at a time per workspace.  FD_ERR_INVALID if the
+ *   workspace does not match the plan; FD_ERR_ALIAS if out_host overlaps psi_host or v_eff_host.
  */
+typedef struct fd_workspace fd_workspace;
 FD_API int fd_apply_hamiltonian_host(const fd_plan *plan, const void *psi_host, const double *v_eff_host,
                               void *out_host, int64_t nbands);
+FD_API int fd_workspace_create(fd_workspace **ws, const fd_plan *plan, int64_t chunk_bytes);
+FD_API int fd_workspace_destroy(fd_workspace *ws);
+FD_API int fd_apply_hamiltonian_host_ws(const fd_plan *plan, fd_workspace *ws, const void *psi_host,
+                                 const double *v_eff_host, void *out_host, int64_t nbands);
+
+/*
+ * the eigensolver epilogue.  Every SCF step (subspace diagonalisation, then the
+ * Davidson / RMM-DIIS step) and every RT-TDDFT step (Eq. 91)
+ * needs, right after H psi, the band energies and the residuals.
+ *
+ * fd_apply_hamiltonian_expect -- out = H psi (v_eff == NULL: T psi) AND, from the same pass,
+ *     eps[b]  = Re sum_i conj(psi_b[i]) (H psi)_b[i]     (H is Hermitian: the imaginary part is zero)
+ *     norm[b] = sum_i |psi_b[i]|^2                         (plain grid sums; x h_x h_y h_z = integrals)
+ *   eps, norm   device pointers, double [nbands]
+ *   workspace   device pointer, 8-byte aligned, >= fd_expect_workspace_bytes(plan, nbands) bytes,
+ *               owned by the caller, scratch (per-warp partial sums; reduced in a fixed order by a
+ *               second small launch: results are bit-reproducible run to run, no atomics)
+ *   Other arguments and errors as fd_apply_hamiltonian; FD_ERR_INVALID also for a short workspace,
+ *   FD_ERR_ALIAS if out overlaps eps / norm / workspace.
+ * fd_expect_workspace_bytes -- bytes needed for a batch of nbands (>= 0), or a negative fd_status.
+ * fd_residual -- r_b = hpsi_b - (eps[b] / norm[b]) psi_b  (the residual R_b = H psi_b - eps_b psi_b
+ *   for normalised psi).  r may be exactly hpsi (in place) but must not overlap psi.
+ */
+FD_API int64_t fd_expect_workspace_bytes(const fd_plan *plan, int64_t nbands);
+FD_API int fd_apply_hamiltonian_expect(const fd_plan *plan, const void *psi, const double *v_eff, void *out,
+                                double *eps, double *norm, int64_t nbands, void *workspace,
+                                int64_t workspace_bytes, void *cuda_stream);
+FD_API int fd_residual(const fd_plan *plan, const void *psi, const void *hpsi, const double *eps,
+                const double *norm, void *r, int64_t nbands, void *cuda_stream);
+
+/*
+ * fd_jacobi_sweep: one weighted-Jacobi relaxation sweep for A phi = rhs with
+ * A = scale lap_FD, the operator of a plan made by fd_create_scaled (scale = 1: the Poisson
+ * operator; "multigrid ... Jacobi or Gauss-Seidel" Poisson solvers):
+ *     out[i] = phi[i] + omega (rhs[i] - (A phi)[i]) / A_ii,   A_ii = scale c_0 sum_d 1/h_d^2
+ * every point from the OLD phi.  phi, rhs, out: device pointers, double [nbands,nx,ny,nz], 16-byte
+ * aligned; out must not overlap phi or rhs.  FD_F64 plans only (FD_ERR_UNSUPPORTED otherwise).
+ */
+FD_API int fd_jacobi_sweep(const fd_plan *plan, const double *phi, const double *rhs, double *out,
+                    int64_t nbands, double omega, void *cuda_stream);
 
 /* fd_destroy -- free the plan; NULL is a no-op.  The caller must have synchronised any stream
  * still running an apply of this plan. */

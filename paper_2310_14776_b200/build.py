@@ -12,10 +12,14 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 ROOT = os.path.dirname(_HERE)
 LIB = os.path.join(_HERE, "libfdham.so")
-SOURCES = ["fd_api.cu", "fd_generic.cu", "fd_sweep.cu", "fd_sweep_inst_real.cu",
-           "fd_sweep_inst_cplx_ph0.cu", "fd_sweep_inst_cplx_ph1.cu", "fd_sweep_inst_cplx_ph3.cu"]
+# the slow units (sweep-kernel instantiations) first, so that the parallel build ends sooner
+SOURCES = ["fd_sweep_inst_real.cu", "fd_sweep_inst_real_ex.cu",
+           "fd_sweep_inst_cplx_ph0.cu", "fd_sweep_inst_cplx_ph1.cu", "fd_sweep_inst_cplx_ph3.cu",
+           "fd_sweep_inst_cplx_ph0_ex.cu", "fd_sweep_inst_cplx_ph1_ex.cu",
+           "fd_sweep_inst_cplx_ph3_ex.cu", "fd_sweep_inst_real_jacobi.cu",
+           "fd_api.cu", "fd_generic.cu", "fd_sweep.cu", "fd_aux.cu"]
 HEADERS = [os.path.join(CSRC, "fd_internal.h"), os.path.join(CSRC, "fd_sweep_kernel.cuh"),
-           os.path.join(ROOT, "include", "fdham.h")]
+           os.path.join(CSRC, "fd_sweep_inst.h"), os.path.join(ROOT, "include", "fdham.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden"]
 OBJDIR = os.path.join(_HERE, "build")

@@ -73,18 +73,44 @@ int kernel_for_batch(const fd_plan *plan, int64_t nbands)
     return t_generic_us < t_sweep_us ? FD_KERNEL_GENERIC : FD_KERNEL_SWEEP;
 }
 
-int apply_device(const fd_plan *plan, const void *psi, const double *v_eff, void *out,
-                 int64_t nbands, cudaStream_t stream)
+// The device the plan was built for must be current in the calling thread (the launches below go
+// to the current device): FD_ERR_INVALID otherwise, instead of a launch in the wrong context.
+int check_device(const fd_plan *plan)
 {
+    int cur = -1;
+    if (cudaGetDevice(&cur) != cudaSuccess) {
+        cudaGetLastError();
+        return FD_ERR_CUDA;
+    }
+    return cur == plan->device ? FD_OK : FD_ERR_INVALID;
+}
+
+// mode 0: T psi, 1: + v_eff psi, 2: Jacobi form (g = pre-scaled copy of the plan's geometry, second =
+// rhs).  eps != nullptr: also the expectation values (fused in the sweep kernel, or a second pass
+// over the stored H psi when the batch runs on the generic kernel); ws as fd_expect_workspace_bytes.
+int apply_device(const fd_plan *plan, const FdGeom &g, int mode, const void *psi, const double *second,
+                 void *out, int64_t nbands, double *eps, double *norm, double *ws,
+                 cudaStream_t stream)
+{
+    const int drc = check_device(plan);
+    if (drc != FD_OK) return drc;
     cudaError_t e;
     int n = 0;
     if (kernel_for_batch(plan, nbands) == FD_KERNEL_SWEEP) {
-        e = fd_launch_sweep(plan, psi, v_eff, out, nbands, stream, &n);
+        const bool fused = eps && fd_sweep_expect_fused(plan);
+        e = fd_launch_sweep(plan, g, mode, psi, second, out, nbands, fused ? eps : nullptr, norm, ws,
+                            stream, &n);
+        if (e == cudaSuccess && eps && !fused)
+            e = fd_launch_dot(plan, psi, out, eps, norm, ws, nbands, stream, &n);
     } else {
-        e = fd_launch_generic(plan, psi, v_eff, out, nbands, stream);
+        e = fd_launch_generic(plan, g, mode, psi, second, out, nbands, stream);
         n = 1;
+        if (e == cudaSuccess && eps) e = fd_launch_dot(plan, psi, out, eps, norm, ws, nbands, stream, &n);
     }
-    if (e != cudaSuccess) return FD_ERR_CUDA;
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return FD_ERR_CUDA;
+    }
     __atomic_add_fetch(&const_cast<fd_plan *>(plan)->launches, (long long)n, __ATOMIC_RELAXED);
     return FD_OK;
 }
@@ -136,12 +162,25 @@ int fd_create_scaled(fd_plan **plan_out, const int32_t shape[3], const double h[
     }
     if ((long long)shape[0] * shape[1] * shape[2] > (1LL << 40)) return FD_ERR_INVALID;
 
+    // shapes the one-thread-per-point kernel cannot launch (its grid is (nz/64, ny/4, nx * groups))
+    if (shape[0] > 65535 || (shape[1] + 3) / 4 > 65535) return FD_ERR_UNSUPPORTED;
+
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) {
         cudaGetLastError();
         return FD_ERR_CUDA;
     }
-    if (cudaSetDevice(device) != cudaSuccess) return FD_ERR_CUDA;
+    // the plan is built with `device` current; the caller's current device is restored on return
+    int prev_device = -1;
+    if (cudaGetDevice(&prev_device) != cudaSuccess) {
+        cudaGetLastError();
+        return FD_ERR_CUDA;
+    }
+    struct DeviceGuard {
+        int prev, now;
+        ~DeviceGuard() { if (prev >= 0 && prev != now) cudaSetDevice(prev); }
+    } guard{prev_device, device};
+    if (prev_device != device && cudaSetDevice(device) != cudaSuccess) return FD_ERR_CUDA;
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return FD_ERR_CUDA;
 
@@ -191,7 +230,8 @@ int fd_apply_kinetic(const fd_plan *plan, const void *psi, void *out, int64_t nb
 {
     const int rc = check_apply_args(plan, psi, nullptr, false, out, nbands);
     if (rc != FD_OK || nbands == 0) return rc;
-    return apply_device(plan, psi, nullptr, out, nbands, (cudaStream_t)cuda_stream);
+    return apply_device(plan, plan->g, 0, psi, nullptr, out, nbands, nullptr, nullptr, nullptr,
+                        (cudaStream_t)cuda_stream);
 }
 
 int fd_apply_hamiltonian(const fd_plan *plan, const void *psi, const double *v_eff, void *out,
@@ -199,7 +239,135 @@ int fd_apply_hamiltonian(const fd_plan *plan, const void *psi, const double *v_e
 {
     const int rc = check_apply_args(plan, psi, v_eff, true, out, nbands);
     if (rc != FD_OK || nbands == 0) return rc;
-    return apply_device(plan, psi, v_eff, out, nbands, (cudaStream_t)cuda_stream);
+    return apply_device(plan, plan->g, 1, psi, v_eff, out, nbands, nullptr, nullptr, nullptr,
+                        (cudaStream_t)cuda_stream);
+}
+
+// Device staging buffers and streams of the host-buffer applies: created once, reused by every
+// fd_apply_hamiltonian_host_ws call (one call at a time per workspace).
+struct fd_workspace {
+    static const int kSlots = 3;
+    int device;
+    size_t npoints;       // grid points of the plan it was created for
+    size_t band_bytes;
+    int64_t chunk;        // bands per ring slot
+    double *v_dev;
+    char *in_dev[kSlots], *out_dev[kSlots];
+    cudaStream_t st[kSlots];
+    cudaEvent_t v_ready;
+};
+
+int fd_workspace_destroy(fd_workspace *ws)
+{
+    if (!ws) return FD_OK;
+    int prev = -1;
+    cudaGetDevice(&prev);
+    if (prev != ws->device) cudaSetDevice(ws->device);
+    if (ws->v_ready) cudaEventDestroy(ws->v_ready);
+    for (int i = 0; i < fd_workspace::kSlots; ++i) {
+        if (ws->st[i]) cudaStreamDestroy(ws->st[i]);
+        if (ws->in_dev[i]) cudaFree(ws->in_dev[i]);
+        if (ws->out_dev[i]) cudaFree(ws->out_dev[i]);
+    }
+    if (ws->v_dev) cudaFree(ws->v_dev);
+    if (prev >= 0 && prev != ws->device) cudaSetDevice(prev);
+    cudaGetLastError();
+    delete ws;
+    return FD_OK;
+}
+
+int fd_workspace_create(fd_workspace **ws_out, const fd_plan *plan, int64_t chunk_bytes)
+{
+    if (!ws_out || !plan || chunk_bytes < 0) return FD_ERR_INVALID;
+    const int drc = check_device(plan);
+    if (drc != FD_OK) return drc;
+    fd_workspace *w = new (std::nothrow) fd_workspace();
+    if (!w) return FD_ERR_NOMEM;
+    memset(w, 0, sizeof(*w));
+    w->device = plan->device;
+    w->npoints = (size_t)plan->g.n[0] * plan->g.n[1] * plan->g.n[2];
+    w->band_bytes = w->npoints * (plan->g.cplx ? 16 : 8);
+    if (chunk_bytes == 0) chunk_bytes = 64 << 20;
+    w->chunk = (int64_t)((size_t)chunk_bytes / w->band_bytes);
+    if (w->chunk < 1) w->chunk = 1;
+    int rc = FD_OK;
+    if (cudaMalloc(&w->v_dev, w->npoints * 8) != cudaSuccess) rc = FD_ERR_NOMEM;
+    for (int i = 0; i < fd_workspace::kSlots && rc == FD_OK; ++i) {
+        if (cudaMalloc(&w->in_dev[i], w->band_bytes * w->chunk) != cudaSuccess ||
+            cudaMalloc(&w->out_dev[i], w->band_bytes * w->chunk) != cudaSuccess)
+            rc = FD_ERR_NOMEM;
+        else if (cudaStreamCreateWithFlags(&w->st[i], cudaStreamNonBlocking) != cudaSuccess)
+            rc = FD_ERR_CUDA;
+    }
+    if (rc == FD_OK && cudaEventCreateWithFlags(&w->v_ready, cudaEventDisableTiming) != cudaSuccess)
+        rc = FD_ERR_CUDA;
+    if (rc != FD_OK) {
+        cudaGetLastError();
+        fd_workspace_destroy(w);
+        return rc;
+    }
+    *ws_out = w;
+    return FD_OK;
+}
+
+int fd_apply_hamiltonian_host_ws(const fd_plan *plan, fd_workspace *ws, const void *psi_host,
+                                 const double *v_eff_host, void *out_host, int64_t nbands)
+{
+    if (!plan || !ws || nbands < 0) return FD_ERR_INVALID;
+    if (nbands == 0) return FD_OK;
+    if (!psi_host || !out_host) return FD_ERR_INVALID;
+    const size_t P = (size_t)plan->g.n[0] * plan->g.n[1] * plan->g.n[2];
+    const size_t band_bytes = P * (plan->g.cplx ? 16 : 8);
+    if (ws->device != plan->device || ws->npoints != P || ws->band_bytes != band_bytes)
+        return FD_ERR_INVALID;
+    if (overlaps(out_host, band_bytes * nbands, psi_host, band_bytes * nbands)) return FD_ERR_ALIAS;
+    if (v_eff_host && overlaps(out_host, band_bytes * nbands, v_eff_host, P * 8)) return FD_ERR_ALIAS;
+    const int drc = check_device(plan);
+    if (drc != FD_OK) return drc;
+
+    // Band chunks ride a 3-slot ring; each slot has its own stream running H2D -> kernel -> D2H, so
+    // the copy engines (both directions) and the SMs overlap.
+    const int kSlots = fd_workspace::kSlots;
+    const int64_t chunk = ws->chunk;
+    int rc = FD_OK;
+    auto fail = [&](int code) { if (rc == FD_OK) rc = code; };
+    double *v_dev = v_eff_host ? ws->v_dev : nullptr;
+    if (v_dev) {
+        if (cudaMemcpyAsync(v_dev, v_eff_host, P * 8, cudaMemcpyHostToDevice, ws->st[0]) != cudaSuccess ||
+            cudaEventRecord(ws->v_ready, ws->st[0]) != cudaSuccess)
+            fail(FD_ERR_CUDA);
+    }
+    int64_t b0 = 0;
+    for (int i = 0; rc == FD_OK && b0 < nbands; ++i, b0 += chunk) {
+        const int s = i % kSlots;
+        const int64_t nb = (nbands - b0 < chunk) ? nbands - b0 : chunk;
+        const char *src = static_cast<const char *>(psi_host) + (size_t)b0 * band_bytes;
+        char *dst = static_cast<char *>(out_host) + (size_t)b0 * band_bytes;
+        if (cudaMemcpyAsync(ws->in_dev[s], src, band_bytes * nb, cudaMemcpyHostToDevice, ws->st[s]) !=
+            cudaSuccess) {
+            fail(FD_ERR_CUDA);
+            break;
+        }
+        if (v_dev && s != 0 && i < kSlots && cudaStreamWaitEvent(ws->st[s], ws->v_ready, 0) != cudaSuccess) {
+            fail(FD_ERR_CUDA);
+            break;
+        }
+        const int arc = apply_device(plan, plan->g, v_dev ? 1 : 0, ws->in_dev[s], v_dev, ws->out_dev[s],
+                                     nb, nullptr, nullptr, nullptr, ws->st[s]);
+        if (arc != FD_OK) {
+            fail(arc);
+            break;
+        }
+        if (cudaMemcpyAsync(dst, ws->out_dev[s], band_bytes * nb, cudaMemcpyDeviceToHost, ws->st[s]) !=
+            cudaSuccess) {
+            fail(FD_ERR_CUDA);
+            break;
+        }
+    }
+    for (int i = 0; i < kSlots; ++i)
+        if (cudaStreamSynchronize(ws->st[i]) != cudaSuccess) fail(FD_ERR_CUDA);
+    if (rc == FD_ERR_CUDA) cudaGetLastError();
+    return rc;
 }
 
 int fd_apply_hamiltonian_host(const fd_plan *plan, const void *psi_host, const double *v_eff_host,
@@ -207,80 +375,90 @@ int fd_apply_hamiltonian_host(const fd_plan *plan, const void *psi_host, const d
 {
     if (!plan || nbands < 0) return FD_ERR_INVALID;
     if (nbands == 0) return FD_OK;
-    if (!psi_host || !out_host) return FD_ERR_INVALID;
-    const size_t P = (size_t)plan->g.n[0] * plan->g.n[1] * plan->g.n[2];
-    const size_t band_bytes = P * (plan->g.cplx ? 16 : 8);
-    if (overlaps(out_host, band_bytes * nbands, psi_host, band_bytes * nbands)) return FD_ERR_ALIAS;
-    if (cudaSetDevice(plan->device) != cudaSuccess) return FD_ERR_CUDA;
-
-    // Band chunks of ~64 MiB ride a 3-slot ring; each slot has its own stream running
-    // H2D -> kernel -> D2H, so the copy engines (both directions) and the SMs overlap.
-    constexpr int kSlots = 3;
-    int64_t chunk = (int64_t)((64u << 20) / band_bytes);
-    if (chunk < 1) chunk = 1;
-    if (chunk > nbands) chunk = nbands;
-    const int nslots = (int)((nbands + chunk - 1) / chunk < kSlots ? (nbands + chunk - 1) / chunk
-                                                                   : kSlots);
-    int rc = FD_OK;
-    double *v_dev = nullptr;
-    char *in_dev[kSlots] = {nullptr, nullptr, nullptr};
-    char *out_dev[kSlots] = {nullptr, nullptr, nullptr};
-    cudaStream_t st[kSlots] = {nullptr, nullptr, nullptr};
-    cudaEvent_t v_ready = nullptr;
-    auto fail = [&](int code) { if (rc == FD_OK) rc = code; };
-
-    if (v_eff_host && cudaMalloc(&v_dev, P * 8) != cudaSuccess) fail(FD_ERR_NOMEM);
-    for (int i = 0; i < nslots && rc == FD_OK; ++i) {
-        if (cudaMalloc(&in_dev[i], band_bytes * chunk) != cudaSuccess ||
-            cudaMalloc(&out_dev[i], band_bytes * chunk) != cudaSuccess)
-            fail(FD_ERR_NOMEM);
-        else if (cudaStreamCreateWithFlags(&st[i], cudaStreamNonBlocking) != cudaSuccess)
-            fail(FD_ERR_CUDA);
-    }
-    if (rc == FD_OK && cudaEventCreateWithFlags(&v_ready, cudaEventDisableTiming) != cudaSuccess)
-        fail(FD_ERR_CUDA);
-    if (rc == FD_OK && v_dev) {
-        if (cudaMemcpyAsync(v_dev, v_eff_host, P * 8, cudaMemcpyHostToDevice, st[0]) != cudaSuccess ||
-            cudaEventRecord(v_ready, st[0]) != cudaSuccess)
-            fail(FD_ERR_CUDA);
-    }
-    int64_t b0 = 0;
-    for (int i = 0; rc == FD_OK && b0 < nbands; ++i, b0 += chunk) {
-        const int s = i % nslots;
-        const int64_t nb = (nbands - b0 < chunk) ? nbands - b0 : chunk;
-        const char *src = static_cast<const char *>(psi_host) + (size_t)b0 * band_bytes;
-        char *dst = static_cast<char *>(out_host) + (size_t)b0 * band_bytes;
-        if (cudaMemcpyAsync(in_dev[s], src, band_bytes * nb, cudaMemcpyHostToDevice, st[s]) !=
-            cudaSuccess) {
-            fail(FD_ERR_CUDA);
-            break;
-        }
-        if (v_dev && s != 0 && i < nslots && cudaStreamWaitEvent(st[s], v_ready, 0) != cudaSuccess) {
-            fail(FD_ERR_CUDA);
-            break;
-        }
-        const int arc = apply_device(plan, in_dev[s], v_dev, out_dev[s], nb, st[s]);
-        if (arc != FD_OK) {
-            fail(arc);
-            break;
-        }
-        if (cudaMemcpyAsync(dst, out_dev[s], band_bytes * nb, cudaMemcpyDeviceToHost, st[s]) !=
-            cudaSuccess) {
-            fail(FD_ERR_CUDA);
-            break;
-        }
-    }
-    for (int i = 0; i < nslots; ++i)
-        if (st[i] && cudaStreamSynchronize(st[i]) != cudaSuccess) fail(FD_ERR_CUDA);
-    if (v_ready) cudaEventDestroy(v_ready);
-    for (int i = 0; i < kSlots; ++i) {
-        if (st[i]) cudaStreamDestroy(st[i]);
-        if (in_dev[i]) cudaFree(in_dev[i]);
-        if (out_dev[i]) cudaFree(out_dev[i]);
-    }
-    if (v_dev) cudaFree(v_dev);
-    if (rc == FD_ERR_CUDA) cudaGetLastError();
+    fd_workspace *ws = nullptr;
+    int rc = fd_workspace_create(&ws, plan, 0);
+    if (rc != FD_OK) return rc;
+    rc = fd_apply_hamiltonian_host_ws(plan, ws, psi_host, v_eff_host, out_host, nbands);
+    fd_workspace_destroy(ws);
     return rc;
+}
+
+// ---- expectation values and residual ---------------------------------------------
+
+int64_t fd_expect_workspace_bytes(const fd_plan *plan, int64_t nbands)
+{
+    if (!plan || nbands < 0) return FD_ERR_INVALID;
+    if (nbands == 0) return 0;
+    const int64_t n = (kernel_for_batch(plan, nbands) == FD_KERNEL_SWEEP && fd_sweep_expect_fused(plan))
+                          ? fd_sweep_expect_ws_bytes(plan, nbands)
+                          : fd_dot_ws_bytes(plan, nbands);
+    return n < 16 ? 16 : n;
+}
+
+int fd_apply_hamiltonian_expect(const fd_plan *plan, const void *psi, const double *v_eff, void *out,
+                                double *eps, double *norm, int64_t nbands, void *workspace,
+                                int64_t workspace_bytes, void *cuda_stream)
+{
+    const int rc = check_apply_args(plan, psi, v_eff, false, out, nbands);
+    if (rc != FD_OK || nbands == 0) return rc;
+    if (!eps || !norm || !workspace) return FD_ERR_INVALID;
+    if (((uintptr_t)eps | (uintptr_t)norm | (uintptr_t)workspace) & 7) return FD_ERR_INVALID;
+    if (workspace_bytes < fd_expect_workspace_bytes(plan, nbands)) return FD_ERR_INVALID;
+    const size_t nb = (size_t)plan->g.n[0] * plan->g.n[1] * plan->g.n[2] * (size_t)nbands *
+                      (plan->g.cplx ? 16 : 8);
+    if (overlaps(out, nb, eps, 8 * (size_t)nbands) || overlaps(out, nb, norm, 8 * (size_t)nbands) ||
+        overlaps(out, nb, workspace, (size_t)workspace_bytes) ||
+        overlaps(eps, 8 * (size_t)nbands, norm, 8 * (size_t)nbands))
+        return FD_ERR_ALIAS;
+    return apply_device(plan, plan->g, v_eff ? 1 : 0, psi, v_eff, out, nbands, eps, norm,
+                        static_cast<double *>(workspace), (cudaStream_t)cuda_stream);
+}
+
+int fd_residual(const fd_plan *plan, const void *psi, const void *hpsi, const double *eps,
+                const double *norm, void *r, int64_t nbands, void *cuda_stream)
+{
+    if (!plan || nbands < 0) return FD_ERR_INVALID;
+    if (nbands == 0) return FD_OK;
+    if (!psi || !hpsi || !eps || !norm || !r) return FD_ERR_INVALID;
+    if (((uintptr_t)psi | (uintptr_t)hpsi | (uintptr_t)r) & 15) return FD_ERR_INVALID;
+    const size_t nb = (size_t)plan->g.n[0] * plan->g.n[1] * plan->g.n[2] * (size_t)nbands *
+                      (plan->g.cplx ? 16 : 8);
+    if (overlaps(r, nb, psi, nb)) return FD_ERR_ALIAS;
+    if (r != hpsi && overlaps(r, nb, hpsi, nb)) return FD_ERR_ALIAS;  // exactly in place is allowed
+    const int drc = check_device(plan);
+    if (drc != FD_OK) return drc;
+    if (fd_launch_residual(plan, psi, hpsi, eps, norm, r, nbands, (cudaStream_t)cuda_stream) !=
+        cudaSuccess) {
+        cudaGetLastError();
+        return FD_ERR_CUDA;
+    }
+    __atomic_add_fetch(&const_cast<fd_plan *>(plan)->launches, 1LL, __ATOMIC_RELAXED);
+    return FD_OK;
+}
+
+// ---- weighted-Jacobi sweep ---------------------------------------------------------
+
+int fd_jacobi_sweep(const fd_plan *plan, const double *phi, const double *rhs, double *out,
+                    int64_t nbands, double omega, void *cuda_stream)
+{
+    if (!plan || nbands < 0 || !isfinite(omega)) return FD_ERR_INVALID;
+    if (plan->g.cplx) return FD_ERR_UNSUPPORTED;
+    if (nbands == 0) return FD_OK;
+    if (!phi || !rhs || !out) return FD_ERR_INVALID;
+    if (((uintptr_t)phi | (uintptr_t)rhs | (uintptr_t)out) & 15) return FD_ERR_INVALID;
+    const size_t nb = (size_t)plan->g.n[0] * plan->g.n[1] * plan->g.n[2] * (size_t)nbands * 8;
+    if (overlaps(out, nb, phi, nb) || overlaps(out, nb, rhs, nb)) return FD_ERR_ALIAS;
+    if (plan->g.wdiag == 0.0) return FD_ERR_INVALID;
+    // out = phi + omega (rhs - A phi) / A_ii = (1 - omega) phi - (omega / A_ii) A_offdiag phi
+    //       + (omega / A_ii) rhs : the stencil kernels with rescaled weights and an additive term
+    FdGeom gj = plan->g;
+    const double f = omega / plan->g.wdiag;
+    for (int d = 0; d < 3; ++d)
+        for (int j = 0; j <= gj.nn; ++j) gj.w[d][j] = -f * plan->g.w[d][j];
+    gj.wdiag = 1.0 - omega;
+    gj.rhs_coef = f;
+    return apply_device(plan, gj, 2, phi, rhs, out, nbands, nullptr, nullptr, nullptr,
+                        (cudaStream_t)cuda_stream);
 }
 
 int fd_destroy(fd_plan *plan)
@@ -312,14 +490,19 @@ int fd_plan_set_kernel(fd_plan *plan, int32_t kernel, int32_t param)
     }
     if (kernel != FD_KERNEL_AUTO && kernel != FD_KERNEL_SWEEP) return FD_ERR_INVALID;
     if (param != 0 || kernel == FD_KERNEL_SWEEP) {
-        fd_sweep_configure(plan, param, plan->sweep.xchunk, plan->sweep.stages_req);
-        if (plan->sweep.supported && fd_sweep_prepare(plan) != cudaSuccess) {
+        // configure a copy: a refused request leaves the plan exactly as it was
+        fd_plan trial = *plan;
+        fd_sweep_configure(&trial, param, plan->sweep.xchunk, plan->sweep.stages_req);
+        if (!trial.sweep.supported) return FD_ERR_UNSUPPORTED;
+        const int drc = check_device(plan);
+        if (drc != FD_OK) return drc;
+        if (fd_sweep_prepare(&trial) != cudaSuccess) {
             cudaGetLastError();
             return FD_ERR_CUDA;
         }
+        plan->sweep = trial.sweep;
     }
     if (!plan->sweep.supported && kernel == FD_KERNEL_SWEEP) return FD_ERR_UNSUPPORTED;
-    // a failed request above leaves the family and the per-batch choice as they were
     plan->kernel = plan->sweep.supported ? FD_KERNEL_SWEEP : FD_KERNEL_GENERIC;
     plan->forced = (kernel != FD_KERNEL_AUTO);
     return FD_OK;

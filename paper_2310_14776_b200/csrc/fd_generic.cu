@@ -65,12 +65,15 @@ __device__ __forceinline__ void store<true>(double *p, long long idx, const Val<
 // straight from the constant bank.  blockIdx.z = x plane * band groups + band group.
 constexpr int kBx = 64, kBy = 4;
 
-template <bool CPLX, bool HAS_V, int NN>
+// MODE 0: T psi; 1: + v_eff psi (v_eff[nx,ny,nz]); 2: the weighted-Jacobi form, v_eff = the right-hand
+// side [nbands,nx,ny,nz], added as g.rhs_coef * rhs (g carries the pre-scaled weights; real only).
+template <bool CPLX, int MODE, int NN>
 __global__ void __launch_bounds__(kBx * kBy)
 fd_generic_kernel(const __grid_constant__ FdGeom g, const double *__restrict__ psi,
                   const double *__restrict__ v_eff, double *__restrict__ out, long long nbands,
                   int bgroups)
 {
+    constexpr bool HAS_V = MODE == 1;
     const int iz = blockIdx.x * kBx + threadIdx.x;
     const int iy = blockIdx.y * kBy + threadIdx.y;
     const int ix = blockIdx.z / bgroups;
@@ -112,11 +115,12 @@ fd_generic_kernel(const __grid_constant__ FdGeom g, const double *__restrict__ p
                 }
             }
         }
+        if constexpr (MODE == 2 && !CPLX) acc.x = ::fma(g.rhs_coef, __ldg(v_eff + b * P + lin), acc.x);
         store<CPLX>(out, b * P + lin, acc);
     }
 }
 
-template <bool CPLX, bool HAS_V>
+template <bool CPLX, int MODE>
 cudaError_t launch_nn(const FdGeom &g, const double *p, const double *v_eff, double *o,
                       long long nbands, cudaStream_t stream)
 {
@@ -131,12 +135,12 @@ cudaError_t launch_nn(const FdGeom &g, const double *p, const double *v_eff, dou
     if (grid.y > 65535) return cudaErrorInvalidConfiguration;
     const int bgi = (int)bgroups;
     switch (g.nn) {
-    case 1: fd_generic_kernel<CPLX, HAS_V, 1><<<grid, block, 0, stream>>>(g, p, v_eff, o, nbands, bgi); break;
-    case 2: fd_generic_kernel<CPLX, HAS_V, 2><<<grid, block, 0, stream>>>(g, p, v_eff, o, nbands, bgi); break;
-    case 3: fd_generic_kernel<CPLX, HAS_V, 3><<<grid, block, 0, stream>>>(g, p, v_eff, o, nbands, bgi); break;
-    case 4: fd_generic_kernel<CPLX, HAS_V, 4><<<grid, block, 0, stream>>>(g, p, v_eff, o, nbands, bgi); break;
-    case 5: fd_generic_kernel<CPLX, HAS_V, 5><<<grid, block, 0, stream>>>(g, p, v_eff, o, nbands, bgi); break;
-    case 6: fd_generic_kernel<CPLX, HAS_V, 6><<<grid, block, 0, stream>>>(g, p, v_eff, o, nbands, bgi); break;
+    case 1: fd_generic_kernel<CPLX, MODE, 1><<<grid, block, 0, stream>>>(g, p, v_eff, o, nbands, bgi); break;
+    case 2: fd_generic_kernel<CPLX, MODE, 2><<<grid, block, 0, stream>>>(g, p, v_eff, o, nbands, bgi); break;
+    case 3: fd_generic_kernel<CPLX, MODE, 3><<<grid, block, 0, stream>>>(g, p, v_eff, o, nbands, bgi); break;
+    case 4: fd_generic_kernel<CPLX, MODE, 4><<<grid, block, 0, stream>>>(g, p, v_eff, o, nbands, bgi); break;
+    case 5: fd_generic_kernel<CPLX, MODE, 5><<<grid, block, 0, stream>>>(g, p, v_eff, o, nbands, bgi); break;
+    case 6: fd_generic_kernel<CPLX, MODE, 6><<<grid, block, 0, stream>>>(g, p, v_eff, o, nbands, bgi); break;
     default: return cudaErrorInvalidConfiguration;
     }
     return cudaPeekAtLastError();
@@ -144,16 +148,19 @@ cudaError_t launch_nn(const FdGeom &g, const double *p, const double *v_eff, dou
 
 }  // namespace
 
-cudaError_t fd_launch_generic(const fd_plan *plan, const void *psi, const double *v_eff, void *out,
-                              int64_t nbands, cudaStream_t stream)
+cudaError_t fd_launch_generic(const fd_plan *plan, const FdGeom &g, int mode, const void *psi,
+                              const double *second, void *out, int64_t nbands, cudaStream_t stream)
 {
-    const FdGeom &g = plan->g;
+    (void)plan;
     if (g.n[0] > 65535) return cudaErrorInvalidConfiguration;
     const double *p = static_cast<const double *>(psi);
     double *o = static_cast<double *>(out);
-    if (g.cplx)
-        return v_eff ? launch_nn<true, true>(g, p, v_eff, o, nbands, stream)
-                     : launch_nn<true, false>(g, p, nullptr, o, nbands, stream);
-    return v_eff ? launch_nn<false, true>(g, p, v_eff, o, nbands, stream)
-                 : launch_nn<false, false>(g, p, nullptr, o, nbands, stream);
+    if (g.cplx) {
+        if (mode == 2) return cudaErrorInvalidValue;
+        return mode ? launch_nn<true, 1>(g, p, second, o, nbands, stream)
+                    : launch_nn<true, 0>(g, p, nullptr, o, nbands, stream);
+    }
+    if (mode == 2) return launch_nn<false, 2>(g, p, second, o, nbands, stream);
+    return mode ? launch_nn<false, 1>(g, p, second, o, nbands, stream)
+                : launch_nn<false, 0>(g, p, nullptr, o, nbands, stream);
 }

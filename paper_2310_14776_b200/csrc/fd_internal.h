@@ -15,6 +15,7 @@ struct FdGeom {
     double w[3][FD_MAX_NN + 1];  // w[d][j] = -1/2 c_j / h_d^2
     double wdiag;                // sum_d w[d][0]
     double ph_re[3], ph_im[3];   // exp(+2 pi i k_d): factor when a tap runs past the UPPER end
+    double rhs_coef;             // Jacobi sweep only (sweep MODE 2 / generic): factor of the rhs
 };
 
 // Limits shared by the sweep kernel (fd_sweep_kernel.cuh) and its host side (fd_sweep.cu)
@@ -61,25 +62,55 @@ struct fd_plan {
 };
 
 // fd_generic.cu
-cudaError_t fd_launch_generic(const fd_plan *plan, const void *psi, const double *v_eff, void *out,
-                              int64_t nbands, cudaStream_t stream);
-// fd_sweep_inst_*.cu: instantiations of the sweep kernel template (fd_sweep_kernel.cuh)
+cudaError_t fd_launch_generic(const fd_plan *plan, const FdGeom &g, int mode, const void *psi,
+                              const double *second, void *out, int64_t nbands, cudaStream_t stream);
+// fd_aux.cu: streaming helper kernels (two-pass expectation values, residual)
+int64_t fd_dot_ws_bytes(const fd_plan *plan, int64_t nbands);
+cudaError_t fd_launch_dot(const fd_plan *plan, const void *psi, const void *hpsi, double *eps,
+                          double *norm, double *ws, int64_t nbands, cudaStream_t stream,
+                          int *nlaunches);
+cudaError_t fd_launch_residual(const fd_plan *plan, const void *psi, const void *hpsi,
+                               const double *eps, const double *norm, void *r, int64_t nbands,
+                               cudaStream_t stream);
+// Extra arguments of the sweep kernel's EX instantiations (fd_apply_hamiltonian_expect): where the
+// per-warp partial sums go.  Entry ((team * maxseg + segment) * nytiles + ytile) * nwarps + warp
+// holds the pair (sum conj(psi) H psi, sum |psi|^2) of that warp for that band segment.
+struct FdSweepAux {
+    double *ws;
+    int maxseg;  // band segments a team can touch: quota / nx + 2
+};
+
+// fd_sweep_inst_*.cu: instantiations of the sweep kernel template (fd_sweep_kernel.cuh).
+// mode: 0 kinetic, 1 + v_eff psi, 2 Jacobi sweep (real, not EX); ex: with the expectation values.
 typedef void (*FdSweepKernelFn)(const FdGeom, const FdSweepCfg, const double *, const double *,
-                                double *, const long long, const int);
-FdSweepKernelFn fd_sweep_pick_real(int rowd, int has_v, int nn);
-FdSweepKernelFn fd_sweep_pick_cplx_ph0(int rowd, int has_v, int nn);
-FdSweepKernelFn fd_sweep_pick_cplx_ph1(int rowd, int has_v, int nn);
-FdSweepKernelFn fd_sweep_pick_cplx_ph3(int rowd, int has_v, int nn);
-inline FdSweepKernelFn fd_sweep_pick_cplx(int rowd, int has_v, int ph, int nn)
+                                double *, const long long, const int, const FdSweepAux);
+FdSweepKernelFn fd_sweep_pick_real(int rowd, int mode, int nn);
+FdSweepKernelFn fd_sweep_pick_real_ex(int rowd, int mode, int nn);
+FdSweepKernelFn fd_sweep_pick_real_jacobi(int rowd, int nn);
+FdSweepKernelFn fd_sweep_pick_cplx_ph0(int rowd, int mode, int nn);
+FdSweepKernelFn fd_sweep_pick_cplx_ph1(int rowd, int mode, int nn);
+FdSweepKernelFn fd_sweep_pick_cplx_ph3(int rowd, int mode, int nn);
+FdSweepKernelFn fd_sweep_pick_cplx_ph0_ex(int rowd, int mode, int nn);
+FdSweepKernelFn fd_sweep_pick_cplx_ph1_ex(int rowd, int mode, int nn);
+FdSweepKernelFn fd_sweep_pick_cplx_ph3_ex(int rowd, int mode, int nn);
+inline FdSweepKernelFn fd_sweep_pick_cplx(int rowd, int mode, int ph, int nn, int ex)
 {
-    if (ph == 0) return fd_sweep_pick_cplx_ph0(rowd, has_v, nn);
-    if (ph == 1) return fd_sweep_pick_cplx_ph1(rowd, has_v, nn);
-    return fd_sweep_pick_cplx_ph3(rowd, has_v, nn);
+    if (ex) {
+        if (ph == 0) return fd_sweep_pick_cplx_ph0_ex(rowd, mode, nn);
+        if (ph == 1) return fd_sweep_pick_cplx_ph1_ex(rowd, mode, nn);
+        return fd_sweep_pick_cplx_ph3_ex(rowd, mode, nn);
+    }
+    if (ph == 0) return fd_sweep_pick_cplx_ph0(rowd, mode, nn);
+    if (ph == 1) return fd_sweep_pick_cplx_ph1(rowd, mode, nn);
+    return fd_sweep_pick_cplx_ph3(rowd, mode, nn);
 }
 // fd_api.cu: integer value of `key` in the FDHAM_TUNE environment variable (0 if absent)
 int fd_tune_value(const char *key);
 // fd_sweep.cu
 void fd_sweep_configure(fd_plan *plan, int tyc_override, int xchunk_override, int stages_override);
 cudaError_t fd_sweep_prepare(fd_plan *plan);  // shared-memory opt-in of the plan's kernels
-cudaError_t fd_launch_sweep(const fd_plan *plan, const void *psi, const double *v_eff, void *out,
-                            int64_t nbands, cudaStream_t stream, int *nlaunches);
+bool fd_sweep_expect_fused(const fd_plan *plan);  // else: two passes (sweep, then fd_launch_dot)
+int64_t fd_sweep_expect_ws_bytes(const fd_plan *plan, int64_t nbands);
+cudaError_t fd_launch_sweep(const fd_plan *plan, const FdGeom &g, int mode, const void *psi,
+                            const double *second, void *out, int64_t nbands, double *eps,
+                            double *norm, double *ws, cudaStream_t stream, int *nlaunches);

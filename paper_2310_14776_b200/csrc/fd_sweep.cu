@@ -82,16 +82,66 @@ void fd_sweep_configure(fd_plan *plan, int tyc_override, int xchunk_override, in
 
 namespace {
 
-FdSweepKernelFn kernel_for(const fd_plan *plan, bool has_v)
+FdSweepKernelFn kernel_for(const fd_plan *plan, int mode, bool ex)
 {
     const FdGeom &g = plan->g;
     const int rowd = g.n[2] * (g.cplx ? 2 : 1);
-    if (!g.cplx) return fd_sweep_pick_real(rowd, has_v, g.nn);
+    if (!g.cplx) {
+        if (mode == 2) return fd_sweep_pick_real_jacobi(rowd, g.nn);
+        return ex ? fd_sweep_pick_real_ex(rowd, mode, g.nn) : fd_sweep_pick_real(rowd, mode, g.nn);
+    }
+    if (mode == 2) return nullptr;  // the Jacobi sweep is real only
     // which Bloch-phase code the kernel needs: bit 0 = x or y, bit 1 = z
     int ph = 0;
     for (int d = 0; d < 3; ++d)
         if (g.bc[d] && (g.ph_re[d] != 1.0 || g.ph_im[d] != 0.0)) ph |= (d == 2) ? 2 : 1;
-    return fd_sweep_pick_cplx(rowd, has_v, ph, g.nn);
+    return fd_sweep_pick_cplx(rowd, mode, ph, g.nn, ex);
+}
+
+// (band, x) planes per team for a launch of `total` planes (persistent teams unless the xchunk
+// tuning knob is set), capped by the step-table capacity.  0 = cannot launch.
+long long team_quota(const fd_plan *plan, long long total)
+{
+    const FdSweepCfg &c = plan->sweep;
+    const FdGeom &g = plan->g;
+    long long quota;
+    if (c.xchunk > 0) {
+        quota = c.xchunk;
+    } else {
+        quota = (total + c.max_teams - 1) / c.max_teams;
+        const int min_quota = g.n[0] < 16 ? g.n[0] : 16;  // below this the halo planes dominate
+        if (quota < min_quota) quota = min_quota;
+    }
+    // the team's steps (quota + 2 nn per band touched, + 1 prefetched entry) must fit the table
+    const long long quota_cap =
+        ((long long)(c.tab_cap - 4 * g.nn - 1) * g.n[0]) / (g.n[0] + 2 * g.nn);
+    if (quota > quota_cap) quota = quota_cap;
+    return quota < 1 ? 0 : quota;
+}
+
+// plane indices in the step table have kPlaneBits bits: very large batches go out in several launches
+int64_t bands_per_launch(const fd_plan *plan) { return (1LL << kPlaneBits) / plan->g.n[0]; }
+
+// Sums the per-warp partials of the EX sweep kernel (layout: FdSweepAux) band by band in a fixed
+// order: team by team, y tile by y tile, warp by warp.  One thread per band.
+__global__ void fd_expect_finalize_sweep(const double *__restrict__ ws, double *__restrict__ eps,
+                                         double *__restrict__ norm, int nbands, int nx,
+                                         long long quota, int maxseg, int nytiles, int nwarps)
+{
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= nbands) return;
+    const long long l_lo = (long long)b * nx, l_hi = l_lo + nx - 1;
+    double e = 0.0, n = 0.0;
+    for (long long t = l_lo / quota; t <= l_hi / quota; ++t) {
+        const long long seg = b - (t * quota) / nx;  // this band's segment index inside team t
+        const double *w = ws + 2 * ((t * maxseg + seg) * nytiles) * (long long)nwarps;
+        for (int i = 0; i < nytiles * nwarps; ++i) {
+            e += w[2 * i];
+            n += w[2 * i + 1];
+        }
+    }
+    eps[b] = e;
+    norm[b] = n;
 }
 
 }  // namespace
@@ -101,52 +151,75 @@ FdSweepKernelFn kernel_for(const fd_plan *plan, bool has_v)
 // plan with a smaller footprint never lowers the limit under an earlier one.
 cudaError_t fd_sweep_prepare(fd_plan *plan)
 {
-    for (int has_v = 0; has_v < 2; ++has_v) {
-        cudaError_t e = cudaFuncSetAttribute(reinterpret_cast<const void *>(kernel_for(plan, has_v)),
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             kSmemMax);
-        if (e != cudaSuccess) return e;
-    }
+    for (int mode = 0; mode < 3; ++mode)
+        for (int ex = 0; ex < 2; ++ex) {
+            if (mode == 2 && (ex || plan->g.cplx)) continue;
+            cudaError_t e = cudaFuncSetAttribute(
+                reinterpret_cast<const void *>(kernel_for(plan, mode, ex != 0)),
+                cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemMax);
+            if (e != cudaSuccess) return e;
+        }
     return cudaSuccess;
 }
 
-cudaError_t fd_launch_sweep(const fd_plan *plan, const void *psi, const double *v_eff, void *out,
-                            int64_t nbands, cudaStream_t stream, int *nlaunches)
+// Plans on the sweep kernel take the expectation values from the same pass; the others take the
+// two-pass form (fd_aux.cu).
+bool fd_sweep_expect_fused(const fd_plan *plan) { return plan->sweep.supported != 0; }
+
+// Bytes of workspace fd_launch_sweep needs for the expectation values of an `nbands` batch.
+int64_t fd_sweep_expect_ws_bytes(const fd_plan *plan, int64_t nbands)
 {
     const FdSweepCfg &c = plan->sweep;
-    const FdGeom &g = plan->g;
+    const int64_t bpl = bands_per_launch(plan);
+    const int64_t nb = nbands < bpl ? nbands : bpl;
+    const long long total = (long long)nb * plan->g.n[0];
+    const long long quota = team_quota(plan, total);
+    if (quota < 1) return 0;
+    const long long nteams = (total + quota - 1) / quota;
+    const long long maxseg = quota / plan->g.n[0] + 2;
+    return (int64_t)(16 * nteams * maxseg * c.nytiles * (c.threads / 32));
+}
+
+// mode 0: out = T psi; 1: + second (v_eff[nx,ny,nz]) psi; 2: Jacobi form with second = rhs
+// [nbands,nx,ny,nz] (g carries the pre-scaled weights).  eps != nullptr: also the expectation values
+// (partials in ws, fd_sweep_expect_ws_bytes), summed by a second small launch.
+cudaError_t fd_launch_sweep(const fd_plan *plan, const FdGeom &g, int mode, const void *psi,
+                            const double *second, void *out, int64_t nbands, double *eps,
+                            double *norm, double *ws, cudaStream_t stream, int *nlaunches)
+{
+    const FdSweepCfg &c = plan->sweep;
     const long long band_d = (long long)g.n[0] * g.n[1] * g.n[2] * (g.cplx ? 2 : 1);
-    const FdSweepKernelFn kern = kernel_for(plan, v_eff != nullptr);
-    // plane indices in the step table have kPlaneBits bits: very large batches go out in several
-    // launches
-    const int64_t bands_per_launch = (1LL << kPlaneBits) / g.n[0];
-    for (int64_t b0 = 0; b0 < nbands; b0 += bands_per_launch) {
-        const int64_t nb = (nbands - b0 < bands_per_launch) ? nbands - b0 : bands_per_launch;
+    const bool ex = eps != nullptr;
+    const FdSweepKernelFn kern = kernel_for(plan, mode, ex);
+    if (!kern) return cudaErrorInvalidValue;
+    const int64_t bpl = bands_per_launch(plan);
+    for (int64_t b0 = 0; b0 < nbands; b0 += bpl) {
+        const int64_t nb = (nbands - b0 < bpl) ? nbands - b0 : bpl;
         const long long total = (long long)nb * g.n[0];
-        long long quota;
-        if (c.xchunk > 0) {
-            quota = c.xchunk;
-        } else {
-            quota = (total + c.max_teams - 1) / c.max_teams;
-            const int min_quota = g.n[0] < 16 ? g.n[0] : 16;  // below this the halo planes dominate
-            if (quota < min_quota) quota = min_quota;
-        }
-        // the team's steps (quota + 2 nn per band touched, + 1 prefetched entry) must fit the table
-        const long long quota_cap =
-            ((long long)(c.tab_cap - 4 * g.nn - 1) * g.n[0]) / (g.n[0] + 2 * g.nn);
-        if (quota > quota_cap) quota = quota_cap;
+        const long long quota = team_quota(plan, total);
         if (quota < 1) return cudaErrorInvalidConfiguration;
         const long long nteams = (total + quota - 1) / quota;
         const long long nblocks = nteams * c.nytiles;
         if (nblocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
         const double *p = static_cast<const double *>(psi) + b0 * band_d;
         double *o = static_cast<double *>(out) + b0 * band_d;
-        kern<<<dim3((unsigned)nblocks), dim3((unsigned)(c.threads_wg + kFdSweepProducerThreads)), (size_t)c.smem_bytes,
-               stream>>>(
-            g, c, p, v_eff, o, total, (int)quota);
+        const double *sec = (mode == 2) ? second + b0 * band_d : second;
+        FdSweepAux aux;
+        aux.ws = ws;
+        aux.maxseg = (int)(quota / g.n[0] + 2);
+        kern<<<dim3((unsigned)nblocks), dim3((unsigned)(c.threads_wg + kFdSweepProducerThreads)),
+               (size_t)c.smem_bytes, stream>>>(g, c, p, sec, o, total, (int)quota, aux);
         cudaError_t e = cudaPeekAtLastError();
         if (e != cudaSuccess) return e;
         if (nlaunches) ++*nlaunches;
+        if (ex) {
+            fd_expect_finalize_sweep<<<dim3((unsigned)((nb + 127) / 128)), dim3(128), 0, stream>>>(
+                ws, eps + b0, norm + b0, (int)nb, g.n[0], quota, aux.maxseg, c.nytiles,
+                c.threads / 32);
+            e = cudaPeekAtLastError();
+            if (e != cudaSuccess) return e;
+            if (nlaunches) ++*nlaunches;
+        }
     }
     return cudaSuccess;
 }

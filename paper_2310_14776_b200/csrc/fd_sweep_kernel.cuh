@@ -225,14 +225,27 @@ struct TeamRange {
     }
 };
 
+// MODE: what rides the second staged array -- 0: nothing (kinetic), 1: v_eff[nx,ny,nz], added to
+//   the diagonal (H psi), 2: a right-hand side rhs[nbands,nx,ny,nz] added as g.rhs_coef * rhs (the
+//   weighted-Jacobi sweep of fd_jacobi_sweep: the plan's weights arrive pre-scaled in g; real only).
 // PH (complex only): which Bloch-phase code is compiled in -- bit 0: x and y wraps, bit 1: z wraps.
 // NN: stencil half width (1..3); 2 NN + 1 register accumulators per point, unrolled 2 NN + 1 times.
-template <bool CPLX, bool HAS_V, int ROWD, int PH, int NN>
+// EX: also accumulate sum conj(psi) H psi and sum |psi|^2 per band (fd_apply_hamiltonian_expect).
+//   H is Hermitian: sum_i conj(psi_i) (F psi)_i = conj( sum_i conj(psi_i) (B psi)_i ) for the
+//   forward / backward halves F, B of the taps along an axis (wrapped taps carry conjugate Bloch
+//   factors), so  eps = sum_i [ d_i |psi_i|^2 + 2 Re conj(psi_i) (B psi)_i ]  needs only taps that
+//   are already in the accumulator when psi_i is in registers (x: the planes that arrived before).
+//   Each warp writes one partial (eps, norm) pair per band segment; fd_expect_finalize_sweep adds
+//   them in a fixed order (deterministic, no atomics).
+template <bool CPLX, int MODE, int ROWD, int PH, int NN, bool EX>
 __global__ void __launch_bounds__(kMaxThreads + kProducerThreads, 1)
 fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSweepCfg cfg,
                 const double *__restrict__ psi, const double *__restrict__ v_eff,
-                double *__restrict__ out, const long long total_planes, const int quota)
+                double *__restrict__ out, const long long total_planes, const int quota,
+                const FdSweepAux aux)
 {
+    constexpr bool HAS_V = MODE != 0;
+    static_assert(!(CPLX && MODE == 2), "the Jacobi sweep is real only");
     constexpr int TY = 4;              // rows per thread
     constexpr int TC = 1;              // 16-byte chunks per thread per row (lane stride 16 B)
     constexpr int ZH = CPLX ? NN : (NN + 1) / 2;   // halo chunks per side along z
@@ -330,9 +343,14 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
                 const double *src = psi + (long long)(me.y + (unsigned)xs) * plane_d;
                 const bool with_v = HAS_V && (mx & kCentre);
                 mbar_expect_tx(bar, tx_psi + (with_v ? tx_v : 0u));
-                if (with_v)
-                    bulk_g2s_hint(stage0 + s * stage_bytes + (uint32_t)cfg.v_off,
-                                  v_eff + ((long long)xl * ny + y0) * nz, tx_v, bar, pol);
+                if (with_v) {
+                    if (MODE == 2)  // the band's own right-hand side plane: streamed once
+                        bulk_g2s(stage0 + s * stage_bytes + (uint32_t)cfg.v_off,
+                                 v_eff + ((long long)(me.y + (unsigned)xl) * ny + y0) * nz, tx_v, bar);
+                    else
+                        bulk_g2s_hint(stage0 + s * stage_bytes + (uint32_t)cfg.v_off,
+                                      v_eff + ((long long)xl * ny + y0) * nz, tx_v, bar, pol);
+                }
                 if (mx & kKeepL2) {
                     if (per_y && nlo > 0)
                         bulk_g2s_hint(dst, src + (long long)(ny - nlo) * rowd, (uint32_t)(nlo * pitch),
@@ -421,6 +439,15 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
 #pragma unroll
         for (int p = 0; p < NP; ++p) acc[a][p] = make_double2(0.0, 0.0);
 
+    // EX: this thread's share of eps / norm of the current band segment.  One chain each: more
+    // chains spill at 160 registers (float64) or run slower (complex128: measured).  Rows outside the
+    // grid (surplus threads, ragged last tile) are masked per row; dropping the masks for grids with
+    // ny % 4 == 0 was measured slower (ptxas schedules the select form better), so they stay.
+    constexpr int EXC = 1;
+    double ex_e[EXC], ex_n[EXC];
+#pragma unroll
+    for (int i = 0; i < EXC; ++i) ex_e[i] = ex_n[i] = 0.0;
+    int ex_seg = 0;
     uint32_t st = 0, par = 0;  // ring slot and mbarrier phase parity of the current step
     uint2 m = tabp[0];         // .x flags (| load plane), .y out plane of the current step
     for (int q7 = 0; q7 < nsteps; q7 += NS) {
@@ -499,13 +526,8 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
                                 x_taps_row(i, c);
                                 double2 &a = acc[J][i];
                                 // diagonal (+ v_eff)
-                                double d0 = wdiag, d1 = wdiag;
-                                if (HAS_V) {
-                                    d0 += lds64(sb + v_off + i * pitchv);
-                                    d1 = d0;
-                                }
-                                a.x = fma(d0, c.x, a.x);
-                                a.y = fma(d1, c.y, a.y);
+                                double d0 = wdiag;
+                                if (HAS_V) d0 += lds64(sb + v_off + i * pitchv);
                                 // z taps
                                 {
                                     // chunk = one complex point; hz = L_NN .. L_1, R_1 .. R_NN
@@ -520,10 +542,30 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
                                             if (wbits == 2) hz[k] = cmul(hz[k], g.ph_re[2], g.ph_im[2]);
                                         }
                                     }
+                                    if constexpr (!EX) {
+                                        a.x = fma(d0, c.x, a.x);
+                                        a.y = fma(d0, c.y, a.y);
+                                    }
+                                    if constexpr (EX) {
+                                        // a holds the backward x and y taps of this row; add the
+                                        // backward z taps: eps += d |c|^2 + 2 Re conj(c) a
 #pragma unroll
-                                    for (int j = 1; j <= NN; ++j) {
-                                        fma2(a, wz[j], hz[NN - j]);
-                                        fma2(a, wz[j], hz[NN + j - 1]);
+                                        for (int j = 1; j <= NN; ++j) fma2(a, wz[j], hz[NN - j]);
+                                        if (row_ok & (1u << i)) {
+                                            const double s2 = fma(c.x, c.x, c.y * c.y);
+                                            ex_n[i % EXC] += s2;
+                                            ex_e[i % EXC] = fma(c.x, a.x, fma(c.y, a.y, fma(0.5 * d0, s2, ex_e[i % EXC])));
+                                        }
+#pragma unroll
+                                        for (int j = 1; j <= NN; ++j) fma2(a, wz[j], hz[NN + j - 1]);
+                                        a.x = fma(d0, c.x, a.x);
+                                        a.y = fma(d0, c.y, a.y);
+                                    } else {
+#pragma unroll
+                                        for (int j = 1; j <= NN; ++j) {
+                                            fma2(a, wz[j], hz[NN - j]);
+                                            fma2(a, wz[j], hz[NN + j - 1]);
+                                        }
                                     }
                                 }
                             }
@@ -567,17 +609,30 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
                     }
 
                     if (m.x & kCentre) {
-                        // ---- diagonal (+ v_eff)
+                        if constexpr (EX) {
+                            // acc[J] holds the backward x taps B of this plane: eps += u (B + H_rest u),
+                            // the second term once acc[J] is complete (below)
+#pragma unroll
+                            for (int i = 0; i < TY; ++i)
+                                if (row_ok & (1u << i))
+                                    ex_e[i % EXC] = fma(u[i].x, acc[J][i].x, fma(u[i].y, acc[J][i].y, ex_e[i % EXC]));
+                        }
+                        // ---- diagonal (+ v_eff), or the Jacobi form (1 - omega) phi + rhs_coef rhs
 #pragma unroll
                         for (int i = 0; i < TY; ++i) {
                             double d0 = wdiag, d1 = wdiag;
-                            if (HAS_V) {
+                            if (MODE == 1) {
                                 const double2 vv = lds128(sb + v_off + i * pitchv);
                                 d0 += vv.x;
                                 d1 += vv.y;
                             }
                             acc[J][i].x = fma(d0, u[i].x, acc[J][i].x);
                             acc[J][i].y = fma(d1, u[i].y, acc[J][i].y);
+                            if (MODE == 2) {
+                                const double2 vv = lds128(sb + v_off + i * pitchv);
+                                acc[J][i].x = fma(g.rhs_coef, vv.x, acc[J][i].x);
+                                acc[J][i].y = fma(g.rhs_coef, vv.y, acc[J][i].y);
+                            }
                         }
                         // ---- y taps: stream the TY + 6 rows of the thread's column through
 #pragma unroll
@@ -663,6 +718,14 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
                                 }
                             }
                         }
+                        if constexpr (EX) {
+#pragma unroll
+                            for (int i = 0; i < TY; ++i)
+                                if (row_ok & (1u << i)) {
+                                    ex_e[i % EXC] = fma(u[i].x, acc[J][i].x, fma(u[i].y, acc[J][i].y, ex_e[i % EXC]));
+                                    ex_n[i % EXC] = fma(u[i].x, u[i].x, fma(u[i].y, u[i].y, ex_n[i % EXC]));
+                                }
+                        }
                     }
 
                 }
@@ -675,6 +738,31 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
                 if constexpr (!CPLX) {
 #pragma unroll
                     for (int p = 0; p < NP; ++p) acc[(J + NN) % NS][p] = mul2(wx[NN], u[p]);
+                }
+                if constexpr (EX) {
+                    // end of a band segment: this warp's partial sums go out, fixed butterfly order
+                    if (mn.y != m.y || q + 1 == nsteps) {
+                        double se = 0.0, sn = 0.0;
+#pragma unroll
+                        for (int i = 0; i < EXC; ++i) {
+                            se += ex_e[i];
+                            sn += ex_n[i];
+                            ex_e[i] = ex_n[i] = 0.0;
+                        }
+                        if (CPLX) se *= 2.0;  // the complex body accumulates half of eps
+#pragma unroll
+                        for (int o = 16; o > 0; o >>= 1) {
+                            se += __shfl_xor_sync(0xffffffffu, se, o);
+                            sn += __shfl_xor_sync(0xffffffffu, sn, o);
+                        }
+                        if ((tid & 31) == 0) {
+                            double *w = aux.ws + 2 * ((((team * aux.maxseg + ex_seg) * cfg.nytiles + yt) *
+                                                       (long long)nwarps) + (tid >> 5));
+                            w[0] = se;
+                            w[1] = sn;
+                        }
+                        ++ex_seg;
+                    }
                 }
                 if (++st == (uint32_t)K) {
                     st = 0;

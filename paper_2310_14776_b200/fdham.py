@@ -24,7 +24,9 @@ LIB_PATH = os.path.join(_HERE, "libfdham.so")
 
 EXPORTED_SYMBOLS = [
     "fd_create", "fd_create_scaled", "fd_apply_kinetic", "fd_apply_hamiltonian",
-    "fd_apply_hamiltonian_host",
+    "fd_apply_hamiltonian_host", "fd_workspace_create", "fd_workspace_destroy",
+    "fd_apply_hamiltonian_host_ws", "fd_expect_workspace_bytes", "fd_apply_hamiltonian_expect",
+    "fd_residual", "fd_jacobi_sweep",
     "fd_destroy", "fd_strerror", "fd_plan_set_kernel", "fd_plan_get_kernel", "fd_plan_kernel_for", "fd_plan_launches",
     "fd_plan_get_weights",
 ]
@@ -62,6 +64,20 @@ def load_library() -> ctypes.CDLL:
     lib.fd_apply_hamiltonian.restype = ctypes.c_int
     lib.fd_apply_hamiltonian_host.argtypes = [vp, vp, vp, vp, i64]
     lib.fd_apply_hamiltonian_host.restype = ctypes.c_int
+    lib.fd_workspace_create.argtypes = [ctypes.POINTER(vp), vp, i64]
+    lib.fd_workspace_create.restype = ctypes.c_int
+    lib.fd_workspace_destroy.argtypes = [vp]
+    lib.fd_workspace_destroy.restype = ctypes.c_int
+    lib.fd_apply_hamiltonian_host_ws.argtypes = [vp, vp, vp, vp, vp, i64]
+    lib.fd_apply_hamiltonian_host_ws.restype = ctypes.c_int
+    lib.fd_expect_workspace_bytes.argtypes = [vp, i64]
+    lib.fd_expect_workspace_bytes.restype = ctypes.c_int64
+    lib.fd_apply_hamiltonian_expect.argtypes = [vp, vp, vp, vp, vp, vp, i64, vp, i64, vp]
+    lib.fd_apply_hamiltonian_expect.restype = ctypes.c_int
+    lib.fd_residual.argtypes = [vp, vp, vp, vp, vp, vp, i64, vp]
+    lib.fd_residual.restype = ctypes.c_int
+    lib.fd_jacobi_sweep.argtypes = [vp, vp, vp, vp, i64, ctypes.c_double, vp]
+    lib.fd_jacobi_sweep.restype = ctypes.c_int
     lib.fd_destroy.argtypes = [vp]
     lib.fd_destroy.restype = ctypes.c_int
     lib.fd_strerror.argtypes = [ctypes.c_int]
@@ -169,6 +185,59 @@ def fd_apply_hamiltonian_host(plan, psi_host, v_eff_host, out_host) -> None:
                                                   _host_ptr(v_eff_host), _host_ptr(out_host),
                                                   int(psi_host.shape[0]))
     _check(rc, "fd_apply_hamiltonian_host")
+
+
+def fd_workspace_create(plan, chunk_bytes: int = 0) -> ctypes.c_void_p:
+    """Staging buffers + streams for fd_apply_hamiltonian_host_ws (include/fdham.h)."""
+    ws = ctypes.c_void_p()
+    _check(load_library().fd_workspace_create(ctypes.byref(ws), plan, int(chunk_bytes)),
+           "fd_workspace_create")
+    return ws
+
+
+def fd_workspace_destroy(ws) -> None:
+    _check(load_library().fd_workspace_destroy(ws), "fd_workspace_destroy")
+
+
+def fd_apply_hamiltonian_host_ws(plan, ws, psi_host, v_eff_host, out_host) -> None:
+    """fd_apply_hamiltonian_host on a caller-owned workspace (no allocation in the call)."""
+    rc = load_library().fd_apply_hamiltonian_host_ws(plan, ws, _host_ptr(psi_host),
+                                                     _host_ptr(v_eff_host), _host_ptr(out_host),
+                                                     int(psi_host.shape[0]))
+    _check(rc, "fd_apply_hamiltonian_host_ws")
+
+
+def fd_expect_workspace_bytes(plan, nbands: int) -> int:
+    n = int(load_library().fd_expect_workspace_bytes(plan, int(nbands)))
+    if n < 0:
+        raise FDError(n, "fd_expect_workspace_bytes")
+    return n
+
+
+def fd_apply_hamiltonian_expect(plan, psi, v_eff, out, eps, norm, workspace, stream=None) -> None:
+    """out = H psi (v_eff None: T psi), eps[b] = Re <psi_b|H psi_b>, norm[b] = <psi_b|psi_b> (grid
+    sums) in one pass; eps/norm float64 CUDA tensors [nbands], workspace a CUDA byte/float64 tensor
+    of at least fd_expect_workspace_bytes(plan, nbands) bytes."""
+    rc = load_library().fd_apply_hamiltonian_expect(
+        plan, _dev_ptr(psi), _dev_ptr(v_eff) if v_eff is not None else ctypes.c_void_p(0),
+        _dev_ptr(out), _dev_ptr(eps), _dev_ptr(norm), int(psi.shape[0]), _dev_ptr(workspace),
+        int(workspace.numel() * workspace.element_size()), _stream_ptr(stream))
+    _check(rc, "fd_apply_hamiltonian_expect")
+
+
+def fd_residual(plan, psi, hpsi, eps, norm, r, stream=None) -> None:
+    """r_b = hpsi_b - (eps[b] / norm[b]) psi_b; r may be hpsi itself."""
+    rc = load_library().fd_residual(plan, _dev_ptr(psi), _dev_ptr(hpsi), _dev_ptr(eps),
+                                    _dev_ptr(norm), _dev_ptr(r), int(psi.shape[0]),
+                                    _stream_ptr(stream))
+    _check(rc, "fd_residual")
+
+
+def fd_jacobi_sweep(plan, phi, rhs, out, omega: float, stream=None) -> None:
+    """out = phi + omega (rhs - A phi) / A_ii for the plan's A = scale lap_FD (fd_create_scaled)."""
+    rc = load_library().fd_jacobi_sweep(plan, _dev_ptr(phi), _dev_ptr(rhs), _dev_ptr(out),
+                                        int(phi.shape[0]), float(omega), _stream_ptr(stream))
+    _check(rc, "fd_jacobi_sweep")
 
 
 def fd_plan_set_kernel(plan, kernel: int, param: int = 0) -> None:

@@ -1,0 +1,322 @@
+"""GPU parity of the SURVEY 8(f) rows that ride the stencil kernels: f2 (fused expectation values,
+residual) and the f3 weighted-Jacobi sweep, through the C ABI, against the CPU oracle."""
+import itertools
+
+import numpy as np
+import pytest
+
+import workloads as W
+from helpers import kinetic_row_sum, parity_tol, planewave, planewave_eig
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def fd():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2310_14776_b200 import build
+    build.build()
+    import paper_2310_14776_b200 as fd
+    fd.load_library()
+    return fd
+
+
+def expect_tol(h, nn, psi, v, scale=-0.5):
+    """|d eps| <= 1e-12 P (max|psi|^2 S + max|v psi^2|): P times the per-point tolerance of H psi
+    times max|psi| (reading R15); |d norm| <= 1e-12 P max|psi|^2."""
+    P = psi[0].size
+    mp = float(np.abs(psi).max())
+    mv = float(np.abs(v[None] * psi * psi).max()) if v is not None else 0.0
+    return 1e-12 * P * (mp * mp * kinetic_row_sum(h, nn, scale) + mv), 1e-12 * P * mp * mp
+
+
+def run_expect(fd, cfg, psi, v, kernel, tyc=0, scale=None):
+    k = cfg.k if cfg.complex else None
+    dt = fd.FD_C128 if cfg.complex else fd.FD_F64
+    plan = (fd.fd_create(cfg.shape, cfg.h, cfg.nn, cfg.bc, k, dt, 0) if scale is None else
+            fd.fd_create_scaled(cfg.shape, cfg.h, cfg.nn, cfg.bc, k, dt, 0, scale))
+    try:
+        if kernel != "auto":
+            fd.fd_plan_set_kernel(plan, kernel, tyc)
+        nb = psi.shape[0]
+        d_psi = torch.from_numpy(psi).cuda()
+        d_v = torch.from_numpy(v).cuda() if v is not None else None
+        d_out = torch.full_like(d_psi, float("nan"))
+        eps = torch.full((nb,), float("nan"), dtype=torch.float64, device="cuda")
+        norm = torch.full((nb,), float("nan"), dtype=torch.float64, device="cuda")
+        ws = torch.full((fd.fd_expect_workspace_bytes(plan, nb) // 8 + 1,), float("nan"),
+                        dtype=torch.float64, device="cuda")
+        fd.fd_apply_hamiltonian_expect(plan, d_psi, d_v, d_out, eps, norm, ws)
+        torch.cuda.synchronize()
+        e1, n1 = eps.cpu().numpy(), norm.cpu().numpy()
+        # bit-reproducible: a second call gives identical sums
+        eps2, norm2 = torch.empty_like(eps), torch.empty_like(norm)
+        fd.fd_apply_hamiltonian_expect(plan, d_psi, d_v, d_out, eps2, norm2, ws)
+        torch.cuda.synchronize()
+        assert torch.equal(eps, eps2) and torch.equal(norm, norm2)
+        return d_out.cpu().numpy(), e1, n1, fd.fd_plan_kernel_for(plan, nb)
+    finally:
+        fd.fd_destroy(plan)
+
+
+def check_expect(oracle, fd, cfg, kernel, tyc=0, with_v=True, scale=None):
+    psi = W.make_psi(cfg)
+    v = W.make_veff(cfg) if with_v else None
+    k = cfg.k if cfg.complex else None
+    sc = -0.5 if scale is None else scale
+    got, eps, norm, used = run_expect(fd, cfg, psi, v, kernel, tyc, scale)
+    w_eps, w_norm, want = oracle.expect(cfg.shape, cfg.h, cfg.nn, cfg.bc, k, psi, v, scale=sc,
+                                        want_out=True)
+    assert np.max(np.abs(got - want)) <= parity_tol(cfg.h, cfg.nn, psi, v, sc)
+    te, tn = expect_tol(cfg.h, cfg.nn, psi, v, sc)
+    assert np.max(np.abs(eps - w_eps.real)) <= te, (np.max(np.abs(eps - w_eps.real)), te)
+    assert np.max(np.abs(norm - w_norm)) <= tn
+    return used
+
+
+@pytest.mark.parametrize("idx", [1, 2])
+@pytest.mark.parametrize("kernel", ["auto", "sweep", "generic"])
+def test_expect_small_configs(oracle, fd, idx, kernel):
+    cfg = W.get(idx)
+    forced = {"auto": "auto", "sweep": fd.FD_KERNEL_SWEEP, "generic": fd.FD_KERNEL_GENERIC}[kernel]
+    check_expect(oracle, fd, cfg, forced)
+
+
+@pytest.mark.parametrize("bc", list(itertools.product((0, 1), repeat=3)))
+def test_expect_all_bc_mixes_ragged_tiles(oracle, fd, bc):
+    """several y tiles with a ragged one, several bands per team, real and complex Bloch, with and
+    without v_eff, nn = 1..3, on the sweep kernel's fused epilogue"""
+    for nn in (3, 2, 1):
+        # ny = 28: tiles of 8, 8, 8, 4 rows (fused epilogue: ny % 4 == 0); ny = 30: two-pass form
+        for ny in (28, 30):
+            cfg = W.custom((10, ny, 16), (0.2, 0.23, 0.17), bc, nbands=5, nn=nn)
+            assert check_expect(oracle, fd, cfg, fd.FD_KERNEL_SWEEP, tyc=8) == fd.FD_KERNEL_SWEEP
+    k = tuple(kk if b else 0.0 for kk, b in zip((0.25, 0.125, -0.3), bc))
+    ck = W.custom((10, 20, 12), (0.2, 0.23, 0.17), bc, k=k, complex_=True, nbands=4)
+    assert check_expect(oracle, fd, ck, fd.FD_KERNEL_SWEEP, tyc=8) == fd.FD_KERNEL_SWEEP
+    check_expect(oracle, fd, ck, fd.FD_KERNEL_SWEEP, tyc=12, with_v=False)
+    ck = W.custom((10, 22, 12), (0.2, 0.23, 0.17), bc, k=k, complex_=True, nbands=4)
+    check_expect(oracle, fd, ck, fd.FD_KERNEL_SWEEP, tyc=8)
+    check_expect(oracle, fd, W.custom((9, 12, 8), (0.2, 0.23, 0.17), bc, nbands=3), fd.FD_KERNEL_SWEEP,
+                 with_v=False, scale=1.0)
+
+
+@pytest.mark.parametrize("xchunk", [3, 7])
+def test_expect_band_segments_split_over_teams(oracle, fd, monkeypatch, xchunk):
+    """FDHAM_TUNE=xchunk cuts bands into many team segments: every band's partial sums come from
+    several teams and the fixed-order reduction must find all of them."""
+    monkeypatch.setenv("FDHAM_TUNE", f"xchunk={xchunk},kernel=2")
+    for bc, cplx, k in [((1, 1, 1), False, (0, 0, 0)), ((0, 1, 0), False, (0, 0, 0)),
+                        ((1, 1, 1), True, (0.25, 0.125, -0.3))]:
+        cfg = W.custom((24, 40, 16), (0.2, 0.21, 0.18), bc, k=k, complex_=cplx, nbands=11)
+        assert check_expect(oracle, fd, cfg, "auto") == fd.FD_KERNEL_SWEEP
+
+
+def test_expect_plane_waves_closed_form(fd):
+    """against the closed form directly: eps = lambda P |a|^2, norm = P |a|^2"""
+    n, h_ang, k = (24, 16, 32), (0.2, 0.21, 0.18), (0.25, 0.125, -0.4)
+    ms = [(1, 2, 3), (0, 0, 0), (3, -2, 1)]
+    cfg = W.custom(n, h_ang, (1, 1, 1), k=k, complex_=True, nbands=len(ms))
+    psi = np.stack([planewave(n, k, m) for m in ms])
+    _, eps, norm, used = run_expect(fd, cfg, psi, None, fd.FD_KERNEL_SWEEP)
+    assert used == fd.FD_KERNEL_SWEEP
+    P = float(np.prod(n))
+    lam = np.array([planewave_eig(n, cfg.h, k, m) for m in ms])
+    assert np.max(np.abs(norm - P)) <= 1e-12 * P
+    assert np.max(np.abs(eps - lam * P)) <= 1e-12 * P * kinetic_row_sum(cfg.h)
+
+
+def _big_expect(oracle, fd, cfg, bands):
+    """full-size config in the launch configuration bench.py times; oracle on a few whole bands"""
+    plan = fd.fd_create(cfg.shape, cfg.h, cfg.nn, cfg.bc, cfg.k if cfg.complex else None,
+                        fd.FD_C128 if cfg.complex else fd.FD_F64, 0)
+    try:
+        tdt = torch.complex128 if cfg.complex else torch.float64
+        d_psi = torch.empty((cfg.nbands,) + cfg.shape, dtype=tdt, device="cuda")
+        for b0 in range(0, cfg.nbands, 32):
+            bs = range(b0, min(cfg.nbands, b0 + 32))
+            d_psi[b0:b0 + len(bs)] = torch.from_numpy(W.make_psi(cfg, bs)).cuda()
+        v = W.make_veff(cfg)
+        d_v = torch.from_numpy(v).cuda()
+        d_out = torch.full_like(d_psi, float("nan"))
+        eps = torch.empty(cfg.nbands, dtype=torch.float64, device="cuda")
+        norm = torch.empty_like(eps)
+        ws = torch.empty(fd.fd_expect_workspace_bytes(plan, cfg.nbands) // 8 + 1,
+                         dtype=torch.float64, device="cuda")
+        fd.fd_apply_hamiltonian_expect(plan, d_psi, d_v, d_out, eps, norm, ws)
+        torch.cuda.synchronize()
+        # all bands: the sums agree with a plain reduction of the kernel's own output (fp64, torch)
+        ref_n = (d_psi.abs() ** 2).sum(dim=(1, 2, 3))
+        ref_e = (d_psi.conj() * d_out).sum(dim=(1, 2, 3)).real
+        psi_s = W.make_psi(cfg, bands)
+        te, tn = expect_tol(cfg.h, cfg.nn, psi_s, v)
+        assert float((norm - ref_n).abs().max()) <= 4 * tn
+        assert float((eps - ref_e).abs().max()) <= 4 * te
+        # sampled whole bands against the oracle
+        w_eps, w_norm, want = oracle.expect(cfg.shape, cfg.h, cfg.nn, cfg.bc,
+                                            cfg.k if cfg.complex else None, psi_s, v, want_out=True)
+        got = d_out[list(bands)].cpu().numpy()
+        assert np.max(np.abs(got - want)) <= parity_tol(cfg.h, cfg.nn, psi_s, v)
+        assert np.max(np.abs(eps[list(bands)].cpu().numpy() - w_eps.real)) <= te
+        assert np.max(np.abs(norm[list(bands)].cpu().numpy() - w_norm)) <= tn
+    finally:
+        fd.fd_destroy(plan)
+
+
+def test_expect_config3_full_size(oracle, fd):
+    _big_expect(oracle, fd, W.get(3), [0, 100, 255])
+
+
+def test_expect_config4_full_size(oracle, fd):
+    _big_expect(oracle, fd, W.get(4), [0, 64, 127])
+
+
+def test_expect_config5_full_size(oracle, fd):
+    _big_expect(oracle, fd, W.get(5), [0, 383])
+
+
+def test_expect_argument_errors(fd):
+    plan = fd.fd_create((16, 16, 16), (0.4,) * 3)
+    try:
+        x = torch.zeros((2, 16, 16, 16), dtype=torch.float64, device="cuda")
+        y = torch.zeros_like(x)
+        e = torch.zeros(2, dtype=torch.float64, device="cuda")
+        n = torch.zeros(2, dtype=torch.float64, device="cuda")
+        need = fd.fd_expect_workspace_bytes(plan, 2)
+        assert need >= 16
+        small = torch.zeros(1, dtype=torch.float64, device="cuda")
+        with pytest.raises(fd.FDError) as ei:
+            fd.fd_apply_hamiltonian_expect(plan, x, None, y, e, n, small)
+        assert ei.value.status == -1
+        ws = torch.zeros(need // 8 + 1, dtype=torch.float64, device="cuda")
+        with pytest.raises(fd.FDError) as ei:
+            fd.fd_apply_hamiltonian_expect(plan, x, None, y, e, e, ws)          # eps aliases norm
+        assert ei.value.status == -3
+        with pytest.raises(fd.FDError) as ei:
+            fd.fd_apply_hamiltonian_expect(plan, x, None, y, y.view(-1)[:2], n, ws)   # eps inside out
+        assert ei.value.status == -3
+        fd.fd_apply_hamiltonian_expect(plan, x, None, y, e, n, ws)
+        torch.cuda.synchronize()
+    finally:
+        fd.fd_destroy(plan)
+
+
+@pytest.mark.parametrize("cplx", [False, True])
+def test_residual(oracle, fd, cplx):
+    cfg = W.custom((12, 16, 20), (0.2, 0.21, 0.19), (1, 0, 1), complex_=cplx, nbands=5,
+                   k=(0.25, 0, 0.125) if cplx else (0, 0, 0))
+    psi, v = W.make_psi(cfg), W.make_veff(cfg)
+    got, eps, norm, _ = run_expect(fd, cfg, psi, v, "auto")
+    plan = fd.fd_create(cfg.shape, cfg.h, 3, cfg.bc, cfg.k if cplx else None,
+                        fd.FD_C128 if cplx else fd.FD_F64, 0)
+    try:
+        d_psi, d_h = torch.from_numpy(psi).cuda(), torch.from_numpy(got).cuda()
+        d_e, d_n = torch.from_numpy(eps).cuda(), torch.from_numpy(norm).cuda()
+        r = torch.full_like(d_psi, float("nan"))
+        fd.fd_residual(plan, d_psi, d_h, d_e, d_n, r)
+        torch.cuda.synchronize()
+        want = oracle.residual(psi, got, eps / norm)
+        tol = 1e-13 * (np.abs(got).max() + np.abs(eps / norm).max() * np.abs(psi).max())
+        assert np.max(np.abs(r.cpu().numpy() - want)) <= tol
+        fd.fd_residual(plan, d_psi, d_h, d_e, d_n, d_h)                        # in place
+        torch.cuda.synchronize()
+        assert np.max(np.abs(d_h.cpu().numpy() - want)) <= tol
+        with pytest.raises(fd.FDError) as ei:
+            fd.fd_residual(plan, d_psi, d_h, d_e, d_n, d_psi)
+        assert ei.value.status == -3
+    finally:
+        fd.fd_destroy(plan)
+
+
+# ------------------------------------------------------------------------------ f3: Jacobi sweep
+
+def jacobi_tol(h, nn, phi, rhs, omega, scale):
+    S = kinetic_row_sum(h, nn, scale)
+    c0 = {1: 2.0, 2: 2.5, 3: 49.0 / 18.0, 4: 205.0 / 72.0, 5: 5269.0 / 1800.0, 6: 5369.0 / 1800.0}[nn]
+    diag = abs(scale) * c0 * sum(1.0 / (x * x) for x in h)
+    return 1e-12 * (np.abs(phi).max() * (1.0 + abs(omega) * S / diag) + abs(omega) * np.abs(rhs).max() / diag)
+
+
+@pytest.mark.parametrize("bc", list(itertools.product((0, 1), repeat=3)))
+def test_jacobi_sweep_both_kernels(oracle, fd, bc):
+    for nn, omega, scale, shape in [(3, 2.0 / 3.0, 1.0, (10, 30, 16)), (1, 1.0, 1.0, (9, 12, 8)),
+                                    (2, 0.8, -0.5, (12, 10, 14)), (4, 0.7, 1.0, (12, 10, 14))]:
+        cfg = W.custom(shape, (0.2, 0.23, 0.17), bc, nbands=4, nn=nn)
+        phi = W.make_psi(cfg)
+        rhs = W.make_psi(W.custom(shape, (0.2, 0.23, 0.17), bc, nbands=4, nn=nn, index=55)) * 30.0
+        want = oracle.jacobi(cfg.shape, cfg.h, nn, bc, phi, rhs, omega, scale)
+        tol = jacobi_tol(cfg.h, nn, phi, rhs, omega, scale)
+        for kern in (fd.FD_KERNEL_SWEEP, fd.FD_KERNEL_GENERIC):
+            plan = fd.fd_create_scaled(cfg.shape, cfg.h, nn, bc, None, fd.FD_F64, 0, scale)
+            try:
+                try:
+                    fd.fd_plan_set_kernel(plan, kern, 8 if kern == fd.FD_KERNEL_SWEEP else 0)
+                except fd.FDError:
+                    assert nn > 3 and kern == fd.FD_KERNEL_SWEEP
+                    continue
+                d_phi, d_rhs = torch.from_numpy(phi).cuda(), torch.from_numpy(rhs).cuda()
+                d_out = torch.full_like(d_phi, float("nan"))
+                fd.fd_jacobi_sweep(plan, d_phi, d_rhs, d_out, omega)
+                torch.cuda.synchronize()
+                err = float(np.max(np.abs(d_out.cpu().numpy() - want)))
+                assert err <= tol, (nn, kern, err, tol)
+            finally:
+                fd.fd_destroy(plan)
+
+
+def test_jacobi_converges_to_the_poisson_solution(fd):
+    """200 damped sweeps on a periodic 16^3 grid reduce the residual of lap phi = rhs for a smooth
+    zero-mean rhs: the kernel is usable as the smoother it is meant to be (no oracle involved)."""
+    n, h = (16, 16, 16), (0.3, 0.3, 0.3)
+    cfg = W.custom(n, h, (1, 1, 1), nbands=1)
+    rhs_np = planewave(n, (0, 0, 0), (1, 0, 0), complex_=False)[None].copy()
+    plan = fd.fd_create_scaled(n, cfg.h, 3, (1, 1, 1), None, fd.FD_F64, 0, 1.0)
+    try:
+        fd.fd_plan_set_kernel(plan, fd.FD_KERNEL_SWEEP)
+        a = torch.zeros((1,) + n, dtype=torch.float64, device="cuda")
+        b = torch.empty_like(a)
+        rhs = torch.from_numpy(rhs_np).cuda()
+        for _ in range(400):
+            fd.fd_jacobi_sweep(plan, a, rhs, b, 0.9)
+            a, b = b, a
+        lap = torch.empty_like(a)
+        fd.fd_apply_kinetic(plan, a, lap)
+        torch.cuda.synchronize()
+        assert float((lap - rhs).abs().max()) < 1e-2 * float(rhs.abs().max())
+    finally:
+        fd.fd_destroy(plan)
+
+
+def test_jacobi_full_size_grid_sampled(oracle, fd):
+    """cfg3's grid, 16 right-hand sides, the launch configuration the bench times; one band in full"""
+    cfg = W.get(3).with_bands(16)
+    phi = W.make_psi(cfg)
+    rhs = W.make_psi(W.custom(cfg.shape, cfg.h_angstrom, cfg.bc, nbands=16, index=56))
+    plan = fd.fd_create_scaled(cfg.shape, cfg.h, 3, cfg.bc, None, fd.FD_F64, 0, 1.0)
+    try:
+        assert fd.fd_plan_kernel_for(plan, 16) == fd.FD_KERNEL_SWEEP
+        d_out = torch.full((16,) + cfg.shape, float("nan"), dtype=torch.float64, device="cuda")
+        fd.fd_jacobi_sweep(plan, torch.from_numpy(phi).cuda(), torch.from_numpy(rhs).cuda(), d_out,
+                           2.0 / 3.0)
+        torch.cuda.synchronize()
+        got = d_out.cpu().numpy()
+        assert np.isfinite(got).all()
+        for b in (0, 15):
+            want = oracle.jacobi(cfg.shape, cfg.h, 3, cfg.bc, phi[b:b + 1], rhs[b:b + 1], 2.0 / 3.0, 1.0)
+            assert np.max(np.abs(got[b:b + 1] - want)) <= jacobi_tol(cfg.h, 3, phi, rhs, 2.0 / 3.0, 1.0)
+    finally:
+        fd.fd_destroy(plan)
+
+
+def test_jacobi_rejects_complex_plans(fd):
+    plan = fd.fd_create((8, 8, 8), (0.4,) * 3, dtype=fd.FD_C128)
+    try:
+        x = torch.zeros((1, 8, 8, 8), dtype=torch.float64, device="cuda")
+        with pytest.raises(fd.FDError) as ei:
+            fd.fd_jacobi_sweep(plan, x, x.clone(), x.clone(), 1.0)
+        assert ei.value.status == -2
+    finally:
+        fd.fd_destroy(plan)

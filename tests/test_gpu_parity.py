@@ -477,3 +477,173 @@ def test_guard_bands_no_out_of_bounds_access(oracle, fd):
                 assert bool((guards == 12345.0).all()), f"{shape} {bc} kernel {kern}: wrote outside out"
             finally:
                 fd.fd_destroy(plan)
+
+
+# ------------------------------------------------------------------------------ every shipped instantiation
+
+# the pick() tables of csrc/fd_sweep_inst_*.cu: row lengths (doubles per z row) with a compile-time
+# pitch.  real: nz; complex: 2 nz.  PH: 0 = Gamma, 1 = k on x / y only, 3 = k_z != 0.
+REAL_ROWD = [24, 48, 64, 96, 128, 192]
+CPLX_NZ = [24, 48, 72, 96]
+
+
+@pytest.mark.parametrize("nz", REAL_ROWD)
+@pytest.mark.parametrize("has_v", [0, 1])
+def test_every_real_row_length_instantiation(oracle, fd, nz, has_v):
+    """mixed BCs, several y tiles with a ragged one, fixed-pitch kernel <0, has_v, nz, 0, 3>"""
+    for bc in [(1, 1, 1), (0, 1, 0), (1, 0, 1)]:
+        cfg = W.custom((9, 22, nz), (0.2, 0.23, 0.17), bc, nbands=3)
+        psi = W.make_psi(cfg)
+        used = check(oracle, fd, cfg, psi, W.make_veff(cfg) if has_v else None,
+                     fd.FD_KERNEL_SWEEP, tyc=8)
+        assert used == fd.FD_KERNEL_SWEEP
+
+
+@pytest.mark.parametrize("nz", CPLX_NZ)
+@pytest.mark.parametrize("ph,k", [(0, (0.0, 0.0, 0.0)), (1, (0.25, 0.125, 0.0)), (3, (0.25, 0.0, -0.3))])
+@pytest.mark.parametrize("has_v", [0, 1])
+def test_every_complex_row_length_and_phase_instantiation(oracle, fd, nz, ph, k, has_v):
+    """fixed-pitch kernels <1, has_v, 2 nz, PH, 3> for PH = 0 (Gamma), 1 (x/y phases), 3 (z phase)"""
+    for bc in [(1, 1, 1), (1, 1, 0) if ph != 3 else (0, 1, 1)]:
+        kk = tuple(x if b else 0.0 for x, b in zip(k, bc))
+        cfg = W.custom((9, 22, nz), (0.2, 0.23, 0.17), bc, k=kk, complex_=True, nbands=3)
+        psi = W.make_psi(cfg)
+        used = check(oracle, fd, cfg, psi, W.make_veff(cfg) if has_v else None,
+                     fd.FD_KERNEL_SWEEP, tyc=8)
+        assert used == fd.FD_KERNEL_SWEEP
+
+
+# ------------------------------------------------------------------------------ metamorphic M5, M6
+
+def test_phase_periodicity_and_gauge_M5(fd):
+    """k and k + integer vector give the same operator; and e^{-ik.r} H_k e^{ik.r} u for periodic u
+    does not depend on which cell the grid origin sits in (shift the origin by one cell: the Bloch
+    function picks up e^{ik.L}, a global phase that must come out of H unchanged)."""
+    shape, h, bc = (12, 16, 20), (0.2, 0.21, 0.19), (1, 1, 1)
+    k = (0.25, 0.125, -0.3)
+    cfg = W.custom(shape, h, bc, k=k, complex_=True, nbands=3)
+    psi, v = W.make_psi(cfg), W.make_veff(cfg)
+    base, _ = gpu_apply(fd, cfg, psi, v, fd.FD_KERNEL_SWEEP, tyc=8)
+    tol = parity_tol(cfg.h, 3, psi, v)
+    for shift in [(1, 0, 0), (0, -2, 0), (3, 1, -1)]:
+        k2 = tuple(a + b for a, b in zip(k, shift))
+        c2 = W.custom(shape, h, bc, k=k2, complex_=True, nbands=3)
+        got, _ = gpu_apply(fd, c2, psi, v, fd.FD_KERNEL_SWEEP, tyc=8)
+        assert np.max(np.abs(got - base)) <= tol
+        gen, _ = gpu_apply(fd, c2, psi, v, fd.FD_KERNEL_GENERIC)
+        assert np.max(np.abs(gen - base)) <= tol
+    # gauge: psi' = e^{2 pi i k_x} psi is the same Bloch function seen from the next cell along x
+    ph = np.exp(2j * np.pi * k[0])
+    got, _ = gpu_apply(fd, cfg, np.ascontiguousarray(ph * psi), v, fd.FD_KERNEL_SWEEP, tyc=8)
+    assert np.max(np.abs(got - ph * base)) <= tol
+    # rolling a Bloch function across the x boundary multiplies the wrapped planes by e^{-ik.L}
+    rolled = np.roll(psi, 5, axis=1).copy()
+    rolled[:, :5] *= np.exp(-2j * np.pi * k[0])
+    vr = np.roll(v, 5, axis=0).copy()
+    got, _ = gpu_apply(fd, cfg, rolled, vr, fd.FD_KERNEL_SWEEP, tyc=8)
+    want = np.roll(base, 5, axis=1).copy()
+    want[:, :5] *= np.exp(-2j * np.pi * k[0])
+    assert np.max(np.abs(got - want)) <= tol
+
+
+def test_separability_with_anisotropic_spacing_M6(fd):
+    """psi = f(x) g(y) h(z)  =>  T psi = (T_x f) g h + f (T_y g) h + f g (T_z h), each 1-D factor
+    taken from the same library on a grid that is trivial along the other two axes."""
+    shape, h, bc = (16, 24, 32), (0.2, 0.26, 0.15), (1, 0, 1)
+    rng = np.random.default_rng(8)
+    f, g, hh = (rng.standard_normal(n) for n in shape)
+    psi = (f[:, None, None] * g[None, :, None] * hh[None, None, :])[None].copy()
+    cfg = W.custom(shape, h, bc, nbands=1)
+    got, _ = gpu_apply(fd, cfg, psi, None, fd.FD_KERNEL_SWEEP, kinetic=True, tyc=8)
+    # 1-D operators from the closed-form weights in helpers (not from the library)
+    from helpers import coeffs_f64
+    c = coeffs_f64(3)
+
+    def t1d(x, hd, per):
+        out = c[0] * x
+        for j in (1, 2, 3):
+            if per:
+                out = out + c[j] * (np.roll(x, j) + np.roll(x, -j))
+            else:
+                up = np.concatenate([x[j:], np.zeros(j)])
+                dn = np.concatenate([np.zeros(j), x[:-j]])
+                out = out + c[j] * (up + dn)
+        return -0.5 * out / (hd * hd)
+
+    hb = cfg.h
+    want = (t1d(f, hb[0], bc[0])[:, None, None] * g[None, :, None] * hh[None, None, :]
+            + f[:, None, None] * t1d(g, hb[1], bc[1])[None, :, None] * hh[None, None, :]
+            + f[:, None, None] * g[None, :, None] * t1d(hh, hb[2], bc[2])[None, None, :])[None]
+    assert np.max(np.abs(got - want)) <= parity_tol(cfg.h, 3, psi, None)
+
+
+# ------------------------------------------------------------------------------ plans living side by side
+
+def test_two_plans_on_one_instantiation_and_refused_set_kernel(oracle, fd):
+    """A later, smaller plan on the same (run-time pitch) instantiation must not break an earlier
+    one; a refused fd_plan_set_kernel leaves the plan usable and unchanged."""
+    ca = W.custom((24, 128, 40), (0.2, 0.2, 0.2), (1, 1, 1), nbands=6, nn=2)
+    cb = W.custom((12, 12, 40), (0.2, 0.2, 0.2), (1, 1, 1), nbands=2, nn=2)
+    pa = fd.fd_create(ca.shape, ca.h, 2, ca.bc)
+    fd.fd_plan_set_kernel(pa, fd.FD_KERNEL_SWEEP)
+    pb = fd.fd_create(cb.shape, cb.h, 2, cb.bc)
+    fd.fd_plan_set_kernel(pb, fd.FD_KERNEL_SWEEP, 4)
+    try:
+        for cfg, plan in ((cb, pb), (ca, pa), (cb, pb)):
+            psi, v = W.make_psi(cfg), W.make_veff(cfg)
+            d_psi = torch.from_numpy(psi).cuda()
+            d_out = torch.full_like(d_psi, float("nan"))
+            fd.fd_apply_hamiltonian(plan, d_psi, torch.from_numpy(v).cuda(), d_out)
+            torch.cuda.synchronize()
+            want = oracle.apply(cfg.shape, cfg.h, 2, cfg.bc, None, psi, v)
+            assert np.max(np.abs(d_out.cpu().numpy() - want)) <= parity_tol(cfg.h, 2, psi, v)
+        # refused request: the sweep family on a plan it cannot run (odd nz); the plan stays usable
+        odd = W.custom((8, 12, 9), (0.2, 0.2, 0.2), (1, 1, 1), nbands=2)
+        pc = fd.fd_create(odd.shape, odd.h, 3, odd.bc)
+        try:
+            before = fd.fd_plan_kernel_for(pc, 2)
+            with pytest.raises(fd.FDError) as ei:
+                fd.fd_plan_set_kernel(pc, fd.FD_KERNEL_SWEEP, 4)
+            assert ei.value.status == -2
+            assert fd.fd_plan_kernel_for(pc, 2) == before == fd.FD_KERNEL_GENERIC
+            psi, v = W.make_psi(odd), W.make_veff(odd)
+            d_psi = torch.from_numpy(psi).cuda()
+            d_out = torch.full_like(d_psi, float("nan"))
+            fd.fd_apply_hamiltonian(pc, d_psi, torch.from_numpy(v).cuda(), d_out)
+            torch.cuda.synchronize()
+            want = oracle.apply(odd.shape, odd.h, 3, odd.bc, None, psi, v)
+            assert np.max(np.abs(d_out.cpu().numpy() - want)) <= parity_tol(odd.h, 3, psi, v)
+        finally:
+            fd.fd_destroy(pc)
+    finally:
+        fd.fd_destroy(pa)
+        fd.fd_destroy(pb)
+
+
+def test_host_workspace_reuse(oracle, fd):
+    cfg = W.custom((24, 32, 48), (0.2,) * 3, (1, 1, 0), nbands=40)
+    psi, v = W.make_psi(cfg), W.make_veff(cfg)
+    plan = fd.fd_create(cfg.shape, cfg.h, 3, cfg.bc)
+    ws = fd.fd_workspace_create(plan, 4 << 20)     # 13 bands per chunk: several ring turns
+    try:
+        want = oracle.apply(cfg.shape, cfg.h, 3, cfg.bc, None, psi, v)
+        p_psi, p_v = torch.from_numpy(psi).pin_memory(), torch.from_numpy(v).pin_memory()
+        for _ in range(3):
+            out = torch.full(psi.shape, float("nan"), dtype=torch.float64).pin_memory()
+            fd.fd_apply_hamiltonian_host_ws(plan, ws, p_psi, p_v, out)
+            assert np.max(np.abs(out.numpy() - want)) <= parity_tol(cfg.h, 3, psi, v)
+        with pytest.raises(fd.FDError) as ei:                    # v_eff inside out
+            big = torch.zeros(psi.size + v.size, dtype=torch.float64)
+            fd.fd_apply_hamiltonian_host_ws(plan, ws, p_psi, big[:v.size].view(v.shape),
+                                            big[:psi.size].view(psi.shape))
+        assert ei.value.status == -3
+        other = fd.fd_create((8, 8, 8), (0.4,) * 3)
+        try:
+            with pytest.raises(fd.FDError) as ei:
+                fd.fd_apply_hamiltonian_host_ws(other, ws, p_psi, p_v, out)
+            assert ei.value.status == -1
+        finally:
+            fd.fd_destroy(other)
+    finally:
+        fd.fd_workspace_destroy(ws)
+        fd.fd_destroy(plan)
