@@ -179,6 +179,30 @@ FD_API int fd_residual(const fd_plan *plan, const void *psi, const void *hpsi, c
 FD_API int fd_jacobi_sweep(const fd_plan *plan, const double *phi, const double *rhs, double *out,
                     int64_t nbands, double omega, void *cuda_stream);
 
+/*
+ * grid transfer between a fine grid (spacing h) and the coarse grid of spacing
+ * 2h ("interpolating from one uniform grid to another", the second C hot spot of PAPER.md:150;
+ * multigrid).  The paper prints no weights; readings R13 / R14:
+ *   1-D interpolation of order p: a fine point on a coarse point copies it; a fine point half way
+ *     between two coarse points is sum_{j=1..p} b_j (c[lo - j + 1] + c[lo + j]) with the midpoint
+ *     Lagrange weights b_j (p = 1: 1/2; p = 2: 9/16, -1/16; p = 3: 150/256, -25/256, 3/256);
+ *     3-D = tensor product.  Restriction = the transpose / 8: per axis weight 1/2 on the fine point
+ *     of the coarse point and b_j / 2 on the fine points at distance 2j - 1.
+ *   Index map per axis: periodic n_f = 2 n_c, coarse I on fine 2I; zero-BC n_f = 2 n_c + 1, coarse
+ *     I on fine 2I + 1 (stored points are interior points; the walls coincide).  Values outside
+ *     [0, n) are wrapped (periodic) or 0 (zero BC).
+ * fd_restrict:    coarse[nbands, nc] <- fine[nbands, nf];   fd_interpolate: fine <- coarse.
+ *   shape_fine   host: nf per axis (even >= 2 on periodic axes, odd >= 3 on zero-BC axes)
+ *   bc           host: FD_BC_* per axis;   p: 1..3 (4..6: FD_ERR_UNSUPPORTED)
+ *   fine, coarse device pointers (current device), double, C-contiguous, 8-byte aligned, no overlap
+ * Stateless (no plan); enqueued on cuda_stream; errors as the applies, FD_ERR_UNSUPPORTED also for
+ * z rows too long for the kernels' tiles (fine nz > 682 for fd_interpolate, coarse nz > 2048).
+ */
+FD_API int fd_restrict(const int32_t shape_fine[3], const int32_t bc[3], int32_t p, const double *fine,
+                double *coarse, int64_t nbands, void *cuda_stream);
+FD_API int fd_interpolate(const int32_t shape_fine[3], const int32_t bc[3], int32_t p,
+                   const double *coarse, double *fine, int64_t nbands, void *cuda_stream);
+
 /* fd_destroy -- free the plan; NULL is a no-op.  The caller must have synchronised any stream
  * still running an apply of this plan. */
 FD_API int fd_destroy(fd_plan *plan);

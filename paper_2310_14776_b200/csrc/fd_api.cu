@@ -461,6 +461,38 @@ int fd_jacobi_sweep(const fd_plan *plan, const double *phi, const double *rhs, d
                         (cudaStream_t)cuda_stream);
 }
 
+// ---- grid transfer ---------------------------------------------------------------
+
+static int transfer_call(int interp, const int32_t shape_fine[3], const int32_t bc[3], int32_t p,
+                         const double *src, double *dst, int64_t nbands, void *cuda_stream)
+{
+    if (!shape_fine || !bc || nbands < 0) return FD_ERR_INVALID;
+    if (nbands == 0) return FD_OK;
+    if (!src || !dst) return FD_ERR_INVALID;
+    if (((uintptr_t)src | (uintptr_t)dst) & 7) return FD_ERR_INVALID;
+    size_t pf = 1, pc = 1;
+    for (int d = 0; d < 3; ++d) {
+        if (shape_fine[d] < 2) return FD_ERR_INVALID;
+        pf *= (size_t)shape_fine[d];
+        pc *= (size_t)(bc[d] ? shape_fine[d] / 2 : (shape_fine[d] - 1) / 2);
+    }
+    const size_t nsrc = (interp ? pc : pf) * 8 * (size_t)nbands, ndst = (interp ? pf : pc) * 8 * (size_t)nbands;
+    if (overlaps(dst, ndst, src, nsrc)) return FD_ERR_ALIAS;
+    return fd_transfer_run(interp, shape_fine, bc, p, src, dst, nbands, (cudaStream_t)cuda_stream);
+}
+
+int fd_restrict(const int32_t shape_fine[3], const int32_t bc[3], int32_t p, const double *fine,
+                double *coarse, int64_t nbands, void *cuda_stream)
+{
+    return transfer_call(0, shape_fine, bc, p, fine, coarse, nbands, cuda_stream);
+}
+
+int fd_interpolate(const int32_t shape_fine[3], const int32_t bc[3], int32_t p, const double *coarse,
+                   double *fine, int64_t nbands, void *cuda_stream)
+{
+    return transfer_call(1, shape_fine, bc, p, coarse, fine, nbands, cuda_stream);
+}
+
 int fd_destroy(fd_plan *plan)
 {
     delete plan;

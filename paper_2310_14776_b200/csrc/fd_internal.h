@@ -114,3 +114,7 @@ int64_t fd_sweep_expect_ws_bytes(const fd_plan *plan, int64_t nbands);
 cudaError_t fd_launch_sweep(const fd_plan *plan, const FdGeom &g, int mode, const void *psi,
                             const double *second, void *out, int64_t nbands, double *eps,
                             double *norm, double *ws, cudaStream_t stream, int *nlaunches);
+// fd_transfer.cu: restriction (interp = 0) / interpolation (interp = 1) between the fine grid
+// `shape_fine` and its coarse grid; returns an fd_status value
+int fd_transfer_run(int interp, const int32_t shape_fine[3], const int32_t bc[3], int p,
+                    const double *src, double *dst, int64_t nbands, cudaStream_t stream);

@@ -1,0 +1,407 @@
+// Grid transfer between a fine grid (spacing h) and the coarse grid of spacing 2h: restriction and
+// interpolation ("interpolating from one uniform grid to another" is the second C
+// hot spot the paper lists; multigrid Poisson / preconditioner).
+// Operation and index conventions: include/fdham.h (fd_restrict / fd_interpolate), DESIGN.md
+// readings R13 (midpoint Lagrange weights b_j of order p, restriction = interpolation^T / 8) and
+// R14 (coarse point I on fine point 2I + off, off = 0 periodic / 1 zero-BC).
+//
+// Both kernels are tensor-product sweeps along x.  A CTA owns a tile of coarse y rows x the full
+// z row and a chunk of coarse x planes; every plane it brings in is staged in shared memory with
+// its z halo resolved (wrapped or zero), reduced / expanded along z and then along y by two small
+// separable passes, and combined along x in REGISTERS:
+//   restriction   -- scatter: the y-z-restricted fine plane adds r_a s to the 2p coarse planes in
+//                    flight (a shifting register queue); a coarse plane is stored when complete;
+//   interpolation -- gather: the y-z-interpolated coarse plane enters a queue of 2p planes; the
+//                    even fine plane is the plane itself, the odd one the b_j-weighted sum.
+// Each fine value therefore crosses HBM once (plus the tile / chunk halos, which hit L2).
+#include "fd_internal.h"
+
+namespace {
+
+constexpr int kThreads = 256;
+constexpr int kMaxPt = 8;   // output points of the swept plane per thread
+
+struct TGeom {
+    int nf[3], nc[3], bc[3], off[3];
+    double b[4];  // b[1..p]: midpoint Lagrange weights
+};
+
+// z index of a padded row -> source index in [0, n) or -1 (zero)
+__device__ __forceinline__ int wrap_or_zero(int i, int n, int periodic)
+{
+    if (i >= 0 && i < n) return i;
+    if (!periodic) return -1;
+    i %= n;
+    return i < 0 ? i + n : i;
+}
+
+// ---------------------------------------------------------------------------------- restriction
+// blockIdx.x: coarse y tile (jt rows), blockIdx.y: chunk of ic coarse x planes, blockIdx.z: band.
+template <int P>
+__global__ void __launch_bounds__(kThreads)
+fd_restrict_kernel(const __grid_constant__ TGeom g, const double *__restrict__ fine,
+                   double *__restrict__ coarse, int jt, int ic)
+{
+    constexpr int M = 2 * P - 1;  // reach of the 1-D restriction in fine points
+    extern __shared__ double sm[];
+    const int nzf = g.nf[2], kc = g.nc[2];
+    const int fp = nzf + 2 * M;               // padded fine row
+    const int rows = 2 * jt - 1 + 2 * M;      // fine rows staged per plane
+    double *F = sm;                           // [rows][fp]
+    double *T = sm + (size_t)rows * fp;       // [rows][kc]  z-restricted rows
+    const int tid = threadIdx.x;
+    const int J0 = blockIdx.x * jt, nj = min(jt, g.nc[1] - J0);
+    const int I0 = blockIdx.y * ic, ni = min(ic, g.nc[0] - I0);
+    const long long band = blockIdx.z;
+    const double *fb = fine + band * ((long long)g.nf[0] * g.nf[1] * nzf);
+    double *cb = coarse + band * ((long long)g.nc[0] * g.nc[1] * kc);
+    const int yf0 = 2 * J0 + g.off[1] - M;    // fine row of staged row 0
+    const int oz = g.off[2];
+    double r[P + 1];                          // 1-D restriction weights: 1/2 and b_j / 2
+    r[0] = 0.5;
+#pragma unroll
+    for (int j = 1; j <= P; ++j) r[j] = 0.5 * g.b[j];
+
+    double acc[2 * P][kMaxPt];                // coarse planes base .. base + 2P - 1 in flight
+#pragma unroll
+    for (int a = 0; a < 2 * P; ++a)
+#pragma unroll
+        for (int n = 0; n < kMaxPt; ++n) acc[a][n] = 0.0;
+    const int npts = jt * kc;
+
+    // y-z restriction of fine plane xf (already wrapped into range) into s[] for the owned points
+    auto plane = [&](int xf, double (&s)[kMaxPt]) {
+        __syncthreads();  // the previous plane's T / F are no longer read
+        const double *fpx = fb + (long long)xf * g.nf[1] * nzf;
+        for (int e = tid; e < rows * fp; e += kThreads) {
+            const int rr = e / fp, zp = e - rr * fp;
+            const int y = wrap_or_zero(yf0 + rr, g.nf[1], g.bc[1]);
+            const int z = wrap_or_zero(zp - M, nzf, g.bc[2]);
+            F[e] = (y < 0 || z < 0) ? 0.0 : __ldg(fpx + (long long)y * nzf + z);
+        }
+        __syncthreads();
+        for (int e = tid; e < rows * kc; e += kThreads) {
+            const int rr = e / kc, k = e - rr * kc;
+            const double *row = F + rr * fp + M + 2 * k + oz;
+            double t = r[0] * row[0];
+#pragma unroll
+            for (int j = 1; j <= P; ++j) t = fma(r[j], row[-(2 * j - 1)] + row[2 * j - 1], t);
+            T[e] = t;
+        }
+        __syncthreads();
+#pragma unroll
+        for (int n = 0; n < kMaxPt; ++n) {
+            const int e = tid + n * kThreads;
+            if (e < npts) {
+                const int j = e / kc, k = e - j * kc;
+                const double *col = T + (2 * j + M) * kc + k;
+                double t = r[0] * col[0];
+#pragma unroll
+                for (int q = 1; q <= P; ++q)
+                    t = fma(r[q], col[-(2 * q - 1) * kc] + col[(2 * q - 1) * kc], t);
+                s[n] = t;
+            } else {
+                s[n] = 0.0;
+            }
+        }
+    };
+
+    // iteration c: odd fine plane d = 2c + 1 (between coarse c and c + 1), then even plane d = 2c + 2
+    // (on coarse c + 1); d = fine x index - off_x.  acc[0] is coarse plane base = c + 1 - P.
+    for (int c = I0 - P; c <= I0 + ni + P - 2; ++c) {
+        double s[kMaxPt];
+        {
+            const int xf = wrap_or_zero(2 * c + 1 + g.off[0], g.nf[0], g.bc[0]);
+            if (xf >= 0) {
+                plane(xf, s);
+#pragma unroll
+                for (int j = 1; j <= P; ++j)
+#pragma unroll
+                    for (int n = 0; n < kMaxPt; ++n) {
+                        acc[P - j][n] = fma(r[j], s[n], acc[P - j][n]);          // coarse c + 1 - j
+                        acc[P + j - 1][n] = fma(r[j], s[n], acc[P + j - 1][n]);  // coarse c + j
+                    }
+            }
+        }
+        const int base = c + 1 - P;  // complete after the odd plane
+        if (base >= I0 && base < I0 + ni) {
+#pragma unroll
+            for (int n = 0; n < kMaxPt; ++n) {
+                const int e = tid + n * kThreads;
+                if (e < npts) {
+                    const int j = e / kc, k = e - j * kc;
+                    if (j < nj) __stcs(cb + ((long long)base * g.nc[1] + J0 + j) * kc + k, acc[0][n]);
+                }
+            }
+        }
+#pragma unroll
+        for (int a = 0; a + 1 < 2 * P; ++a)
+#pragma unroll
+            for (int n = 0; n < kMaxPt; ++n) acc[a][n] = acc[a + 1][n];
+#pragma unroll
+        for (int n = 0; n < kMaxPt; ++n) acc[2 * P - 1][n] = 0.0;
+        // even plane on coarse c + 1 (slot P - 1 after the shift)
+        if (c + 1 >= I0 && c + 1 < I0 + ni) {
+            const int xf = wrap_or_zero(2 * c + 2 + g.off[0], g.nf[0], g.bc[0]);
+            if (xf >= 0) {
+                plane(xf, s);
+#pragma unroll
+                for (int n = 0; n < kMaxPt; ++n) acc[P - 1][n] = fma(r[0], s[n], acc[P - 1][n]);
+            }
+        }
+    }
+}
+
+// -------------------------------------------------------------------------------- interpolation
+// blockIdx.x: coarse y tile (jt rows -> 2 jt fine rows, + the fine row below the first coarse row
+// on a zero-BC axis), blockIdx.y: chunk of ic coarse x planes, blockIdx.z: band.
+template <int P>
+__global__ void __launch_bounds__(kThreads)
+fd_interp_kernel(const __grid_constant__ TGeom g, const double *__restrict__ coarse,
+                 double *__restrict__ fine, int jt, int ic)
+{
+    extern __shared__ double sm[];
+    const int nzf = g.nf[2], kc = g.nc[2];
+    const int cp = kc + 2 * P;                // padded coarse row
+    const int rows = jt + 2 * P;              // coarse rows staged per plane: J0 - P .. J0 + jt + P - 1
+    double *C = sm;                           // [rows][cp]
+    double *T = sm + (size_t)rows * cp;       // [rows][nzf]  z-interpolated rows
+    const int tid = threadIdx.x;
+    const int J0 = blockIdx.x * jt, nj = min(jt, g.nc[1] - J0);
+    const int I0 = blockIdx.y * ic, ni = min(ic, g.nc[0] - I0);
+    const long long band = blockIdx.z;
+    const double *cb = coarse + band * ((long long)g.nc[0] * g.nc[1] * kc);
+    double *fb = fine + band * ((long long)g.nf[0] * g.nf[1] * nzf);
+    const int oy = g.off[1], oz = g.off[2], ox = g.off[0];
+    double b[P + 1];
+#pragma unroll
+    for (int j = 1; j <= P; ++j) b[j] = g.b[j];
+
+    // local fine rows l = 0 .. 2 jt: e_y = 2 J0 - 1 + l (e = fine index - off); row 0 is the midpoint
+    // below the tile's first coarse row: it belongs to this tile only at a zero-BC lower wall.
+    const int nl = 2 * jt + 1;
+    const int npts = nl * nzf;
+    const int ey_lo = (J0 == 0 && oy == 1) ? -1 : 2 * J0;
+    const int ey_hi = min(2 * (J0 + nj), g.nf[1] - oy);  // exclusive
+
+    double sq[2 * P][kMaxPt];  // y-z-interpolated coarse planes i - 2P + 1 .. i
+#pragma unroll
+    for (int a = 0; a < 2 * P; ++a)
+#pragma unroll
+        for (int n = 0; n < kMaxPt; ++n) sq[a][n] = 0.0;
+
+    auto plane = [&](int xc, double (&s)[kMaxPt]) {
+        __syncthreads();
+        const double *cpx = cb + (long long)xc * g.nc[1] * kc;
+        for (int e = tid; e < rows * cp; e += kThreads) {
+            const int rr = e / cp, zp = e - rr * cp;
+            const int y = wrap_or_zero(J0 - P + rr, g.nc[1], g.bc[1]);
+            const int z = wrap_or_zero(zp - P, kc, g.bc[2]);
+            C[e] = (y < 0 || z < 0) ? 0.0 : __ldg(cpx + (long long)y * kc + z);
+        }
+        __syncthreads();
+        for (int e = tid; e < rows * nzf; e += kThreads) {
+            const int rr = e / nzf, fz = e - rr * nzf;
+            const int ez = fz - oz;            // >= -1
+            const double *row = C + rr * cp + P;
+            double t;
+            if ((ez & 1) == 0) {
+                t = row[ez >> 1];
+            } else {
+                const int c = (ez - 1) >> 1;   // lower coarse neighbour (-1 at a zero-BC wall)
+                t = 0.0;
+#pragma unroll
+                for (int j = 1; j <= P; ++j) t = fma(b[j], row[c + 1 - j] + row[c + j], t);
+            }
+            T[e] = t;
+        }
+        __syncthreads();
+#pragma unroll
+        for (int n = 0; n < kMaxPt; ++n) {
+            const int e = tid + n * kThreads;
+            if (e < npts) {
+                const int l = e / nzf, fz = e - l * nzf;
+                const int ey = 2 * J0 - 1 + l;
+                // staged row of coarse row cy is cy - J0 + P
+                if ((ey & 1) == 0) {
+                    s[n] = T[((ey >> 1) - J0 + P) * nzf + fz];
+                } else {
+                    const int c = ((ey - 1) >> 1) - J0 + P;
+                    double t = 0.0;
+#pragma unroll
+                    for (int j = 1; j <= P; ++j)
+                        t = fma(b[j], T[(c + 1 - j) * nzf + fz] + T[(c + j) * nzf + fz], t);
+                    s[n] = t;
+                }
+            } else {
+                s[n] = 0.0;
+            }
+        }
+    };
+    auto store_plane = [&](int ex, const double (&s)[kMaxPt]) {
+        const int fx = ex + ox;
+        if (fx < 0 || fx >= g.nf[0]) return;
+#pragma unroll
+        for (int n = 0; n < kMaxPt; ++n) {
+            const int e = tid + n * kThreads;
+            if (e < npts) {
+                const int l = e / nzf, fz = e - l * nzf;
+                const int ey = 2 * J0 - 1 + l;
+                if (ey >= ey_lo && ey < ey_hi)
+                    __stcs(fb + ((long long)fx * g.nf[1] + ey + oy) * nzf + fz, s[n]);
+            }
+        }
+    };
+
+    // the chunk owns the even planes e_x = 2 i, i in [I0, I0 + ni), and the odd planes e_x = 2 c + 1,
+    // c in [c_first, I0 + ni): c_first = -1 for the first chunk on a zero-BC axis (the wall), else I0
+    const int c_first = (I0 == 0 && ox == 1) ? -1 : I0;
+    for (int i = c_first + 1 - P; i <= I0 + ni - 1 + P; ++i) {
+        double s[kMaxPt];
+        const int xc = wrap_or_zero(i, g.nc[0], g.bc[0]);
+        if (xc >= 0) {
+            plane(xc, s);
+        } else {
+#pragma unroll
+            for (int n = 0; n < kMaxPt; ++n) s[n] = 0.0;
+        }
+#pragma unroll
+        for (int a = 0; a + 1 < 2 * P; ++a)
+#pragma unroll
+            for (int n = 0; n < kMaxPt; ++n) sq[a][n] = sq[a + 1][n];
+#pragma unroll
+        for (int n = 0; n < kMaxPt; ++n) sq[2 * P - 1][n] = s[n];
+        if (i >= I0 && i < I0 + ni) store_plane(2 * i, s);
+        const int c = i - P;  // odd plane between coarse c and c + 1: sq[P - j] and sq[P + j - 1]
+        if (c >= c_first && c < I0 + ni) {
+            double o[kMaxPt];
+#pragma unroll
+            for (int n = 0; n < kMaxPt; ++n) {
+                double t = 0.0;
+#pragma unroll
+                for (int j = 1; j <= P; ++j) t = fma(b[j], sq[P - j][n] + sq[P + j - 1][n], t);
+                o[n] = t;
+            }
+            store_plane(2 * c + 1, o);
+        }
+    }
+}
+
+// midpoint Lagrange weights b_1 .. b_p (reading R13), closed form of the product
+void transfer_weights(int p, double *b)
+{
+    for (int j = 1; j <= p; ++j) {
+        const double tj = j - 0.5;
+        double w = 1.0;
+        for (int m = 1; m <= p; ++m) {
+            const double tm = m - 0.5;
+            if (m != j) w *= (-tm / (tj - tm));   // node +t_m
+            w *= (tm / (tj + tm));                // node -t_m
+        }
+        b[j] = w;
+    }
+}
+
+int fill_geom(TGeom &g, const int32_t shape_fine[3], const int32_t bc[3], int p)
+{
+    for (int d = 0; d < 3; ++d) {
+        if (bc[d] != 0 && bc[d] != 1) return -1;
+        g.nf[d] = shape_fine[d];
+        g.bc[d] = bc[d];
+        if (bc[d]) {
+            if (shape_fine[d] < 2 || (shape_fine[d] & 1)) return -1;
+            g.nc[d] = shape_fine[d] / 2;
+            g.off[d] = 0;
+        } else {
+            if (shape_fine[d] < 3 || !(shape_fine[d] & 1)) return -1;
+            g.nc[d] = (shape_fine[d] - 1) / 2;
+            g.off[d] = 1;
+        }
+    }
+    g.b[0] = 0.0;
+    transfer_weights(p, g.b);
+    return 0;
+}
+
+// coarse rows per tile and coarse planes per chunk: the swept plane's points fit kMaxPt per thread
+// and the grid has a few CTAs per SM where the problem allows it
+void tile_choice(int pts_per_row, bool interp, int ncx, int ncy, int64_t nbands, int sm_count,
+                 int *jt, int *ic)
+{
+    int t = 8;
+    while (t > 1 && (interp ? (2 * t + 1) : t) * pts_per_row > kThreads * kMaxPt) t >>= 1;
+    if (t > ncy) t = ncy;
+    const long long ytiles = (ncy + t - 1) / t;
+    long long chunks = (4LL * sm_count + ytiles * nbands - 1) / (ytiles * nbands);
+    const long long max_chunks = (ncx + 7) / 8;  // at least 8 coarse planes per chunk: halo planes
+    if (chunks > max_chunks) chunks = max_chunks;
+    if (chunks < 1) chunks = 1;
+    *jt = t;
+    *ic = (int)((ncx + chunks - 1) / chunks);
+}
+
+template <int P>
+cudaError_t launch(bool interp, const TGeom &g, const double *src, double *dst, int64_t nbands,
+                   cudaStream_t stream)
+{
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    int jt, ic;
+    tile_choice(interp ? g.nf[2] : g.nc[2], interp, g.nc[0], g.nc[1], nbands, sms, &jt, &ic);
+    if ((interp ? (2 * jt + 1) * g.nf[2] : jt * g.nc[2]) > kThreads * kMaxPt)
+        return cudaErrorInvalidConfiguration;
+    size_t smem;
+    if (interp)
+        smem = sizeof(double) * ((size_t)(jt + 2 * P) * (g.nc[2] + 2 * P) + (size_t)(jt + 2 * P) * g.nf[2]);
+    else
+        smem = sizeof(double) * (size_t)(2 * jt - 1 + 2 * (2 * P - 1)) * (g.nf[2] + 2 * (2 * P - 1) + g.nc[2]);
+    if (smem > (size_t)kFdSweepSmemMax) return cudaErrorInvalidConfiguration;
+    const void *fn = interp ? (const void *)fd_interp_kernel<P> : (const void *)fd_restrict_kernel<P>;
+    cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, kFdSweepSmemMax);
+    if (e != cudaSuccess) return e;
+    const unsigned gx = (unsigned)((g.nc[1] + jt - 1) / jt), gy = (unsigned)((g.nc[0] + ic - 1) / ic);
+    if (gy > 65535) return cudaErrorInvalidConfiguration;
+    const long long band_f = (long long)g.nf[0] * g.nf[1] * g.nf[2];
+    const long long band_c = (long long)g.nc[0] * g.nc[1] * g.nc[2];
+    for (int64_t b0 = 0; b0 < nbands; b0 += 65535) {
+        const unsigned nb = (unsigned)((nbands - b0 < 65535) ? nbands - b0 : 65535);
+        if (interp)
+            fd_interp_kernel<P><<<dim3(gx, gy, nb), kThreads, smem, stream>>>(
+                g, src + b0 * band_c, dst + b0 * band_f, jt, ic);
+        else
+            fd_restrict_kernel<P><<<dim3(gx, gy, nb), kThreads, smem, stream>>>(
+                g, src + b0 * band_f, dst + b0 * band_c, jt, ic);
+        e = cudaPeekAtLastError();
+        if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
+}
+
+}  // namespace
+
+// rc: 0 ok, -1 invalid argument, -2 unsupported, -4 CUDA
+int fd_transfer_run(int interp, const int32_t shape_fine[3], const int32_t bc[3], int p,
+                    const double *src, double *dst, int64_t nbands, cudaStream_t stream)
+{
+    TGeom g;
+    if (p < 1 || p > 3) return (p >= 1 && p <= 6) ? -2 : -1;
+    if (fill_geom(g, shape_fine, bc, p) != 0) return -1;
+    for (int d = 0; d < 3; ++d)
+        if (g.nc[d] < 1) return -1;
+    cudaError_t e;
+    switch (p) {
+    case 1: e = launch<1>(interp != 0, g, src, dst, nbands, stream); break;
+    case 2: e = launch<2>(interp != 0, g, src, dst, nbands, stream); break;
+    default: e = launch<3>(interp != 0, g, src, dst, nbands, stream); break;
+    }
+    if (e == cudaErrorInvalidConfiguration) {
+        cudaGetLastError();
+        return -2;
+    }
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return -4;
+    }
+    return 0;
+}

@@ -26,7 +26,7 @@ EXPORTED_SYMBOLS = [
     "fd_create", "fd_create_scaled", "fd_apply_kinetic", "fd_apply_hamiltonian",
     "fd_apply_hamiltonian_host", "fd_workspace_create", "fd_workspace_destroy",
     "fd_apply_hamiltonian_host_ws", "fd_expect_workspace_bytes", "fd_apply_hamiltonian_expect",
-    "fd_residual", "fd_jacobi_sweep",
+    "fd_residual", "fd_jacobi_sweep", "fd_restrict", "fd_interpolate",
     "fd_destroy", "fd_strerror", "fd_plan_set_kernel", "fd_plan_get_kernel", "fd_plan_kernel_for", "fd_plan_launches",
     "fd_plan_get_weights",
 ]
@@ -78,6 +78,10 @@ def load_library() -> ctypes.CDLL:
     lib.fd_residual.restype = ctypes.c_int
     lib.fd_jacobi_sweep.argtypes = [vp, vp, vp, vp, i64, ctypes.c_double, vp]
     lib.fd_jacobi_sweep.restype = ctypes.c_int
+    lib.fd_restrict.argtypes = [i32p, i32p, i32, vp, vp, i64, vp]
+    lib.fd_restrict.restype = ctypes.c_int
+    lib.fd_interpolate.argtypes = [i32p, i32p, i32, vp, vp, i64, vp]
+    lib.fd_interpolate.restype = ctypes.c_int
     lib.fd_destroy.argtypes = [vp]
     lib.fd_destroy.restype = ctypes.c_int
     lib.fd_strerror.argtypes = [ctypes.c_int]
@@ -238,6 +242,29 @@ def fd_jacobi_sweep(plan, phi, rhs, out, omega: float, stream=None) -> None:
     rc = load_library().fd_jacobi_sweep(plan, _dev_ptr(phi), _dev_ptr(rhs), _dev_ptr(out),
                                         int(phi.shape[0]), float(omega), _stream_ptr(stream))
     _check(rc, "fd_jacobi_sweep")
+
+
+def coarse_shape(shape_fine: Sequence[int], bc: Sequence[int]):
+    """Coarse extents of a fine grid (include/fdham.h: n/2 periodic, (n-1)/2 zero-BC)."""
+    return tuple(int(n) // 2 if b else (int(n) - 1) // 2 for n, b in zip(shape_fine, bc))
+
+
+def fd_restrict(shape_fine, bc, p: int, fine, coarse, stream=None) -> None:
+    """coarse[nbands, nc] <- fine[nbands, nf] (float64 CUDA tensors; include/fdham.h)."""
+    rc = load_library().fd_restrict((ctypes.c_int32 * 3)(*[int(s) for s in shape_fine]),
+                                    (ctypes.c_int32 * 3)(*[int(b) for b in bc]), int(p),
+                                    _dev_ptr(fine), _dev_ptr(coarse), int(fine.shape[0]),
+                                    _stream_ptr(stream))
+    _check(rc, "fd_restrict")
+
+
+def fd_interpolate(shape_fine, bc, p: int, coarse, fine, stream=None) -> None:
+    """fine[nbands, nf] <- coarse[nbands, nc] (float64 CUDA tensors; include/fdham.h)."""
+    rc = load_library().fd_interpolate((ctypes.c_int32 * 3)(*[int(s) for s in shape_fine]),
+                                       (ctypes.c_int32 * 3)(*[int(b) for b in bc]), int(p),
+                                       _dev_ptr(coarse), _dev_ptr(fine), int(coarse.shape[0]),
+                                       _stream_ptr(stream))
+    _check(rc, "fd_interpolate")
 
 
 def fd_plan_set_kernel(plan, kernel: int, param: int = 0) -> None:

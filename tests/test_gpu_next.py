@@ -320,3 +320,90 @@ def test_jacobi_rejects_complex_plans(fd):
         assert ei.value.status == -2
     finally:
         fd.fd_destroy(plan)
+
+
+# ------------------------------------------------------------------------------ f3: grid transfer
+
+def transfer_tol(p, x):
+    """row sum of |weights| of the 3-D operator times 1e-12 max|x| (interpolation: (2 sum|b_j|)^3,
+    restriction: (1/2 + sum|b_j|)^3; both <= 2.2 for p <= 3)"""
+    return 1e-12 * 2.2 * float(np.abs(x).max())
+
+
+@pytest.mark.parametrize("bc", list(itertools.product((0, 1), repeat=3)))
+@pytest.mark.parametrize("p", [1, 2, 3])
+def test_restrict_and_interpolate_all_bc_mixes(oracle, fd, bc, p):
+    """several y tiles (ragged), several x chunks, several bands"""
+    rng = np.random.default_rng(100 + p)
+    nf = tuple(n if b else n + 1 for n, b in zip((44, 36, 24), bc))
+    nc = fd.coarse_shape(nf, bc)
+    assert nc == oracle.coarse_shape(nf, bc)
+    f = rng.standard_normal((3,) + nf)
+    c = rng.standard_normal((3,) + nc)
+    d_c = torch.full((3,) + nc, float("nan"), dtype=torch.float64, device="cuda")
+    fd.fd_restrict(nf, bc, p, torch.from_numpy(f).cuda(), d_c)
+    d_f = torch.full((3,) + nf, float("nan"), dtype=torch.float64, device="cuda")
+    fd.fd_interpolate(nf, bc, p, torch.from_numpy(c).cuda(), d_f)
+    torch.cuda.synchronize()
+    got_r, got_i = d_c.cpu().numpy(), d_f.cpu().numpy()
+    assert np.isfinite(got_r).all() and np.isfinite(got_i).all()
+    assert np.max(np.abs(got_r - oracle.restrict(nf, bc, p, f))) <= transfer_tol(p, f)
+    assert np.max(np.abs(got_i - oracle.interpolate(nf, bc, p, c))) <= transfer_tol(p, c)
+    # adjointness on the device results: 8 <R f, c> = <f, I c>
+    assert abs(8.0 * np.sum(got_r * c) - np.sum(f * got_i)) <= 1e-10 * np.sqrt(f.size)
+
+
+@pytest.mark.parametrize("nf,bc", [((8, 8, 8), (1, 1, 1)), ((5, 7, 9), (0, 0, 0)), ((6, 9, 130), (1, 0, 1)),
+                                   ((20, 70, 12), (1, 1, 1)), ((3, 3, 3), (0, 0, 0)), ((2, 2, 2), (1, 1, 1))])
+def test_transfer_awkward_shapes(oracle, fd, nf, bc):
+    rng = np.random.default_rng(7)
+    nc = fd.coarse_shape(nf, bc)
+    for p in (1, 3):
+        f = rng.standard_normal((2,) + tuple(nf))
+        c = rng.standard_normal((2,) + nc)
+        d_c = torch.full((2,) + nc, float("nan"), dtype=torch.float64, device="cuda")
+        d_f = torch.full((2,) + tuple(nf), float("nan"), dtype=torch.float64, device="cuda")
+        fd.fd_restrict(nf, bc, p, torch.from_numpy(f).cuda(), d_c)
+        fd.fd_interpolate(nf, bc, p, torch.from_numpy(c).cuda(), d_f)
+        torch.cuda.synchronize()
+        assert np.max(np.abs(d_c.cpu().numpy() - oracle.restrict(nf, bc, p, f))) <= transfer_tol(p, f)
+        assert np.max(np.abs(d_f.cpu().numpy() - oracle.interpolate(nf, bc, p, c))) <= transfer_tol(p, c)
+
+
+def test_transfer_full_size_192_to_96(oracle, fd):
+    """the fine density grid of cfg3 (2 x 96 per axis) <-> cfg3's grid, the sizes the bench times;
+    guard bands around the outputs; one band in full against the oracle"""
+    nf, bc, p, nb = (192, 192, 192), (1, 1, 1), 3, 4
+    nc = fd.coarse_shape(nf, bc)
+    rng = np.random.default_rng(9)
+    f = rng.standard_normal((nb,) + nf)
+    c = rng.standard_normal((nb,) + nc)
+    pad = 4096
+    big_c = torch.full((c.size + 2 * pad,), 777.0, dtype=torch.float64, device="cuda")
+    big_f = torch.full((f.size + 2 * pad,), 777.0, dtype=torch.float64, device="cuda")
+    d_c = big_c[pad:pad + c.size].view(c.shape)
+    d_f = big_f[pad:pad + f.size].view(f.shape)
+    fd.fd_restrict(nf, bc, p, torch.from_numpy(f).cuda(), d_c)
+    fd.fd_interpolate(nf, bc, p, torch.from_numpy(c).cuda(), d_f)
+    torch.cuda.synchronize()
+    for big, n in ((big_c, c.size), (big_f, f.size)):
+        assert bool((torch.cat([big[:pad], big[pad + n:]]) == 777.0).all())
+    for b in (0, nb - 1):
+        assert np.max(np.abs(d_c[b:b + 1].cpu().numpy() - oracle.restrict(nf, bc, p, f[b:b + 1]))) \
+            <= transfer_tol(p, f)
+        assert np.max(np.abs(d_f[b:b + 1].cpu().numpy() - oracle.interpolate(nf, bc, p, c[b:b + 1]))) \
+            <= transfer_tol(p, c)
+
+
+def test_transfer_argument_errors(fd):
+    x = torch.zeros((1, 8, 8, 8), dtype=torch.float64, device="cuda")
+    y = torch.zeros((1, 4, 4, 4), dtype=torch.float64, device="cuda")
+    for nf, bc, p, status in [((8, 8, 7), (1, 1, 1), 1, -1),      # odd periodic axis
+                              ((8, 8, 8), (1, 1, 0), 1, -1),      # even zero-BC axis
+                              ((8, 8, 8), (1, 1, 1), 0, -1), ((8, 8, 8), (1, 1, 1), 4, -2)]:
+        with pytest.raises(fd.FDError) as ei:
+            fd.fd_restrict(nf, bc, p, x, y)
+        assert ei.value.status == status
+    with pytest.raises(fd.FDError) as ei:
+        fd.fd_interpolate((8, 8, 8), (1, 1, 1), 1, x.view(-1)[:64].view(1, 4, 4, 4), x)
+    assert ei.value.status == -3
