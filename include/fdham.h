@@ -203,6 +203,54 @@ FD_API int fd_restrict(const int32_t shape_fine[3], const int32_t bc[3], int32_t
 FD_API int fd_interpolate(const int32_t shape_fine[3], const int32_t bc[3], int32_t p,
                    const double *coarse, double *fine, int64_t nbands, void *cuda_stream);
 
+/*
+ * the PAW non-local term: third term of the PAW Hamiltonian, Eq. 6
+ * "sum_a sum_ii' |p~^a_i> Delta H^a_ii' <p~^a_i'|", and with Delta S the overlap
+ * operator S~ = 1 + sum |p~> Delta S <p~| of Eq. 7; "overlaps between projector
+ * functions and wave functions" is the third C hot spot the paper lists.
+ *
+ *     P_b[a,i]  = dv sum_{r in box_a} p~^a_i(r) psi^_b(r),        dv = h_x h_y h_z
+ *     out_b(r') += conj(phase(r)) sum_{i,i'} p~^a_i(r) dO^a_ii' P_b[a,i']   for every atom a
+ *
+ * PAW data sets are not available here, so the library takes whatever localised functions the
+ * caller supplies (synthetic in tests and bench).  Atom a owns a box of box_size[a]
+ * grid points starting at index box_start[a] (may be negative / past the end); p~^a_i is a real
+ * array over the box, [n_i][sx][sy][sz]; dO^a a real n_i x n_i matrix.  A box point outside [0,n)
+ * on a periodic axis stands for its home-cell image and carries the Bloch factor of psi^ (as in
+ * the stencil) when read and its conjugate when written; on a zero-BC axis it is dropped.
+ *
+ * fd_paw_create -- copy the projector data to the plan's device, resolve the boxes into index
+ *   tables, colour the atoms so that boxes handled together are disjoint (results do not depend on
+ *   scheduling; no atomics).  All array arguments are HOST pointers: box_start, box_size
+ *   [natoms][3], nproj [natoms] (1..32 each), proj (concatenated per atom), dh / ds (concatenated
+ *   [n_i][n_i] per atom; either may be NULL).  FD_ERR_UNSUPPORTED: a box longer than a periodic
+ *   axis, more than 32 functions on an atom, grids of 2^31 points or more.
+ * fd_paw_nproj_total -- sum_a n_i (row length of P), or a negative fd_status.
+ * fd_paw_project   -- coef[nbands][sum n_i] = P (plan dtype; device pointer, 16-byte aligned).
+ * fd_paw_add_nonlocal -- out += sum |p~> Delta H <p~|psi>  (coef: scratch of the same size as P;
+ *   it holds P on return).
+ * fd_apply_hamiltonian_paw -- out = -1/2 lap_FD psi + v_eff psi + the Delta H term: the complete
+ *   H~ psi~ of Eq. 6 (v_eff == NULL: kinetic + non-local).
+ * fd_apply_overlap -- out = psi + sum |p~> Delta S <p~|psi>  (Eq. 7).
+ * Errors as fd_apply_hamiltonian; FD_ERR_INVALID also when paw does not belong to a plan of the
+ * same grid, dtype and device, or the matrix the call needs was not given at fd_paw_create.
+ */
+typedef struct fd_paw fd_paw;
+FD_API int fd_paw_create(fd_paw **paw, const fd_plan *plan, int32_t natoms, const int32_t *box_start,
+                  const int32_t *box_size, const int32_t *nproj, const double *proj_host,
+                  const double *dh_host, const double *ds_host);
+FD_API int fd_paw_destroy(fd_paw *paw);
+FD_API int32_t fd_paw_nproj_total(const fd_paw *paw);
+FD_API int fd_paw_project(const fd_plan *plan, const fd_paw *paw, const void *psi, void *coef,
+                   int64_t nbands, void *cuda_stream);
+FD_API int fd_paw_add_nonlocal(const fd_plan *plan, const fd_paw *paw, const void *psi, void *out,
+                        void *coef, int64_t nbands, void *cuda_stream);
+FD_API int fd_apply_hamiltonian_paw(const fd_plan *plan, const fd_paw *paw, const void *psi,
+                             const double *v_eff, void *out, void *coef, int64_t nbands,
+                             void *cuda_stream);
+FD_API int fd_apply_overlap(const fd_plan *plan, const fd_paw *paw, const void *psi, void *out,
+                     void *coef, int64_t nbands, void *cuda_stream);
+
 /* fd_destroy -- free the plan; NULL is a no-op.  The caller must have synchronised any stream
  * still running an apply of this plan. */
 FD_API int fd_destroy(fd_plan *plan);

@@ -493,6 +493,109 @@ int fd_interpolate(const int32_t shape_fine[3], const int32_t bc[3], int32_t p, 
     return transfer_call(1, shape_fine, bc, p, coarse, fine, nbands, cuda_stream);
 }
 
+// ---- PAW non-local term ----------------------------------------------------------
+
+int fd_paw_create(fd_paw **paw, const fd_plan *plan, int32_t natoms, const int32_t *box_start,
+                  const int32_t *box_size, const int32_t *nproj, const double *proj_host,
+                  const double *dh_host, const double *ds_host)
+{
+    if (!paw || !plan || natoms < 0) return FD_ERR_INVALID;
+    if (natoms > 0 && (!box_start || !box_size || !nproj || !proj_host)) return FD_ERR_INVALID;
+    if (!dh_host && !ds_host && natoms > 0) return FD_ERR_INVALID;
+    const int drc = check_device(plan);
+    if (drc != FD_OK) return drc;
+    return fd_paw_build(paw, plan, natoms, box_start, box_size, nproj, proj_host, dh_host, ds_host);
+}
+
+int fd_paw_destroy(fd_paw *paw)
+{
+    fd_paw_free(paw);
+    return FD_OK;
+}
+
+int32_t fd_paw_nproj_total(const fd_paw *paw) { return paw ? fd_paw_ntot(paw) : FD_ERR_INVALID; }
+
+static int paw_args(const fd_plan *plan, const fd_paw *paw, const void *psi, const void *coef,
+                    int64_t nbands)
+{
+    if (!plan || !paw || nbands < 0) return FD_ERR_INVALID;
+    if (!fd_paw_matches(paw, plan)) return FD_ERR_INVALID;
+    if (nbands == 0) return FD_OK;
+    if (!psi || !coef) return FD_ERR_INVALID;
+    if (((uintptr_t)psi | (uintptr_t)coef) & 15) return FD_ERR_INVALID;
+    return check_device(plan);
+}
+
+static int paw_finish(const fd_plan *plan, cudaError_t e, int n)
+{
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return FD_ERR_CUDA;
+    }
+    __atomic_add_fetch(&const_cast<fd_plan *>(plan)->launches, (long long)n, __ATOMIC_RELAXED);
+    return FD_OK;
+}
+
+int fd_paw_project(const fd_plan *plan, const fd_paw *paw, const void *psi, void *coef,
+                   int64_t nbands, void *cuda_stream)
+{
+    const int rc = paw_args(plan, paw, psi, coef, nbands);
+    if (rc != FD_OK || nbands == 0) return rc;
+    int n = 0;
+    return paw_finish(plan, fd_paw_launch_project(paw, psi, coef, nbands, (cudaStream_t)cuda_stream, &n), n);
+}
+
+// out += sum |p~> dO <p~|psi>, which: 0 = Delta H, 1 = Delta S
+static int paw_add(const fd_plan *plan, const fd_paw *paw, int which, const void *psi, void *out,
+                   void *coef, int64_t nbands, cudaStream_t stream)
+{
+    if (!fd_paw_has(paw, which)) return FD_ERR_INVALID;
+    int n = 0;
+    cudaError_t e = fd_paw_launch_project(paw, psi, coef, nbands, stream, &n);
+    if (e == cudaSuccess) e = fd_paw_launch_add(paw, which, coef, out, nbands, stream, &n);
+    return paw_finish(plan, e, n);
+}
+
+int fd_paw_add_nonlocal(const fd_plan *plan, const fd_paw *paw, const void *psi, void *out, void *coef,
+                        int64_t nbands, void *cuda_stream)
+{
+    int rc = paw_args(plan, paw, psi, coef, nbands);
+    if (rc != FD_OK || nbands == 0) return rc;
+    rc = check_apply_args(plan, psi, nullptr, false, out, nbands);
+    if (rc != FD_OK) return rc;
+    return paw_add(plan, paw, 0, psi, out, coef, nbands, (cudaStream_t)cuda_stream);
+}
+
+int fd_apply_hamiltonian_paw(const fd_plan *plan, const fd_paw *paw, const void *psi,
+                             const double *v_eff, void *out, void *coef, int64_t nbands,
+                             void *cuda_stream)
+{
+    int rc = paw_args(plan, paw, psi, coef, nbands);
+    if (rc != FD_OK || nbands == 0) return rc;
+    rc = check_apply_args(plan, psi, v_eff, false, out, nbands);
+    if (rc != FD_OK) return rc;
+    rc = apply_device(plan, plan->g, v_eff ? 1 : 0, psi, v_eff, out, nbands, nullptr, nullptr, nullptr,
+                      (cudaStream_t)cuda_stream);
+    if (rc != FD_OK) return rc;
+    return paw_add(plan, paw, 0, psi, out, coef, nbands, (cudaStream_t)cuda_stream);
+}
+
+int fd_apply_overlap(const fd_plan *plan, const fd_paw *paw, const void *psi, void *out, void *coef,
+                     int64_t nbands, void *cuda_stream)
+{
+    int rc = paw_args(plan, paw, psi, coef, nbands);
+    if (rc != FD_OK || nbands == 0) return rc;
+    rc = check_apply_args(plan, psi, nullptr, false, out, nbands);
+    if (rc != FD_OK) return rc;
+    const size_t nb = (size_t)plan->g.n[0] * plan->g.n[1] * plan->g.n[2] * (size_t)nbands *
+                      (plan->g.cplx ? 16 : 8);
+    if (cudaMemcpyAsync(out, psi, nb, cudaMemcpyDeviceToDevice, (cudaStream_t)cuda_stream) != cudaSuccess) {
+        cudaGetLastError();
+        return FD_ERR_CUDA;
+    }
+    return paw_add(plan, paw, 1, psi, out, coef, nbands, (cudaStream_t)cuda_stream);
+}
+
 int fd_destroy(fd_plan *plan)
 {
     delete plan;

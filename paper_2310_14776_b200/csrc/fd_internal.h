@@ -118,3 +118,16 @@ cudaError_t fd_launch_sweep(const fd_plan *plan, const FdGeom &g, int mode, cons
 // `shape_fine` and its coarse grid; returns an fd_status value
 int fd_transfer_run(int interp, const int32_t shape_fine[3], const int32_t bc[3], int p,
                     const double *src, double *dst, int64_t nbands, cudaStream_t stream);
+// fd_paw.cu: PAW non-local term
+struct fd_paw;
+int fd_paw_build(fd_paw **out, const fd_plan *plan, int natoms, const int32_t *box_start,
+                 const int32_t *box_size, const int32_t *nproj, const double *proj_host,
+                 const double *dh_host, const double *ds_host);  // returns an fd_status value
+void fd_paw_free(fd_paw *w);
+int fd_paw_ntot(const fd_paw *w);
+int fd_paw_has(const fd_paw *w, int which);            // which: 0 = Delta H, 1 = Delta S
+int fd_paw_matches(const fd_paw *w, const fd_plan *plan);
+cudaError_t fd_paw_launch_project(const fd_paw *w, const void *psi, void *coef, int64_t nbands,
+                                  cudaStream_t stream, int *nlaunches);
+cudaError_t fd_paw_launch_add(const fd_paw *w, int which, const void *coef, void *out, int64_t nbands,
+                              cudaStream_t stream, int *nlaunches);

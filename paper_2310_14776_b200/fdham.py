@@ -27,6 +27,8 @@ EXPORTED_SYMBOLS = [
     "fd_apply_hamiltonian_host", "fd_workspace_create", "fd_workspace_destroy",
     "fd_apply_hamiltonian_host_ws", "fd_expect_workspace_bytes", "fd_apply_hamiltonian_expect",
     "fd_residual", "fd_jacobi_sweep", "fd_restrict", "fd_interpolate",
+    "fd_paw_create", "fd_paw_destroy", "fd_paw_nproj_total", "fd_paw_project", "fd_paw_add_nonlocal",
+    "fd_apply_hamiltonian_paw", "fd_apply_overlap",
     "fd_destroy", "fd_strerror", "fd_plan_set_kernel", "fd_plan_get_kernel", "fd_plan_kernel_for", "fd_plan_launches",
     "fd_plan_get_weights",
 ]
@@ -82,6 +84,20 @@ def load_library() -> ctypes.CDLL:
     lib.fd_restrict.restype = ctypes.c_int
     lib.fd_interpolate.argtypes = [i32p, i32p, i32, vp, vp, i64, vp]
     lib.fd_interpolate.restype = ctypes.c_int
+    lib.fd_paw_create.argtypes = [ctypes.POINTER(vp), vp, i32, i32p, i32p, i32p, f64p, f64p, f64p]
+    lib.fd_paw_create.restype = ctypes.c_int
+    lib.fd_paw_destroy.argtypes = [vp]
+    lib.fd_paw_destroy.restype = ctypes.c_int
+    lib.fd_paw_nproj_total.argtypes = [vp]
+    lib.fd_paw_nproj_total.restype = ctypes.c_int32
+    lib.fd_paw_project.argtypes = [vp, vp, vp, vp, i64, vp]
+    lib.fd_paw_project.restype = ctypes.c_int
+    lib.fd_paw_add_nonlocal.argtypes = [vp, vp, vp, vp, vp, i64, vp]
+    lib.fd_paw_add_nonlocal.restype = ctypes.c_int
+    lib.fd_apply_hamiltonian_paw.argtypes = [vp, vp, vp, vp, vp, vp, i64, vp]
+    lib.fd_apply_hamiltonian_paw.restype = ctypes.c_int
+    lib.fd_apply_overlap.argtypes = [vp, vp, vp, vp, vp, i64, vp]
+    lib.fd_apply_overlap.restype = ctypes.c_int
     lib.fd_destroy.argtypes = [vp]
     lib.fd_destroy.restype = ctypes.c_int
     lib.fd_strerror.argtypes = [ctypes.c_int]
@@ -265,6 +281,72 @@ def fd_interpolate(shape_fine, bc, p: int, coarse, fine, stream=None) -> None:
                                        _dev_ptr(coarse), _dev_ptr(fine), int(coarse.shape[0]),
                                        _stream_ptr(stream))
     _check(rc, "fd_interpolate")
+
+
+def fd_paw_create(plan, box_start, box_size, nproj, proj, dh=None, ds=None) -> ctypes.c_void_p:
+    """Projector set on the plan's device (include/fdham.h: fd_paw_create); arguments are host
+    arrays (numpy / sequences): box_start, box_size [natoms,3], nproj [natoms], proj and dh / ds
+    concatenated per atom."""
+    import numpy as np
+    bs = np.ascontiguousarray(box_start, dtype=np.int32).reshape(-1, 3)
+    bz = np.ascontiguousarray(box_size, dtype=np.int32).reshape(-1, 3)
+    npj = np.ascontiguousarray(nproj, dtype=np.int32).reshape(-1)
+    pr = np.ascontiguousarray(proj, dtype=np.float64).reshape(-1)
+    i32p, f64p = ctypes.POINTER(ctypes.c_int32), ctypes.POINTER(ctypes.c_double)
+
+    def mat(m):
+        if m is None:
+            return None, None
+        a = np.ascontiguousarray(m, dtype=np.float64).reshape(-1)
+        return a, a.ctypes.data_as(f64p)
+    dh_a, dh_p = mat(dh)
+    ds_a, ds_p = mat(ds)
+    paw = ctypes.c_void_p()
+    rc = load_library().fd_paw_create(ctypes.byref(paw), plan, int(npj.shape[0]),
+                                      bs.ctypes.data_as(i32p), bz.ctypes.data_as(i32p),
+                                      npj.ctypes.data_as(i32p), pr.ctypes.data_as(f64p), dh_p, ds_p)
+    _check(rc, "fd_paw_create")
+    return paw
+
+
+def fd_paw_destroy(paw) -> None:
+    _check(load_library().fd_paw_destroy(paw), "fd_paw_destroy")
+
+
+def fd_paw_nproj_total(paw) -> int:
+    n = int(load_library().fd_paw_nproj_total(paw))
+    if n < 0:
+        raise FDError(n, "fd_paw_nproj_total")
+    return n
+
+
+def fd_paw_project(plan, paw, psi, coef, stream=None) -> None:
+    """coef[nbands, sum n_i] = dv <p~|psi> (dtype of psi)."""
+    rc = load_library().fd_paw_project(plan, paw, _dev_ptr(psi), _dev_ptr(coef), int(psi.shape[0]),
+                                       _stream_ptr(stream))
+    _check(rc, "fd_paw_project")
+
+
+def fd_paw_add_nonlocal(plan, paw, psi, out, coef, stream=None) -> None:
+    """out += sum |p~> Delta H <p~|psi>; coef is scratch [nbands, sum n_i]."""
+    rc = load_library().fd_paw_add_nonlocal(plan, paw, _dev_ptr(psi), _dev_ptr(out), _dev_ptr(coef),
+                                            int(psi.shape[0]), _stream_ptr(stream))
+    _check(rc, "fd_paw_add_nonlocal")
+
+
+def fd_apply_hamiltonian_paw(plan, paw, psi, v_eff, out, coef, stream=None) -> None:
+    """out = -1/2 lap psi + v_eff psi + sum |p~> Delta H <p~|psi> (Eq. 6 complete)."""
+    rc = load_library().fd_apply_hamiltonian_paw(
+        plan, paw, _dev_ptr(psi), _dev_ptr(v_eff) if v_eff is not None else ctypes.c_void_p(0),
+        _dev_ptr(out), _dev_ptr(coef), int(psi.shape[0]), _stream_ptr(stream))
+    _check(rc, "fd_apply_hamiltonian_paw")
+
+
+def fd_apply_overlap(plan, paw, psi, out, coef, stream=None) -> None:
+    """out = psi + sum |p~> Delta S <p~|psi> (Eq. 7)."""
+    rc = load_library().fd_apply_overlap(plan, paw, _dev_ptr(psi), _dev_ptr(out), _dev_ptr(coef),
+                                         int(psi.shape[0]), _stream_ptr(stream))
+    _check(rc, "fd_apply_overlap")
 
 
 def fd_plan_set_kernel(plan, kernel: int, param: int = 0) -> None:

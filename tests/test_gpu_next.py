@@ -407,3 +407,121 @@ def test_transfer_argument_errors(fd):
     with pytest.raises(fd.FDError) as ei:
         fd.fd_interpolate((8, 8, 8), (1, 1, 1), 1, x.view(-1)[:64].view(1, 4, 4, 4), x)
     assert ei.value.status == -3
+
+
+# ------------------------------------------------------------------------------ f4: PAW non-local term
+
+def paw_tol(cfg, paw, psi, dmat):
+    """|d| <= 1e-12 * (sum over an output point's atoms of sum_ii' |p_i| |dO_ii'| * dv sum_r |p_i'| |psi|):
+    bounded with maxima; the projections carry ~npts rounding errors each."""
+    dv = float(np.prod(cfg.h))
+    pmax = float(np.abs(paw.proj).max())
+    npts = int(np.prod(paw.box_size, axis=1).max())
+    ni = int(paw.nproj.max())
+    return 1e-12 * paw.natoms * ni * ni * pmax * pmax * float(np.abs(dmat).max()) * dv * npts * \
+        float(np.abs(psi).max())
+
+
+@pytest.mark.parametrize("bc,cplx", [((1, 1, 1), False), ((1, 1, 1), True), ((1, 0, 1), True),
+                                     ((0, 0, 0), False), ((1, 1, 0), False), ((0, 1, 1), True)])
+def test_paw_nonlocal_term_overlap_and_full_hamiltonian(oracle, fd, bc, cplx):
+    k = tuple(kk if b else 0.0 for kk, b in zip((0.25, 0.125, -0.3), bc)) if cplx else (0, 0, 0)
+    cfg = W.custom((20, 18, 24), (0.2, 0.22, 0.18), bc, k=k, complex_=cplx, nbands=7)
+    paw = W.make_paw(cfg, 12, nproj=5)        # 12 atoms in a small cell: boxes overlap, several colours
+    ds = W.make_paw(W.custom(cfg.shape, cfg.h_angstrom, bc, k=k, complex_=cplx, nbands=7, index=3),
+                    12, nproj=5).dmat * 0.1
+    psi, v = W.make_psi(cfg), W.make_veff(cfg)
+    kk = k if cplx else None
+    tdt = torch.complex128 if cplx else torch.float64
+    plan = fd.fd_create(cfg.shape, cfg.h, 3, bc, kk, fd.FD_C128 if cplx else fd.FD_F64, 0)
+    pw = fd.fd_paw_create(plan, paw.box_start, paw.box_size, paw.nproj, paw.proj, paw.dmat, ds)
+    try:
+        assert fd.fd_paw_nproj_total(pw) == paw.ntot
+        d_psi = torch.from_numpy(psi).cuda()
+        coef = torch.full((7, paw.ntot), float("nan"), dtype=tdt, device="cuda")
+        want_nl, want_c = oracle.paw_apply(cfg.shape, cfg.h, bc, kk, psi, paw.box_start, paw.box_size,
+                                           paw.nproj, paw.proj, paw.dmat, want_coef=True)
+        tol = paw_tol(cfg, paw, psi, paw.dmat)
+        # projections
+        fd.fd_paw_project(plan, pw, d_psi, coef)
+        torch.cuda.synchronize()
+        assert np.max(np.abs(coef.cpu().numpy() - want_c)) <= 1e-12 * np.prod(cfg.h) * \
+            np.prod(paw.box_size, axis=1).max() * np.abs(paw.proj).max() * np.abs(psi).max()
+        # non-local term added to an existing array
+        base = W.make_psi(W.custom(cfg.shape, cfg.h_angstrom, bc, k=k, complex_=cplx, nbands=7, index=8))
+        d_out = torch.from_numpy(base).cuda()
+        fd.fd_paw_add_nonlocal(plan, pw, d_psi, d_out, coef)
+        torch.cuda.synchronize()
+        assert np.max(np.abs(d_out.cpu().numpy() - (base + want_nl))) <= tol + 1e-15 * np.abs(base).max()
+        # full H~ psi~ (Eq. 6) and S~ psi~ (Eq. 7)
+        want_h = oracle.apply(cfg.shape, cfg.h, 3, bc, kk, psi, v) + want_nl
+        d_out = torch.full_like(d_psi, float("nan"))
+        fd.fd_apply_hamiltonian_paw(plan, pw, d_psi, torch.from_numpy(v).cuda(), d_out, coef)
+        torch.cuda.synchronize()
+        assert np.max(np.abs(d_out.cpu().numpy() - want_h)) <= tol + parity_tol(cfg.h, 3, psi, v)
+        want_s = oracle.paw_apply(cfg.shape, cfg.h, bc, kk, psi, paw.box_start, paw.box_size, paw.nproj,
+                                  paw.proj, ds, out=psi)
+        d_out = torch.full_like(d_psi, float("nan"))
+        fd.fd_apply_overlap(plan, pw, d_psi, d_out, coef)
+        torch.cuda.synchronize()
+        assert np.max(np.abs(d_out.cpu().numpy() - want_s)) <= paw_tol(cfg, paw, psi, ds) + 1e-15 * np.abs(psi).max()
+        # deterministic: same bits on a second call
+        d_out2 = torch.full_like(d_psi, float("nan"))
+        fd.fd_apply_overlap(plan, pw, d_psi, d_out2, coef)
+        torch.cuda.synchronize()
+        assert torch.equal(torch.view_as_real(d_out) if cplx else d_out,
+                           torch.view_as_real(d_out2) if cplx else d_out2)
+    finally:
+        fd.fd_paw_destroy(pw)
+        fd.fd_destroy(plan)
+
+
+def test_paw_full_size_grid_sampled_bands(oracle, fd):
+    """cfg3's grid, 64 atoms x up to 13 functions, 32 bands: the configuration the bench times;
+    two whole bands against the oracle"""
+    cfg = W.get(3).with_bands(32)
+    paw = W.make_paw(cfg, 64, nproj=13, radius_angstrom=1.1)
+    psi = W.make_psi(cfg)
+    plan = fd.fd_create(cfg.shape, cfg.h, 3, cfg.bc)
+    pw = fd.fd_paw_create(plan, paw.box_start, paw.box_size, paw.nproj, paw.proj, paw.dmat, None)
+    try:
+        d_psi = torch.from_numpy(psi).cuda()
+        d_out = torch.zeros_like(d_psi)
+        coef = torch.empty((32, paw.ntot), dtype=torch.float64, device="cuda")
+        fd.fd_paw_add_nonlocal(plan, pw, d_psi, d_out, coef)
+        torch.cuda.synchronize()
+        got = d_out.cpu().numpy()
+        for b in (0, 31):
+            want = oracle.paw_apply(cfg.shape, cfg.h, cfg.bc, None, psi[b:b + 1], paw.box_start,
+                                    paw.box_size, paw.nproj, paw.proj, paw.dmat)
+            assert np.max(np.abs(got[b:b + 1] - want)) <= paw_tol(cfg, paw, psi, paw.dmat)
+        with pytest.raises(fd.FDError) as ei:                      # Delta S was not given
+            fd.fd_apply_overlap(plan, pw, d_psi, d_out, coef)
+        assert ei.value.status == -1
+    finally:
+        fd.fd_paw_destroy(pw)
+        fd.fd_destroy(plan)
+
+
+def test_paw_create_errors(fd):
+    plan = fd.fd_create((8, 8, 8), (0.4,) * 3)
+    try:
+        with pytest.raises(fd.FDError) as ei:                      # box longer than a periodic axis
+            fd.fd_paw_create(plan, [[0, 0, 0]], [[9, 2, 2]], [1], np.zeros(36), np.zeros(1))
+        assert ei.value.status == -2
+        with pytest.raises(fd.FDError) as ei:                      # no matrix at all
+            fd.fd_paw_create(plan, [[0, 0, 0]], [[2, 2, 2]], [1], np.zeros(8), None, None)
+        assert ei.value.status == -1
+        other = fd.fd_create((8, 8, 10), (0.4,) * 3)
+        pw = fd.fd_paw_create(plan, [[0, 0, 0]], [[2, 2, 2]], [1], np.ones(8), np.ones(1))
+        try:
+            x = torch.zeros((1, 8, 8, 10), dtype=torch.float64, device="cuda")
+            c = torch.zeros((1, 2), dtype=torch.float64, device="cuda")
+            with pytest.raises(fd.FDError) as ei:                  # paw of another grid
+                fd.fd_paw_project(other, pw, x, c)
+            assert ei.value.status == -1
+        finally:
+            fd.fd_paw_destroy(pw)
+            fd.fd_destroy(other)
+    finally:
+        fd.fd_destroy(plan)
