@@ -18,7 +18,7 @@
 
 namespace {
 
-constexpr int kThreads = 256;
+constexpr int kThreads = 512;
 constexpr int kMaxPt = 8;   // output points of the swept plane per thread
 
 struct TGeom {
@@ -35,9 +35,35 @@ __device__ __forceinline__ int wrap_or_zero(int i, int n, int periodic)
     return i < 0 ? i + n : i;
 }
 
+// Stage `rows` rows of a plane in shared memory, z halo resolved: dst[rr][0 .. n + 2 pad), source row
+// index y0 + rr and z index zp - pad, both wrapped (periodic) or zero.  One warp per row, lanes
+// along z: coalesced, no division.
+__device__ __forceinline__ void stage_rows(double *dst, const double *__restrict__ plane, int rows,
+                                           int y0, int ny, int per_y, int n, int pad, int per_z)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int pitch = n + 2 * pad;
+    for (int rr = warp; rr < rows; rr += kThreads / 32) {
+        const int y = wrap_or_zero(y0 + rr, ny, per_y);
+        double *d = dst + rr * pitch;
+        if (y < 0) {
+            for (int z = lane; z < pitch; z += 32) d[z] = 0.0;
+            continue;
+        }
+        const double *srow = plane + (long long)y * n;
+        for (int z = lane; z < n; z += 32) d[pad + z] = __ldg(srow + z);
+        if (lane < 2 * pad) {  // pad <= 5: one lane per halo word
+            const int zp = (lane < pad) ? lane : n + lane;          // padded index
+            const int z = wrap_or_zero(zp - pad, n, per_z);
+            d[zp] = z < 0 ? 0.0 : __ldg(srow + z);
+        }
+    }
+}
+
 // ---------------------------------------------------------------------------------- restriction
 // blockIdx.x: coarse y tile (jt rows), blockIdx.y: chunk of ic coarse x planes, blockIdx.z: band.
-template <int P>
+// NPT: coarse points of the swept plane per thread (point e = tid + n * kThreads of the jt x kc tile).
+template <int P, int NPT>
 __global__ void __launch_bounds__(kThreads)
 fd_restrict_kernel(const __grid_constant__ TGeom g, const double *__restrict__ fine,
                    double *__restrict__ coarse, int jt, int ic)
@@ -49,7 +75,7 @@ fd_restrict_kernel(const __grid_constant__ TGeom g, const double *__restrict__ f
     const int rows = 2 * jt - 1 + 2 * M;      // fine rows staged per plane
     double *F = sm;                           // [rows][fp]
     double *T = sm + (size_t)rows * fp;       // [rows][kc]  z-restricted rows
-    const int tid = threadIdx.x;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int J0 = blockIdx.x * jt, nj = min(jt, g.nc[1] - J0);
     const int I0 = blockIdx.y * ic, ni = min(ic, g.nc[0] - I0);
     const long long band = blockIdx.z;
@@ -62,54 +88,53 @@ fd_restrict_kernel(const __grid_constant__ TGeom g, const double *__restrict__ f
 #pragma unroll
     for (int j = 1; j <= P; ++j) r[j] = 0.5 * g.b[j];
 
-    double acc[2 * P][kMaxPt];                // coarse planes base .. base + 2P - 1 in flight
+    // this thread's points: offset of the centre row in T, offset in a coarse plane (-1: none)
+    int toff[NPT], coff[NPT];
+#pragma unroll
+    for (int n = 0; n < NPT; ++n) {
+        const int e = tid + n * kThreads;
+        const int j = e / kc, k = e - j * kc;
+        const bool in_tile = e < jt * kc;
+        toff[n] = in_tile ? (2 * j + M) * kc + k : M * kc;
+        coff[n] = (in_tile && j < nj) ? (J0 + j) * kc + k : -1;
+    }
+    double acc[2 * P][NPT];                   // coarse planes base .. base + 2P - 1 in flight
 #pragma unroll
     for (int a = 0; a < 2 * P; ++a)
 #pragma unroll
-        for (int n = 0; n < kMaxPt; ++n) acc[a][n] = 0.0;
-    const int npts = jt * kc;
+        for (int n = 0; n < NPT; ++n) acc[a][n] = 0.0;
 
     // y-z restriction of fine plane xf (already wrapped into range) into s[] for the owned points
-    auto plane = [&](int xf, double (&s)[kMaxPt]) {
+    auto plane = [&](int xf, double (&s)[NPT]) {
         __syncthreads();  // the previous plane's T / F are no longer read
-        const double *fpx = fb + (long long)xf * g.nf[1] * nzf;
-        for (int e = tid; e < rows * fp; e += kThreads) {
-            const int rr = e / fp, zp = e - rr * fp;
-            const int y = wrap_or_zero(yf0 + rr, g.nf[1], g.bc[1]);
-            const int z = wrap_or_zero(zp - M, nzf, g.bc[2]);
-            F[e] = (y < 0 || z < 0) ? 0.0 : __ldg(fpx + (long long)y * nzf + z);
-        }
+        stage_rows(F, fb + (long long)xf * g.nf[1] * nzf, rows, yf0, g.nf[1], g.bc[1], nzf, M, g.bc[2]);
         __syncthreads();
-        for (int e = tid; e < rows * kc; e += kThreads) {
-            const int rr = e / kc, k = e - rr * kc;
-            const double *row = F + rr * fp + M + 2 * k + oz;
-            double t = r[0] * row[0];
+        for (int rr = warp; rr < rows; rr += kThreads / 32) {
+            const double *row = F + rr * fp + M + oz;
+            for (int k = lane; k < kc; k += 32) {
+                double t = r[0] * row[2 * k];
 #pragma unroll
-            for (int j = 1; j <= P; ++j) t = fma(r[j], row[-(2 * j - 1)] + row[2 * j - 1], t);
-            T[e] = t;
-        }
-        __syncthreads();
-#pragma unroll
-        for (int n = 0; n < kMaxPt; ++n) {
-            const int e = tid + n * kThreads;
-            if (e < npts) {
-                const int j = e / kc, k = e - j * kc;
-                const double *col = T + (2 * j + M) * kc + k;
-                double t = r[0] * col[0];
-#pragma unroll
-                for (int q = 1; q <= P; ++q)
-                    t = fma(r[q], col[-(2 * q - 1) * kc] + col[(2 * q - 1) * kc], t);
-                s[n] = t;
-            } else {
-                s[n] = 0.0;
+                for (int j = 1; j <= P; ++j)
+                    t = fma(r[j], row[2 * k - (2 * j - 1)] + row[2 * k + (2 * j - 1)], t);
+                T[rr * kc + k] = t;
             }
+        }
+        __syncthreads();
+#pragma unroll
+        for (int n = 0; n < NPT; ++n) {
+            const double *col = T + toff[n];
+            double t = r[0] * col[0];
+#pragma unroll
+            for (int q = 1; q <= P; ++q)
+                t = fma(r[q], col[-(2 * q - 1) * kc] + col[(2 * q - 1) * kc], t);
+            s[n] = t;
         }
     };
 
     // iteration c: odd fine plane d = 2c + 1 (between coarse c and c + 1), then even plane d = 2c + 2
     // (on coarse c + 1); d = fine x index - off_x.  acc[0] is coarse plane base = c + 1 - P.
     for (int c = I0 - P; c <= I0 + ni + P - 2; ++c) {
-        double s[kMaxPt];
+        double s[NPT];
         {
             const int xf = wrap_or_zero(2 * c + 1 + g.off[0], g.nf[0], g.bc[0]);
             if (xf >= 0) {
@@ -117,7 +142,7 @@ fd_restrict_kernel(const __grid_constant__ TGeom g, const double *__restrict__ f
 #pragma unroll
                 for (int j = 1; j <= P; ++j)
 #pragma unroll
-                    for (int n = 0; n < kMaxPt; ++n) {
+                    for (int n = 0; n < NPT; ++n) {
                         acc[P - j][n] = fma(r[j], s[n], acc[P - j][n]);          // coarse c + 1 - j
                         acc[P + j - 1][n] = fma(r[j], s[n], acc[P + j - 1][n]);  // coarse c + j
                     }
@@ -125,28 +150,24 @@ fd_restrict_kernel(const __grid_constant__ TGeom g, const double *__restrict__ f
         }
         const int base = c + 1 - P;  // complete after the odd plane
         if (base >= I0 && base < I0 + ni) {
+            double *cp = cb + (long long)base * g.nc[1] * kc;
 #pragma unroll
-            for (int n = 0; n < kMaxPt; ++n) {
-                const int e = tid + n * kThreads;
-                if (e < npts) {
-                    const int j = e / kc, k = e - j * kc;
-                    if (j < nj) __stcs(cb + ((long long)base * g.nc[1] + J0 + j) * kc + k, acc[0][n]);
-                }
-            }
+            for (int n = 0; n < NPT; ++n)
+                if (coff[n] >= 0) __stcs(cp + coff[n], acc[0][n]);
         }
 #pragma unroll
         for (int a = 0; a + 1 < 2 * P; ++a)
 #pragma unroll
-            for (int n = 0; n < kMaxPt; ++n) acc[a][n] = acc[a + 1][n];
+            for (int n = 0; n < NPT; ++n) acc[a][n] = acc[a + 1][n];
 #pragma unroll
-        for (int n = 0; n < kMaxPt; ++n) acc[2 * P - 1][n] = 0.0;
+        for (int n = 0; n < NPT; ++n) acc[2 * P - 1][n] = 0.0;
         // even plane on coarse c + 1 (slot P - 1 after the shift)
         if (c + 1 >= I0 && c + 1 < I0 + ni) {
             const int xf = wrap_or_zero(2 * c + 2 + g.off[0], g.nf[0], g.bc[0]);
             if (xf >= 0) {
                 plane(xf, s);
 #pragma unroll
-                for (int n = 0; n < kMaxPt; ++n) acc[P - 1][n] = fma(r[0], s[n], acc[P - 1][n]);
+                for (int n = 0; n < NPT; ++n) acc[P - 1][n] = fma(r[0], s[n], acc[P - 1][n]);
             }
         }
     }
@@ -155,7 +176,8 @@ fd_restrict_kernel(const __grid_constant__ TGeom g, const double *__restrict__ f
 // -------------------------------------------------------------------------------- interpolation
 // blockIdx.x: coarse y tile (jt rows -> 2 jt fine rows, + the fine row below the first coarse row
 // on a zero-BC axis), blockIdx.y: chunk of ic coarse x planes, blockIdx.z: band.
-template <int P>
+// NPT: fine-plane points per thread (point e = tid + n * kThreads of the (2 jt + 1) x nzf tile).
+template <int P, int NPT>
 __global__ void __launch_bounds__(kThreads)
 fd_interp_kernel(const __grid_constant__ TGeom g, const double *__restrict__ coarse,
                  double *__restrict__ fine, int jt, int ic)
@@ -166,7 +188,7 @@ fd_interp_kernel(const __grid_constant__ TGeom g, const double *__restrict__ coa
     const int rows = jt + 2 * P;              // coarse rows staged per plane: J0 - P .. J0 + jt + P - 1
     double *C = sm;                           // [rows][cp]
     double *T = sm + (size_t)rows * cp;       // [rows][nzf]  z-interpolated rows
-    const int tid = threadIdx.x;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int J0 = blockIdx.x * jt, nj = min(jt, g.nc[1] - J0);
     const int I0 = blockIdx.y * ic, ni = min(ic, g.nc[0] - I0);
     const long long band = blockIdx.z;
@@ -179,104 +201,98 @@ fd_interp_kernel(const __grid_constant__ TGeom g, const double *__restrict__ coa
 
     // local fine rows l = 0 .. 2 jt: e_y = 2 J0 - 1 + l (e = fine index - off); row 0 is the midpoint
     // below the tile's first coarse row: it belongs to this tile only at a zero-BC lower wall.
-    const int nl = 2 * jt + 1;
-    const int npts = nl * nzf;
     const int ey_lo = (J0 == 0 && oy == 1) ? -1 : 2 * J0;
     const int ey_hi = min(2 * (J0 + nj), g.nf[1] - oy);  // exclusive
+    // this thread's points: T offset of the (lower) coarse row, odd-row flag, fine-plane offset (-1: none)
+    int toff[NPT], foff[NPT];
+    unsigned oddmask = 0;
+#pragma unroll
+    for (int n = 0; n < NPT; ++n) {
+        const int e = tid + n * kThreads;
+        const int l = e / nzf, fz = e - l * nzf;
+        const bool in_tile = e < (2 * jt + 1) * nzf;
+        const int ey = 2 * J0 - 1 + l;
+        const bool odd = (ey & 1) != 0;
+        // staged row of coarse row cy is cy - J0 + P; odd rows: lower neighbour c = (ey - 1) / 2
+        const int crow = (odd ? ((ey - 1) >> 1) : (ey >> 1)) - J0 + P;
+        toff[n] = in_tile ? crow * nzf + fz : P * nzf;
+        if (odd && in_tile) oddmask |= 1u << n;
+        foff[n] = (in_tile && ey >= ey_lo && ey < ey_hi) ? (ey + oy) * nzf + fz : -1;
+    }
 
-    double sq[2 * P][kMaxPt];  // y-z-interpolated coarse planes i - 2P + 1 .. i
+    double sq[2 * P][NPT];  // y-z-interpolated coarse planes i - 2P + 1 .. i
 #pragma unroll
     for (int a = 0; a < 2 * P; ++a)
 #pragma unroll
-        for (int n = 0; n < kMaxPt; ++n) sq[a][n] = 0.0;
+        for (int n = 0; n < NPT; ++n) sq[a][n] = 0.0;
 
-    auto plane = [&](int xc, double (&s)[kMaxPt]) {
+    auto plane = [&](int xc, double (&s)[NPT]) {
         __syncthreads();
-        const double *cpx = cb + (long long)xc * g.nc[1] * kc;
-        for (int e = tid; e < rows * cp; e += kThreads) {
-            const int rr = e / cp, zp = e - rr * cp;
-            const int y = wrap_or_zero(J0 - P + rr, g.nc[1], g.bc[1]);
-            const int z = wrap_or_zero(zp - P, kc, g.bc[2]);
-            C[e] = (y < 0 || z < 0) ? 0.0 : __ldg(cpx + (long long)y * kc + z);
-        }
+        stage_rows(C, cb + (long long)xc * g.nc[1] * kc, rows, J0 - P, g.nc[1], g.bc[1], kc, P, g.bc[2]);
         __syncthreads();
-        for (int e = tid; e < rows * nzf; e += kThreads) {
-            const int rr = e / nzf, fz = e - rr * nzf;
-            const int ez = fz - oz;            // >= -1
+        for (int rr = warp; rr < rows; rr += kThreads / 32) {
             const double *row = C + rr * cp + P;
-            double t;
-            if ((ez & 1) == 0) {
-                t = row[ez >> 1];
-            } else {
-                const int c = (ez - 1) >> 1;   // lower coarse neighbour (-1 at a zero-BC wall)
-                t = 0.0;
+            for (int fz = lane; fz < nzf; fz += 32) {
+                const int ez = fz - oz;            // >= -1
+                double t;
+                if ((ez & 1) == 0) {
+                    t = row[ez >> 1];
+                } else {
+                    const int c = (ez - 1) >> 1;   // lower coarse neighbour (-1 at a zero-BC wall)
+                    t = 0.0;
 #pragma unroll
-                for (int j = 1; j <= P; ++j) t = fma(b[j], row[c + 1 - j] + row[c + j], t);
+                    for (int j = 1; j <= P; ++j) t = fma(b[j], row[c + 1 - j] + row[c + j], t);
+                }
+                T[rr * nzf + fz] = t;
             }
-            T[e] = t;
         }
         __syncthreads();
 #pragma unroll
-        for (int n = 0; n < kMaxPt; ++n) {
-            const int e = tid + n * kThreads;
-            if (e < npts) {
-                const int l = e / nzf, fz = e - l * nzf;
-                const int ey = 2 * J0 - 1 + l;
-                // staged row of coarse row cy is cy - J0 + P
-                if ((ey & 1) == 0) {
-                    s[n] = T[((ey >> 1) - J0 + P) * nzf + fz];
-                } else {
-                    const int c = ((ey - 1) >> 1) - J0 + P;
-                    double t = 0.0;
+        for (int n = 0; n < NPT; ++n) {
+            const double *col = T + toff[n];
+            if (oddmask & (1u << n)) {
+                double t = 0.0;
 #pragma unroll
-                    for (int j = 1; j <= P; ++j)
-                        t = fma(b[j], T[(c + 1 - j) * nzf + fz] + T[(c + j) * nzf + fz], t);
-                    s[n] = t;
-                }
+                for (int j = 1; j <= P; ++j) t = fma(b[j], col[(1 - j) * nzf] + col[j * nzf], t);
+                s[n] = t;
             } else {
-                s[n] = 0.0;
+                s[n] = col[0];
             }
         }
     };
-    auto store_plane = [&](int ex, const double (&s)[kMaxPt]) {
+    auto store_plane = [&](int ex, const double (&s)[NPT]) {
         const int fx = ex + ox;
         if (fx < 0 || fx >= g.nf[0]) return;
+        double *fpx = fb + (long long)fx * g.nf[1] * nzf;
 #pragma unroll
-        for (int n = 0; n < kMaxPt; ++n) {
-            const int e = tid + n * kThreads;
-            if (e < npts) {
-                const int l = e / nzf, fz = e - l * nzf;
-                const int ey = 2 * J0 - 1 + l;
-                if (ey >= ey_lo && ey < ey_hi)
-                    __stcs(fb + ((long long)fx * g.nf[1] + ey + oy) * nzf + fz, s[n]);
-            }
-        }
+        for (int n = 0; n < NPT; ++n)
+            if (foff[n] >= 0) __stcs(fpx + foff[n], s[n]);
     };
 
     // the chunk owns the even planes e_x = 2 i, i in [I0, I0 + ni), and the odd planes e_x = 2 c + 1,
     // c in [c_first, I0 + ni): c_first = -1 for the first chunk on a zero-BC axis (the wall), else I0
     const int c_first = (I0 == 0 && ox == 1) ? -1 : I0;
     for (int i = c_first + 1 - P; i <= I0 + ni - 1 + P; ++i) {
-        double s[kMaxPt];
+        double s[NPT];
         const int xc = wrap_or_zero(i, g.nc[0], g.bc[0]);
         if (xc >= 0) {
             plane(xc, s);
         } else {
 #pragma unroll
-            for (int n = 0; n < kMaxPt; ++n) s[n] = 0.0;
+            for (int n = 0; n < NPT; ++n) s[n] = 0.0;
         }
 #pragma unroll
         for (int a = 0; a + 1 < 2 * P; ++a)
 #pragma unroll
-            for (int n = 0; n < kMaxPt; ++n) sq[a][n] = sq[a + 1][n];
+            for (int n = 0; n < NPT; ++n) sq[a][n] = sq[a + 1][n];
 #pragma unroll
-        for (int n = 0; n < kMaxPt; ++n) sq[2 * P - 1][n] = s[n];
+        for (int n = 0; n < NPT; ++n) sq[2 * P - 1][n] = s[n];
         if (i >= I0 && i < I0 + ni) store_plane(2 * i, s);
         const int c = i - P;  // odd plane between coarse c and c + 1: sq[P - j] and sq[P + j - 1]
         if (c >= c_first && c < I0 + ni) {
-            double o[kMaxPt];
+            double o[NPT];
 #pragma unroll
-            for (int n = 0; n < kMaxPt; ++n) {
+            for (int n = 0; n < NPT; ++n) {
                 double t = 0.0;
 #pragma unroll
                 for (int j = 1; j <= P; ++j) t = fma(b[j], sq[P - j][n] + sq[P + j - 1][n], t);
@@ -328,6 +344,8 @@ int fill_geom(TGeom &g, const int32_t shape_fine[3], const int32_t bc[3], int p)
 void tile_choice(int pts_per_row, bool interp, int ncx, int ncy, int64_t nbands, int sm_count,
                  int *jt, int *ic)
 {
+    // 8 coarse rows per tile where the swept plane fits (16 was measured: fewer halo rows, but too few
+    // CTAs for single arrays and small grids)
     int t = 8;
     while (t > 1 && (interp ? (2 * t + 1) : t) * pts_per_row > kThreads * kMaxPt) t >>= 1;
     if (t > ncy) t = ncy;
@@ -340,24 +358,11 @@ void tile_choice(int pts_per_row, bool interp, int ncx, int ncy, int64_t nbands,
     *ic = (int)((ncx + chunks - 1) / chunks);
 }
 
-template <int P>
-cudaError_t launch(bool interp, const TGeom &g, const double *src, double *dst, int64_t nbands,
-                   cudaStream_t stream)
+template <int P, int NPT>
+cudaError_t launch_npt(bool interp, const TGeom &g, const double *src, double *dst, int64_t nbands,
+                       int jt, int ic, size_t smem, cudaStream_t stream)
 {
-    int dev = 0, sms = 148;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    int jt, ic;
-    tile_choice(interp ? g.nf[2] : g.nc[2], interp, g.nc[0], g.nc[1], nbands, sms, &jt, &ic);
-    if ((interp ? (2 * jt + 1) * g.nf[2] : jt * g.nc[2]) > kThreads * kMaxPt)
-        return cudaErrorInvalidConfiguration;
-    size_t smem;
-    if (interp)
-        smem = sizeof(double) * ((size_t)(jt + 2 * P) * (g.nc[2] + 2 * P) + (size_t)(jt + 2 * P) * g.nf[2]);
-    else
-        smem = sizeof(double) * (size_t)(2 * jt - 1 + 2 * (2 * P - 1)) * (g.nf[2] + 2 * (2 * P - 1) + g.nc[2]);
-    if (smem > (size_t)kFdSweepSmemMax) return cudaErrorInvalidConfiguration;
-    const void *fn = interp ? (const void *)fd_interp_kernel<P> : (const void *)fd_restrict_kernel<P>;
+    const void *fn = interp ? (const void *)fd_interp_kernel<P, NPT> : (const void *)fd_restrict_kernel<P, NPT>;
     cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, kFdSweepSmemMax);
     if (e != cudaSuccess) return e;
     const unsigned gx = (unsigned)((g.nc[1] + jt - 1) / jt), gy = (unsigned)((g.nc[0] + ic - 1) / ic);
@@ -367,15 +372,41 @@ cudaError_t launch(bool interp, const TGeom &g, const double *src, double *dst, 
     for (int64_t b0 = 0; b0 < nbands; b0 += 65535) {
         const unsigned nb = (unsigned)((nbands - b0 < 65535) ? nbands - b0 : 65535);
         if (interp)
-            fd_interp_kernel<P><<<dim3(gx, gy, nb), kThreads, smem, stream>>>(
+            fd_interp_kernel<P, NPT><<<dim3(gx, gy, nb), kThreads, smem, stream>>>(
                 g, src + b0 * band_c, dst + b0 * band_f, jt, ic);
         else
-            fd_restrict_kernel<P><<<dim3(gx, gy, nb), kThreads, smem, stream>>>(
+            fd_restrict_kernel<P, NPT><<<dim3(gx, gy, nb), kThreads, smem, stream>>>(
                 g, src + b0 * band_f, dst + b0 * band_c, jt, ic);
         e = cudaPeekAtLastError();
         if (e != cudaSuccess) return e;
     }
     return cudaSuccess;
+}
+
+template <int P>
+cudaError_t launch(bool interp, const TGeom &g, const double *src, double *dst, int64_t nbands,
+                   cudaStream_t stream)
+{
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    int jt, ic;
+    tile_choice(interp ? g.nf[2] : g.nc[2], interp, g.nc[0], g.nc[1], nbands, sms, &jt, &ic);
+    const int pts = interp ? (2 * jt + 1) * g.nf[2] : jt * g.nc[2];
+    if (pts > kThreads * kMaxPt) return cudaErrorInvalidConfiguration;
+    size_t smem;
+    if (interp)
+        smem = sizeof(double) * ((size_t)(jt + 2 * P) * (g.nc[2] + 2 * P) + (size_t)(jt + 2 * P) * g.nf[2]);
+    else
+        smem = sizeof(double) * (size_t)(2 * jt - 1 + 2 * (2 * P - 1)) * (g.nf[2] + 2 * (2 * P - 1) + g.nc[2]);
+    if (smem > (size_t)kFdSweepSmemMax) return cudaErrorInvalidConfiguration;
+    const int npt = (pts + kThreads - 1) / kThreads;
+    if (npt <= 1) return launch_npt<P, 1>(interp, g, src, dst, nbands, jt, ic, smem, stream);
+    if (npt <= 2) return launch_npt<P, 2>(interp, g, src, dst, nbands, jt, ic, smem, stream);
+    if (npt <= 3) return launch_npt<P, 3>(interp, g, src, dst, nbands, jt, ic, smem, stream);
+    if (npt <= 4) return launch_npt<P, 4>(interp, g, src, dst, nbands, jt, ic, smem, stream);
+    if (npt <= 6) return launch_npt<P, 6>(interp, g, src, dst, nbands, jt, ic, smem, stream);
+    return launch_npt<P, 8>(interp, g, src, dst, nbands, jt, ic, smem, stream);
 }
 
 }  // namespace
