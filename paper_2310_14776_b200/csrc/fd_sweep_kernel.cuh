@@ -48,7 +48,7 @@
 //     faster and catches up, so the drift stays far below what the 126 MB L2 retains (measured:
 //     DRAM reads 1.92 GB against 1.82 GB algorithmic on the 96^3 x 256 workload).  A progress
 //     throttle through global memory was tried and removed: its polls sit behind the bulk
-//     traffic in the memory system and cost more than 2x (profiles/r1c notes).
+//     traffic in the memory system and cost more than 2x (dropped variants).
 //   * L2 policy: planes that the periodic x wrap reads twice (the first and last three of a band)
 //     are loaded evict_last the first time, as is v_eff (shared by all bands).
 #pragma once
