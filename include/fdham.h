@@ -81,7 +81,8 @@ enum {
  *   nn         stencil half width (order 2*nn), 1..6
  *   bc         host: FD_BC_ZERO | FD_BC_PERIODIC per axis; a periodic axis needs n_d >= nn
  *   k_reduced  host: Bloch vector in reduced coordinates, NULL = Gamma; must be 0 on zero-BC axes
- *   dtype      FD_F64 (requires k = 0) or FD_C128
+ *   dtype      FD_F64 (requires 2 k_d integer on every axis: the Bloch factors are then +-1 and the
+ *              data stay real, e.g. the zone-boundary point k = 1/2) or FD_C128
  *   device     CUDA device ordinal
  * Errors: FD_ERR_INVALID for any violated constraint above, FD_ERR_UNSUPPORTED for nx > 65535 or
  * ny > 262140 (no kernel of this build launches such a grid), FD_ERR_CUDA if the device cannot be

@@ -96,7 +96,9 @@ int apply_device(const fd_plan *plan, const FdGeom &g, int mode, const void *psi
     if (drc != FD_OK) return drc;
     cudaError_t e;
     int n = 0;
-    if (kernel_for_batch(plan, nbands) == FD_KERNEL_SWEEP) {
+    // float64 plans with a Bloch factor -1 have no Jacobi instantiation of the sweep kernel
+    const bool sweep_ok = !(mode == 2 && fd_plan_real_phase(plan));
+    if (sweep_ok && kernel_for_batch(plan, nbands) == FD_KERNEL_SWEEP) {
         const bool fused = eps && fd_sweep_expect_fused(plan);
         e = fd_launch_sweep(plan, g, mode, psi, second, out, nbands, fused ? eps : nullptr, norm, ws,
                             stream, &n);
@@ -158,7 +160,9 @@ int fd_create_scaled(fd_plan **plan_out, const int32_t shape[3], const double h[
         if (bc[d] == FD_BC_PERIODIC && shape[d] < nn) return FD_ERR_INVALID;
         const double kd = k_reduced ? k_reduced[d] : 0.0;
         if (!isfinite(kd)) return FD_ERR_INVALID;
-        if (kd != 0.0 && (bc[d] == FD_BC_ZERO || dtype == FD_F64)) return FD_ERR_INVALID;
+        if (kd != 0.0 && bc[d] == FD_BC_ZERO) return FD_ERR_INVALID;
+        // real data: the Bloch factor exp(2 pi i k_d) must be real: +-1, i.e. 2 k_d an integer
+        if (dtype == FD_F64 && 2.0 * kd != rint(2.0 * kd)) return FD_ERR_INVALID;
     }
     if ((long long)shape[0] * shape[1] * shape[2] > (1LL << 40)) return FD_ERR_INVALID;
 
@@ -205,6 +209,10 @@ int fd_create_scaled(fd_plan **plan_out, const int32_t shape[3], const double h[
         // exp(+2 pi i k_d); exact 1 at Gamma so real-valued data stays phase free
         if (p->k[d] == 0.0) {
             g.ph_re[d] = 1.0;
+            g.ph_im[d] = 0.0;
+        } else if (2.0 * p->k[d] == rint(2.0 * p->k[d])) {
+            // integer or half-integer k: exactly +1 / -1 (float64 plans rely on it)
+            g.ph_re[d] = (fmod(fabs(2.0 * p->k[d]), 2.0) == 1.0) ? -1.0 : 1.0;
             g.ph_im[d] = 0.0;
         } else {
             g.ph_re[d] = cos(2.0 * kPi * p->k[d]);

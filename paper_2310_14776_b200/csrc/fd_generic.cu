@@ -16,7 +16,8 @@ struct Val<false> {
     double x;
     __device__ __forceinline__ static Val zero() { return {0.0}; }
     __device__ __forceinline__ void fma(double w, const Val &o) { x = ::fma(w, o.x, x); }
-    __device__ __forceinline__ Val mulphase(double, double) const { return *this; }
+    // real data: the Bloch factor is +1 or -1 (k_d = 1/2), its imaginary part 0
+    __device__ __forceinline__ Val mulphase(double pr, double) const { return {x * pr}; }
 };
 template <>
 struct Val<true> {

@@ -87,6 +87,7 @@ typedef void (*FdSweepKernelFn)(const FdGeom, const FdSweepCfg, const double *, 
 FdSweepKernelFn fd_sweep_pick_real(int rowd, int mode, int nn);
 FdSweepKernelFn fd_sweep_pick_real_ex(int rowd, int mode, int nn);
 FdSweepKernelFn fd_sweep_pick_real_jacobi(int rowd, int nn);
+FdSweepKernelFn fd_sweep_pick_real_ph(int mode, int nn);  // float64, Bloch factors -1 (k = 1/2)
 FdSweepKernelFn fd_sweep_pick_cplx_ph0(int rowd, int mode, int nn);
 FdSweepKernelFn fd_sweep_pick_cplx_ph1(int rowd, int mode, int nn);
 FdSweepKernelFn fd_sweep_pick_cplx_ph3(int rowd, int mode, int nn);
@@ -109,6 +110,7 @@ int fd_tune_value(const char *key);
 // fd_sweep.cu
 void fd_sweep_configure(fd_plan *plan, int tyc_override, int xchunk_override, int stages_override);
 cudaError_t fd_sweep_prepare(fd_plan *plan);  // shared-memory opt-in of the plan's kernels
+bool fd_plan_real_phase(const fd_plan *plan);      // float64 plan with a Bloch factor -1
 bool fd_sweep_expect_fused(const fd_plan *plan);  // else: two passes (sweep, then fd_launch_dot)
 int64_t fd_sweep_expect_ws_bytes(const fd_plan *plan, int64_t nbands);
 cudaError_t fd_launch_sweep(const fd_plan *plan, const FdGeom &g, int mode, const void *psi,

@@ -80,6 +80,15 @@ void fd_sweep_configure(fd_plan *plan, int tyc_override, int xchunk_override, in
     c.supported = 1;
 }
 
+bool fd_plan_real_phase(const fd_plan *plan)
+{
+    const FdGeom &g = plan->g;
+    if (g.cplx) return false;
+    for (int d = 0; d < 3; ++d)
+        if (g.bc[d] && g.ph_re[d] != 1.0) return true;
+    return false;
+}
+
 namespace {
 
 FdSweepKernelFn kernel_for(const fd_plan *plan, int mode, bool ex)
@@ -87,6 +96,8 @@ FdSweepKernelFn kernel_for(const fd_plan *plan, int mode, bool ex)
     const FdGeom &g = plan->g;
     const int rowd = g.n[2] * (g.cplx ? 2 : 1);
     if (!g.cplx) {
+        if (fd_plan_real_phase(plan))  // plain applies only; the other forms fall back (fd_api.cu)
+            return (mode == 2 || ex) ? nullptr : fd_sweep_pick_real_ph(mode, g.nn);
         if (mode == 2) return fd_sweep_pick_real_jacobi(rowd, g.nn);
         return ex ? fd_sweep_pick_real_ex(rowd, mode, g.nn) : fd_sweep_pick_real(rowd, mode, g.nn);
     }
@@ -154,8 +165,10 @@ cudaError_t fd_sweep_prepare(fd_plan *plan)
     for (int mode = 0; mode < 3; ++mode)
         for (int ex = 0; ex < 2; ++ex) {
             if (mode == 2 && (ex || plan->g.cplx)) continue;
+            const FdSweepKernelFn fn = kernel_for(plan, mode, ex != 0);
+            if (!fn) continue;  // form not on the sweep kernel for this plan
             cudaError_t e = cudaFuncSetAttribute(
-                reinterpret_cast<const void *>(kernel_for(plan, mode, ex != 0)),
+                reinterpret_cast<const void *>(fn),
                 cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemMax);
             if (e != cudaSuccess) return e;
         }
@@ -164,7 +177,10 @@ cudaError_t fd_sweep_prepare(fd_plan *plan)
 
 // Plans on the sweep kernel take the expectation values from the same pass; the others take the
 // two-pass form (fd_aux.cu).
-bool fd_sweep_expect_fused(const fd_plan *plan) { return plan->sweep.supported != 0; }
+bool fd_sweep_expect_fused(const fd_plan *plan)
+{
+    return plan->sweep.supported != 0 && !fd_plan_real_phase(plan);
+}
 
 // Bytes of workspace fd_launch_sweep needs for the expectation values of an `nbands` batch.
 int64_t fd_sweep_expect_ws_bytes(const fd_plan *plan, int64_t nbands)

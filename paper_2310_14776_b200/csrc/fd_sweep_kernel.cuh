@@ -407,9 +407,10 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
     const bool swp = !CPLX && (tid & 8) != 0;
     const int off8a = swp ? hb[2 * ZH - 1] : hb[0] + 8;
     const int off8b = swp ? hb[0] + 8 : hb[2 * ZH - 1];
-    const bool zphase = CPLX && (PH & 2) && per_z && (g.ph_re[2] != 1.0 || g.ph_im[2] != 0.0) && zwrap != 0;
-    const bool yphase = CPLX && (PH & 1) && per_y && (g.ph_re[1] != 1.0 || g.ph_im[1] != 0.0);
-    const bool xphase = CPLX && (PH & 1) && per_x && (g.ph_re[0] != 1.0 || g.ph_im[0] != 0.0);
+    // float64 with PH != 0: real Bloch factors -1 (k_d = 1/2): the same wraps flip a sign instead
+    const bool zphase = (PH & 2) && per_z && (g.ph_re[2] != 1.0 || g.ph_im[2] != 0.0) && zwrap != 0;
+    const bool yphase = (PH & 1) && per_y && (g.ph_re[1] != 1.0 || g.ph_im[1] != 0.0);
+    const bool xphase = (PH & 1) && per_x && (g.ph_re[0] != 1.0 || g.ph_im[0] != 0.0);
 
     // only the first row group of tile 0 has wrapped rows below, only row groups reaching past the
     // last valid row of the last tile have wrapped rows above
@@ -580,6 +581,18 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
 #pragma unroll
                             for (int t = 0; t < TC; ++t)
                                 u[i * TC + t] = lds128(ub + (NN + i) * pitch + t * 16);
+                        if constexpr ((PH & 1) != 0) {
+                            // real Bloch factor -1: wrapped x planes, and own rows past a ragged tile
+                            // end (wrapped rows: y neighbours of the last valid rows)
+                            const bool xneg = xphase && (m.x & (kWrapLo | kWrapHi));
+#pragma unroll
+                            for (int i = 0; i < TY; ++i)
+                                if (xneg != (yhi && r0 + NN + i >= nlo + nmid)) {
+#pragma unroll
+                                    for (int t = 0; t < TC; ++t)
+                                        u[i * TC + t] = make_double2(-u[i * TC + t].x, -u[i * TC + t].y);
+                                }
+                        }
                     } else {
 #pragma unroll
                         for (int p = 0; p < NP; ++p) u[p] = make_double2(0.0, 0.0);
@@ -641,6 +654,14 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
                             double2 c[TC];
 #pragma unroll
                             for (int t = 0; t < TC; ++t) c[t] = lds128(ub + rr * pitch + t * 16);
+                            if constexpr ((PH & 1) != 0) {
+                                // the own values above carry the x sign of a wrapped plane, but a centre
+                                // plane is never wrapped: only the y wraps matter here
+                                if ((rr < NN) ? (ylo && r0 + rr < nlo) : (yhi && r0 + rr >= nlo + nmid)) {
+#pragma unroll
+                                    for (int t = 0; t < TC; ++t) c[t] = make_double2(-c[t].x, -c[t].y);
+                                }
+                            }
 #pragma unroll
                             for (int i = 0; i < TY; ++i) {
                                 const int d = rr - NN - i;
@@ -677,10 +698,18 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
                                     // lane stride would be a 2-way bank conflict).
                                     const double e0 = lds64(sb + off8a + i * pitch);
                                     const double e1 = lds64(sb + off8b + i * pitch);
-                                    const double l3 = swp ? e1 : e0;
-                                    const double r4 = swp ? e0 : e1;
-                                    const double2 l21 = lds128(sb + hb[1] + i * pitch);
-                                    const double2 r23 = lds128(sb + hb[2] + i * pitch);
+                                    double l3 = swp ? e1 : e0;
+                                    double r4 = swp ? e0 : e1;
+                                    double2 l21 = lds128(sb + hb[1] + i * pitch);
+                                    double2 r23 = lds128(sb + hb[2] + i * pitch);
+                                    if constexpr ((PH & 2) != 0) {
+                                        if (zphase) {  // wrapped halo chunks flip their sign
+                                            if (zwrap & (3 << 0)) l3 = -l3;
+                                            if (zwrap & (3 << 2)) l21 = make_double2(-l21.x, -l21.y);
+                                            if (zwrap & (3 << 4)) r23 = make_double2(-r23.x, -r23.y);
+                                            if (zwrap & (3 << 6)) r4 = -r4;
+                                        }
+                                    }
                                     a.x = fma(wz[1], l21.y, a.x);
                                     a.x = fma(wz[1], o.y, a.x);
                                     a.x = fma(wz[2], l21.x, a.x);
@@ -695,8 +724,14 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
                                     a.y = fma(wz[3], r4, a.y);
                                 } else if constexpr (NN == 2) {
                                     // halo = z-2,z-1 | z+2,z+3: the two neighbouring chunks
-                                    const double2 l21 = lds128(sb + hb[0] + i * pitch);
-                                    const double2 r23 = lds128(sb + hb[1] + i * pitch);
+                                    double2 l21 = lds128(sb + hb[0] + i * pitch);
+                                    double2 r23 = lds128(sb + hb[1] + i * pitch);
+                                    if constexpr ((PH & 2) != 0) {
+                                        if (zphase) {
+                                            if (zwrap & (3 << 0)) l21 = make_double2(-l21.x, -l21.y);
+                                            if (zwrap & (3 << 2)) r23 = make_double2(-r23.x, -r23.y);
+                                        }
+                                    }
                                     a.x = fma(wz[1], l21.y, a.x);
                                     a.x = fma(wz[1], o.y, a.x);
                                     a.x = fma(wz[2], l21.x, a.x);
@@ -709,8 +744,14 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
                                     // halo = z-1 | z+2: two 8-byte words, fetched pairwise as above
                                     const double e0 = lds64(sb + off8a + i * pitch);
                                     const double e1 = lds64(sb + off8b + i * pitch);
-                                    const double l1 = swp ? e1 : e0;
-                                    const double r2 = swp ? e0 : e1;
+                                    double l1 = swp ? e1 : e0;
+                                    double r2 = swp ? e0 : e1;
+                                    if constexpr ((PH & 2) != 0) {
+                                        if (zphase) {
+                                            if (zwrap & (3 << 0)) l1 = -l1;
+                                            if (zwrap & (3 << 2)) r2 = -r2;
+                                        }
+                                    }
                                     a.x = fma(wz[1], l1, a.x);
                                     a.x = fma(wz[1], o.y, a.x);
                                     a.y = fma(wz[1], o.x, a.y);

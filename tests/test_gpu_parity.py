@@ -647,3 +647,44 @@ def test_host_workspace_reuse(oracle, fd):
     finally:
         fd.fd_workspace_destroy(ws)
         fd.fd_destroy(plan)
+
+
+# ------------------------------------------------------------------------------ f1: real dtype at k = 1/2
+
+@pytest.mark.parametrize("k", [(0.5, 0.0, 0.0), (0.0, 0.5, 0.0), (0.0, 0.0, 0.5), (0.5, 0.5, 0.5),
+                               (-0.5, 1.0, 1.5)])
+def test_real_dtype_at_zone_boundary_k(oracle, fd, k):
+    """FD_F64 with Bloch factors -1.  The oracle runs the complex definition on the
+    real input (its imaginary part must vanish); both kernel families, nn = 1..3, ragged tiles."""
+    for nn, shape, bc in [(3, (10, 22, 16), (1, 1, 1)), (2, (9, 20, 12), (1, 1, 1)), (1, (12, 10, 8), (1, 1, 1)),
+                          (3, (12, 18, 24), (1, 0, 1))]:
+        kk = tuple(x if b else 0.0 for x, b in zip(k, bc))
+        cfg = W.custom(shape, (0.2, 0.23, 0.17), bc, nbands=5, nn=nn)
+        psi, v = W.make_psi(cfg), W.make_veff(cfg)
+        want_c = oracle.apply(cfg.shape, cfg.h, nn, bc, kk, psi.astype(np.complex128), v)
+        assert np.max(np.abs(want_c.imag)) <= 1e-13 * np.abs(want_c).max()
+        tol = parity_tol(cfg.h, nn, psi, v)
+        for kern in (fd.FD_KERNEL_SWEEP, fd.FD_KERNEL_GENERIC):
+            plan = fd.fd_create(cfg.shape, cfg.h, nn, bc, kk, fd.FD_F64, 0)
+            try:
+                fd.fd_plan_set_kernel(plan, kern, 8 if kern == fd.FD_KERNEL_SWEEP else 0)
+                d_psi = torch.from_numpy(psi).cuda()
+                d_out = torch.full_like(d_psi, float("nan"))
+                fd.fd_apply_hamiltonian(plan, d_psi, torch.from_numpy(v).cuda(), d_out)
+                torch.cuda.synchronize()
+                err = float(np.max(np.abs(d_out.cpu().numpy() - want_c.real)))
+                assert err <= tol, (k, nn, kern, err, tol)
+                # the other forms fall back to code that knows the sign: expectation values, Jacobi
+                eps = torch.empty(5, dtype=torch.float64, device="cuda")
+                nrm = torch.empty_like(eps)
+                ws = torch.empty(fd.fd_expect_workspace_bytes(plan, 5) // 8 + 1, dtype=torch.float64,
+                                 device="cuda")
+                fd.fd_apply_hamiltonian_expect(plan, d_psi, torch.from_numpy(v).cuda(), d_out, eps, nrm, ws)
+                torch.cuda.synchronize()
+                w_eps = np.sum(psi * want_c.real, axis=(1, 2, 3))
+                assert np.max(np.abs(eps.cpu().numpy() - w_eps)) <= tol * psi[0].size * np.abs(psi).max()
+            finally:
+                fd.fd_destroy(plan)
+    with pytest.raises(fd.FDError) as ei:
+        fd.fd_create((8, 8, 8), (0.4,) * 3, 3, (1, 1, 1), (0.25, 0, 0), fd.FD_F64, 0)
+    assert ei.value.status == -1
