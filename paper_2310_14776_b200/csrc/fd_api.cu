@@ -96,8 +96,8 @@ int apply_device(const fd_plan *plan, const FdGeom &g, int mode, const void *psi
     if (drc != FD_OK) return drc;
     cudaError_t e;
     int n = 0;
-    // float64 plans with a Bloch factor -1 have no Jacobi instantiation of the sweep kernel
-    const bool sweep_ok = !(mode == 2 && fd_plan_real_phase(plan));
+    // float64 plans with a Bloch factor -1 and nn > 3 have no Jacobi instantiation of the sweep kernel
+    const bool sweep_ok = !(mode == 2 && (fd_plan_real_phase(plan) || plan->g.nn > 3));
     if (sweep_ok && kernel_for_batch(plan, nbands) == FD_KERNEL_SWEEP) {
         const bool fused = eps && fd_sweep_expect_fused(plan);
         e = fd_launch_sweep(plan, g, mode, psi, second, out, nbands, fused ? eps : nullptr, norm, ws,

@@ -87,7 +87,9 @@ typedef void (*FdSweepKernelFn)(const FdGeom, const FdSweepCfg, const double *, 
 FdSweepKernelFn fd_sweep_pick_real(int rowd, int mode, int nn);
 FdSweepKernelFn fd_sweep_pick_real_ex(int rowd, int mode, int nn);
 FdSweepKernelFn fd_sweep_pick_real_jacobi(int rowd, int nn);
-FdSweepKernelFn fd_sweep_pick_real_ph(int mode, int nn);  // float64, Bloch factors -1 (k = 1/2)
+FdSweepKernelFn fd_sweep_pick_real_ph(int mode, int nn);
+FdSweepKernelFn fd_sweep_pick_real_hi(int mode, int nn);  // nn = 4..6, float64
+FdSweepKernelFn fd_sweep_pick_cplx_hi(int mode, int nn);  // nn = 4..6, complex128 (all phase code)  // float64, Bloch factors -1 (k = 1/2)
 FdSweepKernelFn fd_sweep_pick_cplx_ph0(int rowd, int mode, int nn);
 FdSweepKernelFn fd_sweep_pick_cplx_ph1(int rowd, int mode, int nn);
 FdSweepKernelFn fd_sweep_pick_cplx_ph3(int rowd, int mode, int nn);

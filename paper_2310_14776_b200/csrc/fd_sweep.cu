@@ -20,11 +20,11 @@ void fd_sweep_configure(fd_plan *plan, int tyc_override, int xchunk_override, in
     c = FdSweepCfg{};
     c.xchunk = xchunk_override;  // 0 = automatic (persistent teams), else planes per team
     c.stages_req = stages_override;
-    if (g.nn > 3) return;  // 2 nn + 1 accumulator planes: the register budget ends at nn = 3
+    if (g.nn > 3 && fd_plan_real_phase(plan)) return;  // no sign-flip instantiation for nn > 3
     const int halo = 2 * g.nn;
     if (g.n[0] < 8 || g.n[1] < 8 || g.n[2] < 8 || (g.n[2] & 1)) return;
     if (g.n[0] > 65536) return;  // x index + 2 nn in 17 bits of a step-table entry
-    c.ty = 4;
+    c.ty = g.nn <= 3 ? 4 : 2;  // 2 nn + 1 accumulator planes x ty rows per thread (registers)
     c.tc = 1;
     const int pitch = g.n[2] * (g.cplx ? 16 : 8);
     const int pitchv = g.n[2] * 8;
@@ -95,6 +95,10 @@ FdSweepKernelFn kernel_for(const fd_plan *plan, int mode, bool ex)
 {
     const FdGeom &g = plan->g;
     const int rowd = g.n[2] * (g.cplx ? 2 : 1);
+    if (g.nn > 3) {  // plain applies only; expectation values and Jacobi fall back (fd_api.cu)
+        if (mode == 2 || ex) return nullptr;
+        return g.cplx ? fd_sweep_pick_cplx_hi(mode, g.nn) : fd_sweep_pick_real_hi(mode, g.nn);
+    }
     if (!g.cplx) {
         if (fd_plan_real_phase(plan))  // plain applies only; the other forms fall back (fd_api.cu)
             return (mode == 2 || ex) ? nullptr : fd_sweep_pick_real_ph(mode, g.nn);
@@ -179,7 +183,7 @@ cudaError_t fd_sweep_prepare(fd_plan *plan)
 // two-pass form (fd_aux.cu).
 bool fd_sweep_expect_fused(const fd_plan *plan)
 {
-    return plan->sweep.supported != 0 && !fd_plan_real_phase(plan);
+    return plan->sweep.supported != 0 && !fd_plan_real_phase(plan) && plan->g.nn <= 3;
 }
 
 // Bytes of workspace fd_launch_sweep needs for the expectation values of an `nbands` batch.

@@ -229,7 +229,8 @@ struct TeamRange {
 //   the diagonal (H psi), 2: a right-hand side rhs[nbands,nx,ny,nz] added as g.rhs_coef * rhs (the
 //   weighted-Jacobi sweep of fd_jacobi_sweep: the plan's weights arrive pre-scaled in g; real only).
 // PH (complex only): which Bloch-phase code is compiled in -- bit 0: x and y wraps, bit 1: z wraps.
-// NN: stencil half width (1..3); 2 NN + 1 register accumulators per point, unrolled 2 NN + 1 times.
+// NN: stencil half width (1..6); 2 NN + 1 register accumulators per point, unrolled 2 NN + 1 times.
+//   nn = 4..6 run with a 2-row micro tile and the general z-tap form.
 // EX: also accumulate sum conj(psi) H psi and sum |psi|^2 per band (fd_apply_hamiltonian_expect).
 //   H is Hermitian: sum_i conj(psi_i) (F psi)_i = conj( sum_i conj(psi_i) (B psi)_i ) for the
 //   forward / backward halves F, B of the taps along an axis (wrapped taps carry conjugate Bloch
@@ -246,7 +247,8 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
 {
     constexpr bool HAS_V = MODE != 0;
     static_assert(!(CPLX && MODE == 2), "the Jacobi sweep is real only");
-    constexpr int TY = 4;              // rows per thread
+    constexpr int TY = (NN <= 3) ? 4 : 2;  // rows per thread: 2 NN + 1 accumulator planes x TY rows
+                                           // must fit the registers (nn = 4..6: half-height micro tile)
     constexpr int TC = 1;              // 16-byte chunks per thread per row (lane stride 16 B)
     constexpr int ZH = CPLX ? NN : (NN + 1) / 2;   // halo chunks per side along z
     constexpr int NS = 2 * NN + 1;     // in-flight output planes (accumulator slots)
@@ -740,6 +742,27 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
                                     a.y = fma(wz[1], r23.x, a.y);
                                     a.y = fma(wz[2], l21.y, a.y);
                                     a.y = fma(wz[2], r23.y, a.y);
+                                } else if constexpr (NN >= 4) {
+                                    // general form: all halo chunks as 16-byte loads.  zl[p] = point
+                                    // z - 2 ZH + p (left block, farthest chunk first), zr[p] = point
+                                    // z + 2 + p (right block); own chunk = points z, z + 1.
+                                    double zl[2 * ZH], zr[2 * ZH];
+#pragma unroll
+                                    for (int k = 0; k < ZH; ++k) {
+                                        const double2 tl = lds128(sb + hb[k] + i * pitch);
+                                        const double2 tr = lds128(sb + hb[ZH + k] + i * pitch);
+                                        zl[2 * k] = tl.x;
+                                        zl[2 * k + 1] = tl.y;
+                                        zr[2 * k] = tr.x;
+                                        zr[2 * k + 1] = tr.y;
+                                    }
+#pragma unroll
+                                    for (int j = 1; j <= NN; ++j) {
+                                        a.x = fma(wz[j], zl[2 * ZH - j], a.x);
+                                        a.x = fma(wz[j], (j == 1) ? o.y : zr[j - 2 < 0 ? 0 : j - 2], a.x);
+                                        a.y = fma(wz[j], (j == 1) ? o.x : zl[2 * ZH - (j - 1)], a.y);
+                                        a.y = fma(wz[j], zr[j - 1], a.y);
+                                    }
                                 } else {
                                     // halo = z-1 | z+2: two 8-byte words, fetched pairwise as above
                                     const double e0 = lds64(sb + off8a + i * pitch);

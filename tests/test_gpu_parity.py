@@ -688,3 +688,47 @@ def test_real_dtype_at_zone_boundary_k(oracle, fd, k):
     with pytest.raises(fd.FDError) as ei:
         fd.fd_create((8, 8, 8), (0.4,) * 3, 3, (1, 1, 1), (0.25, 0, 0), fd.FD_F64, 0)
     assert ei.value.status == -1
+
+
+# ------------------------------------------------------------------------------ f1: nn = 4, 5, 6 on the sweep kernel
+
+@pytest.mark.parametrize("nn", [4, 5, 6])
+def test_sweep_kernel_higher_orders(oracle, fd, nn):
+    """2 nn + 1 = 9 / 11 / 13 accumulator planes with a 2-row micro tile, 2 nn halo
+    rows / planes, the general z-tap form: all BC mixes, several tiles with a ragged one, real and
+    complex with Bloch phases on every axis, several bands per team and several teams."""
+    for bc in itertools.product((0, 1), repeat=3):
+        cfg = W.custom((13, 26, 16), (0.2, 0.23, 0.17), bc, nbands=7, nn=nn)
+        used = check(oracle, fd, cfg, W.make_psi(cfg), W.make_veff(cfg), fd.FD_KERNEL_SWEEP, tyc=8)
+        assert used == fd.FD_KERNEL_SWEEP
+    for bc in [(1, 1, 1), (0, 1, 1), (1, 1, 0)]:
+        k = tuple(kk if b else 0.0 for kk, b in zip((0.25, 0.125, -0.3), bc))
+        cfg = W.custom((14, 20, 12), (0.2, 0.23, 0.17), bc, k=k, complex_=True, nbands=5, nn=nn)
+        used = check(oracle, fd, cfg, W.make_psi(cfg), W.make_veff(cfg), fd.FD_KERNEL_SWEEP, tyc=6)
+        assert used == fd.FD_KERNEL_SWEEP
+        check(oracle, fd, cfg, W.make_psi(cfg), None, fd.FD_KERNEL_SWEEP)
+    cfg = W.custom((40, 48, 64), (0.2, 0.2, 0.18), (1, 1, 0), nbands=40, nn=nn)
+    used = check(oracle, fd, cfg, W.make_psi(cfg), W.make_veff(cfg), "auto")
+    assert used == fd.FD_KERNEL_SWEEP
+    # n = 2 nn on a periodic axis: taps +nn and -nn hit the same point (R7)
+    cfg = W.custom((2 * nn, 2 * nn + 2, 2 * nn), (0.2, 0.23, 0.17), (1, 1, 1), nbands=3, nn=nn)
+    if min(cfg.shape) >= 8:
+        check(oracle, fd, cfg, W.make_psi(cfg), W.make_veff(cfg), fd.FD_KERNEL_SWEEP)
+    # the forms without an nn > 3 instantiation fall back and stay correct
+    cfg = W.custom((12, 16, 16), (0.2, 0.23, 0.17), (1, 0, 1), nbands=3, nn=nn)
+    psi, v = W.make_psi(cfg), W.make_veff(cfg)
+    plan = fd.fd_create(cfg.shape, cfg.h, nn, cfg.bc)
+    try:
+        fd.fd_plan_set_kernel(plan, fd.FD_KERNEL_SWEEP)
+        d_psi = torch.from_numpy(psi).cuda()
+        d_out = torch.full_like(d_psi, float("nan"))
+        eps = torch.empty(3, dtype=torch.float64, device="cuda")
+        nrm = torch.empty_like(eps)
+        ws = torch.empty(fd.fd_expect_workspace_bytes(plan, 3) // 8 + 1, dtype=torch.float64, device="cuda")
+        fd.fd_apply_hamiltonian_expect(plan, d_psi, torch.from_numpy(v).cuda(), d_out, eps, nrm, ws)
+        torch.cuda.synchronize()
+        w_eps, w_n, want = oracle.expect(cfg.shape, cfg.h, nn, cfg.bc, None, psi, v, want_out=True)
+        assert np.max(np.abs(d_out.cpu().numpy() - want)) <= parity_tol(cfg.h, nn, psi, v)
+        assert np.max(np.abs(eps.cpu().numpy() - w_eps.real)) <= parity_tol(cfg.h, nn, psi, v) * psi[0].size * np.abs(psi).max()
+    finally:
+        fd.fd_destroy(plan)
