@@ -25,7 +25,8 @@
  *     allocates inside an apply, or synchronises the device (the *_host variant excepted);
  *   - "device pointer" = memory of the plan's CUDA device; "host pointer" = ordinary CPU memory;
  *   - arrays are C-contiguous, z fastest: psi/out [nbands, nx, ny, nz], v_eff [nx, ny, nz];
- *     element = double (FD_F64) or interleaved (re, im) doubles (FD_C128); v_eff is always double;
+ *     element = double (FD_F64) or interleaved (re, im) doubles (FD_C128); v_eff is double (float
+ *     for the single-precision dtypes FD_F32 / FD_C64);
  *   - psi and v_eff are read-only; out is fully overwritten (no accumulate) and must not overlap
  *     psi or v_eff;  the caller owns all three; the library owns only the plan;
  *   - applies are enqueued on `cuda_stream` (a cudaStream_t cast to void*, NULL = legacy default
@@ -54,7 +55,7 @@ extern "C" {
 typedef struct fd_plan fd_plan; /* opaque, owned by the library */
 
 enum { FD_BC_ZERO = 0, FD_BC_PERIODIC = 1 };
-enum { FD_F64 = 0, FD_C128 = 1 };
+enum { FD_F64 = 0, FD_C128 = 1, FD_F32 = 2, FD_C64 = 3 };
 enum {
     FD_OK = 0,
     FD_ERR_INVALID = -1,     /* NULL pointer, bad shape/h/nn/bc/dtype/nbands, misaligned pointer  */
@@ -82,7 +83,12 @@ enum {
  *   bc         host: FD_BC_ZERO | FD_BC_PERIODIC per axis; a periodic axis needs n_d >= nn
  *   k_reduced  host: Bloch vector in reduced coordinates, NULL = Gamma; must be 0 on zero-BC axes
  *   dtype      FD_F64 (requires 2 k_d integer on every axis: the Bloch factors are then +-1 and the
- *              data stay real, e.g. the zone-boundary point k = 1/2) or FD_C128
+ *              data stay real, e.g. the zone-boundary point k = 1/2) or FD_C128; FD_F32 / FD_C64:
+ *              the same in single precision: psi, out AND v_eff are float32 /
+ *              interleaved float32 pairs, fp32 accumulation, fd_apply_kinetic / fd_apply_hamiltonian
+ *              only (every other call returns FD_ERR_UNSUPPORTED), nn <= 3, every axis >= 8,
+ *              nz a multiple of 4 (FD_F32) or 2 (FD_C64), FD_F32 at Gamma only: FD_ERR_UNSUPPORTED
+ *              at fd_create otherwise (there is no fallback to another precision)
  *   device     CUDA device ordinal
  * Errors: FD_ERR_INVALID for any violated constraint above, FD_ERR_UNSUPPORTED for nx > 65535 or
  * ny > 262140 (no kernel of this build launches such a grid), FD_ERR_CUDA if the device cannot be

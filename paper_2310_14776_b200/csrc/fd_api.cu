@@ -48,9 +48,9 @@ int check_apply_args(const fd_plan *plan, const void *psi, const double *v_eff, 
     if (!psi || !out || (need_v && !v_eff)) return FD_ERR_INVALID;
     if (((uintptr_t)psi | (uintptr_t)out | (uintptr_t)v_eff) & 15) return FD_ERR_INVALID;
     const size_t P = (size_t)plan->g.n[0] * plan->g.n[1] * plan->g.n[2];
-    const size_t nb = P * (size_t)nbands * (plan->g.cplx ? 16 : 8);
+    const size_t nb = P * (size_t)nbands * (size_t)fd_elem_bytes(plan->g.cplx, plan->g.f32);
     if (overlaps(out, nb, psi, nb)) return FD_ERR_ALIAS;
-    if (v_eff && overlaps(out, nb, v_eff, P * 8)) return FD_ERR_ALIAS;
+    if (v_eff && overlaps(out, nb, v_eff, P * (plan->g.f32 ? 4 : 8))) return FD_ERR_ALIAS;
     return FD_OK;
 }
 
@@ -60,7 +60,7 @@ int check_apply_args(const fd_plan *plan, const void *psi, const double *v_eff, 
 // 24^3 x 8 bands takes 8 us there against 27 us; 48^3 x 64 bands 115 us against 39 us).
 int kernel_for_batch(const fd_plan *plan, int64_t nbands)
 {
-    if (plan->kernel != FD_KERNEL_SWEEP || plan->forced) return plan->kernel;
+    if (plan->kernel != FD_KERNEL_SWEEP || plan->forced || plan->g.f32) return plan->kernel;
     const FdGeom &g = plan->g;
     const double units = (double)g.n[0] * g.n[1] * g.n[2] * (double)nbands * (g.cplx ? 2.0 : 1.0);
     const double total = (double)nbands * g.n[0];
@@ -152,7 +152,8 @@ int fd_create_scaled(fd_plan **plan_out, const int32_t shape[3], const double h[
 {
     if (!plan_out || !shape || !h || !bc || !isfinite(scale)) return FD_ERR_INVALID;
     if (nn < 1 || nn > FD_MAX_NN) return FD_ERR_INVALID;
-    if (dtype != FD_F64 && dtype != FD_C128) return FD_ERR_INVALID;
+    if (dtype != FD_F64 && dtype != FD_C128 && dtype != FD_F32 && dtype != FD_C64) return FD_ERR_INVALID;
+    const bool real_dtype = (dtype == FD_F64 || dtype == FD_F32);
     for (int d = 0; d < 3; ++d) {
         if (shape[d] < 1) return FD_ERR_INVALID;
         if (!(h[d] > 0.0) || !isfinite(h[d])) return FD_ERR_INVALID;
@@ -162,7 +163,7 @@ int fd_create_scaled(fd_plan **plan_out, const int32_t shape[3], const double h[
         if (!isfinite(kd)) return FD_ERR_INVALID;
         if (kd != 0.0 && bc[d] == FD_BC_ZERO) return FD_ERR_INVALID;
         // real data: the Bloch factor exp(2 pi i k_d) must be real: +-1, i.e. 2 k_d an integer
-        if (dtype == FD_F64 && 2.0 * kd != rint(2.0 * kd)) return FD_ERR_INVALID;
+        if (real_dtype && 2.0 * kd != rint(2.0 * kd)) return FD_ERR_INVALID;
     }
     if ((long long)shape[0] * shape[1] * shape[2] > (1LL << 40)) return FD_ERR_INVALID;
 
@@ -195,7 +196,8 @@ int fd_create_scaled(fd_plan **plan_out, const int32_t shape[3], const double h[
     p->sm_count = prop.multiProcessorCount;
     FdGeom &g = p->g;
     g.nn = nn;
-    g.cplx = (dtype == FD_C128);
+    g.cplx = (dtype == FD_C128 || dtype == FD_C64);
+    g.f32 = (dtype == FD_F32 || dtype == FD_C64);
     double c[FD_MAX_NN + 1];
     stencil_coeffs(nn, c);
     g.wdiag = 0.0;
@@ -224,6 +226,12 @@ int fd_create_scaled(fd_plan **plan_out, const int32_t shape[3], const double h[
     p->kernel = p->sweep.supported ? FD_KERNEL_SWEEP : FD_KERNEL_GENERIC;
     if (tune_value("kernel") == FD_KERNEL_GENERIC) p->kernel = FD_KERNEL_GENERIC;
     if (tune_value("kernel") != 0) p->forced = 1;
+    if (g.f32 && p->kernel != FD_KERNEL_SWEEP) {
+        // float32 / complex64 exist on the sweep kernel only (nn <= 3, whole 16-byte chunks per row,
+        // axes >= 8): no generic float kernel, and no silent fallback to another precision
+        delete p;
+        return FD_ERR_UNSUPPORTED;
+    }
     if (p->sweep.supported && fd_sweep_prepare(p) != cudaSuccess) {
         cudaGetLastError();
         delete p;
@@ -287,6 +295,7 @@ int fd_workspace_destroy(fd_workspace *ws)
 int fd_workspace_create(fd_workspace **ws_out, const fd_plan *plan, int64_t chunk_bytes)
 {
     if (!ws_out || !plan || chunk_bytes < 0) return FD_ERR_INVALID;
+    if (plan->g.f32) return FD_ERR_UNSUPPORTED;
     const int drc = check_device(plan);
     if (drc != FD_OK) return drc;
     fd_workspace *w = new (std::nothrow) fd_workspace();
@@ -322,6 +331,7 @@ int fd_apply_hamiltonian_host_ws(const fd_plan *plan, fd_workspace *ws, const vo
                                  const double *v_eff_host, void *out_host, int64_t nbands)
 {
     if (!plan || !ws || nbands < 0) return FD_ERR_INVALID;
+    if (plan->g.f32) return FD_ERR_UNSUPPORTED;
     if (nbands == 0) return FD_OK;
     if (!psi_host || !out_host) return FD_ERR_INVALID;
     const size_t P = (size_t)plan->g.n[0] * plan->g.n[1] * plan->g.n[2];
@@ -396,6 +406,7 @@ int fd_apply_hamiltonian_host(const fd_plan *plan, const void *psi_host, const d
 int64_t fd_expect_workspace_bytes(const fd_plan *plan, int64_t nbands)
 {
     if (!plan || nbands < 0) return FD_ERR_INVALID;
+    if (plan->g.f32) return FD_ERR_UNSUPPORTED;
     if (nbands == 0) return 0;
     const int64_t n = (kernel_for_batch(plan, nbands) == FD_KERNEL_SWEEP && fd_sweep_expect_fused(plan))
                           ? fd_sweep_expect_ws_bytes(plan, nbands)
@@ -407,6 +418,7 @@ int fd_apply_hamiltonian_expect(const fd_plan *plan, const void *psi, const doub
                                 double *eps, double *norm, int64_t nbands, void *workspace,
                                 int64_t workspace_bytes, void *cuda_stream)
 {
+    if (plan && plan->g.f32) return FD_ERR_UNSUPPORTED;
     const int rc = check_apply_args(plan, psi, v_eff, false, out, nbands);
     if (rc != FD_OK || nbands == 0) return rc;
     if (!eps || !norm || !workspace) return FD_ERR_INVALID;
@@ -426,6 +438,7 @@ int fd_residual(const fd_plan *plan, const void *psi, const void *hpsi, const do
                 const double *norm, void *r, int64_t nbands, void *cuda_stream)
 {
     if (!plan || nbands < 0) return FD_ERR_INVALID;
+    if (plan->g.f32) return FD_ERR_UNSUPPORTED;
     if (nbands == 0) return FD_OK;
     if (!psi || !hpsi || !eps || !norm || !r) return FD_ERR_INVALID;
     if (((uintptr_t)psi | (uintptr_t)hpsi | (uintptr_t)r) & 15) return FD_ERR_INVALID;
@@ -450,7 +463,7 @@ int fd_jacobi_sweep(const fd_plan *plan, const double *phi, const double *rhs, d
                     int64_t nbands, double omega, void *cuda_stream)
 {
     if (!plan || nbands < 0 || !isfinite(omega)) return FD_ERR_INVALID;
-    if (plan->g.cplx) return FD_ERR_UNSUPPORTED;
+    if (plan->g.cplx || plan->g.f32) return FD_ERR_UNSUPPORTED;
     if (nbands == 0) return FD_OK;
     if (!phi || !rhs || !out) return FD_ERR_INVALID;
     if (((uintptr_t)phi | (uintptr_t)rhs | (uintptr_t)out) & 15) return FD_ERR_INVALID;
@@ -508,6 +521,7 @@ int fd_paw_create(fd_paw **paw, const fd_plan *plan, int32_t natoms, const int32
                   const double *dh_host, const double *ds_host)
 {
     if (!paw || !plan || natoms < 0) return FD_ERR_INVALID;
+    if (plan->g.f32) return FD_ERR_UNSUPPORTED;
     if (natoms > 0 && (!box_start || !box_size || !nproj || !proj_host)) return FD_ERR_INVALID;
     if (!dh_host && !ds_host && natoms > 0) return FD_ERR_INVALID;
     const int drc = check_device(plan);
@@ -627,6 +641,7 @@ int fd_plan_set_kernel(fd_plan *plan, int32_t kernel, int32_t param)
 {
     if (!plan) return FD_ERR_INVALID;
     if (kernel == FD_KERNEL_GENERIC) {
+        if (plan->g.f32) return FD_ERR_UNSUPPORTED;  // no generic float32 kernel
         plan->kernel = FD_KERNEL_GENERIC;
         plan->forced = 1;
         return FD_OK;

@@ -6,12 +6,16 @@
 
 #define FD_MAX_NN 6
 
+// bytes of one element of psi / out
+inline int fd_elem_bytes(int cplx, int f32) { return (cplx ? 16 : 8) >> (f32 ? 1 : 0); }
+
 // Plan constants handed to every kernel by value.
 struct FdGeom {
     int n[3];                    // nx, ny, nz
     int bc[3];                   // FD_BC_*
     int nn;
-    int cplx;                    // 0: double, 1: complex128
+    int cplx;                    // 0: real, 1: complex data
+    int f32;                     // 0: float64 / complex128, 1: float32 / complex64 (v_eff float32)
     double w[3][FD_MAX_NN + 1];  // w[d][j] = -1/2 c_j / h_d^2
     double wdiag;                // sum_d w[d][0]
     double ph_re[3], ph_im[3];   // exp(+2 pi i k_d): factor when a tap runs past the UPPER end
@@ -89,7 +93,8 @@ FdSweepKernelFn fd_sweep_pick_real_ex(int rowd, int mode, int nn);
 FdSweepKernelFn fd_sweep_pick_real_jacobi(int rowd, int nn);
 FdSweepKernelFn fd_sweep_pick_real_ph(int mode, int nn);
 FdSweepKernelFn fd_sweep_pick_real_hi(int mode, int nn);  // nn = 4..6, float64
-FdSweepKernelFn fd_sweep_pick_cplx_hi(int mode, int nn);  // nn = 4..6, complex128 (all phase code)  // float64, Bloch factors -1 (k = 1/2)
+FdSweepKernelFn fd_sweep_pick_cplx_hi(int mode, int nn);
+FdSweepKernelFn fd_sweep_pick_f32(int cplx, int mode, int nn);  // float32 / complex64, nn = 1..3  // nn = 4..6, complex128 (all phase code)  // float64, Bloch factors -1 (k = 1/2)
 FdSweepKernelFn fd_sweep_pick_cplx_ph0(int rowd, int mode, int nn);
 FdSweepKernelFn fd_sweep_pick_cplx_ph1(int rowd, int mode, int nn);
 FdSweepKernelFn fd_sweep_pick_cplx_ph3(int rowd, int mode, int nn);

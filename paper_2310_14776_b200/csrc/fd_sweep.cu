@@ -23,11 +23,13 @@ void fd_sweep_configure(fd_plan *plan, int tyc_override, int xchunk_override, in
     if (g.nn > 3 && fd_plan_real_phase(plan)) return;  // no sign-flip instantiation for nn > 3
     const int halo = 2 * g.nn;
     if (g.n[0] < 8 || g.n[1] < 8 || g.n[2] < 8 || (g.n[2] & 1)) return;
+    if (g.f32 && (g.nn > 3 || fd_plan_real_phase(plan))) return;  // float32: nn <= 3, no sign flips
+    if (g.f32 && !g.cplx && (g.n[2] & 3)) return;                  // rows are whole 16-byte chunks
     if (g.n[0] > 65536) return;  // x index + 2 nn in 17 bits of a step-table entry
     c.ty = g.nn <= 3 ? 4 : 2;  // 2 nn + 1 accumulator planes x ty rows per thread (registers)
     c.tc = 1;
-    const int pitch = g.n[2] * (g.cplx ? 16 : 8);
-    const int pitchv = g.n[2] * 8;
+    const int pitch = g.n[2] * fd_elem_bytes(g.cplx, g.f32);
+    const int pitchv = g.n[2] * (g.f32 ? 4 : 8);
     c.lanes = (pitch / 16) / c.tc;
     if (c.lanes > kMaxThreads) return;
     c.zb_bytes = (g.bc[2] == 0) ? (c.ty * pitch + 127) / 128 * 128 : 0;
@@ -95,6 +97,7 @@ FdSweepKernelFn kernel_for(const fd_plan *plan, int mode, bool ex)
 {
     const FdGeom &g = plan->g;
     const int rowd = g.n[2] * (g.cplx ? 2 : 1);
+    if (g.f32) return (mode == 2 || ex) ? nullptr : fd_sweep_pick_f32(g.cplx, mode, g.nn);
     if (g.nn > 3) {  // plain applies only; expectation values and Jacobi fall back (fd_api.cu)
         if (mode == 2 || ex) return nullptr;
         return g.cplx ? fd_sweep_pick_cplx_hi(mode, g.nn) : fd_sweep_pick_real_hi(mode, g.nn);
@@ -183,7 +186,7 @@ cudaError_t fd_sweep_prepare(fd_plan *plan)
 // two-pass form (fd_aux.cu).
 bool fd_sweep_expect_fused(const fd_plan *plan)
 {
-    return plan->sweep.supported != 0 && !fd_plan_real_phase(plan) && plan->g.nn <= 3;
+    return plan->sweep.supported != 0 && !fd_plan_real_phase(plan) && plan->g.nn <= 3 && !plan->g.f32;
 }
 
 // Bytes of workspace fd_launch_sweep needs for the expectation values of an `nbands` batch.
@@ -208,7 +211,8 @@ cudaError_t fd_launch_sweep(const fd_plan *plan, const FdGeom &g, int mode, cons
                             double *norm, double *ws, cudaStream_t stream, int *nlaunches)
 {
     const FdSweepCfg &c = plan->sweep;
-    const long long band_d = (long long)g.n[0] * g.n[1] * g.n[2] * (g.cplx ? 2 : 1);
+    // 8-byte units per band (the kernel addresses psi / out in 8-byte units for every dtype)
+    const long long band_d = (long long)g.n[0] * g.n[1] * g.n[2] * fd_elem_bytes(g.cplx, g.f32) / 8;
     const bool ex = eps != nullptr;
     const FdSweepKernelFn kern = kernel_for(plan, mode, ex);
     if (!kern) return cudaErrorInvalidValue;

@@ -164,6 +164,36 @@ __device__ __forceinline__ double2 mul2(double w, const double2 &x)
 {
     return make_double2(w * x.x, w * x.y);
 }
+__device__ __forceinline__ float4 lds128f(const unsigned char *p)
+{
+    return *reinterpret_cast<const float4 *>(p);
+}
+__device__ __forceinline__ void fma4(float4 &a, float w, const float4 &x)
+{
+    a.x = fmaf(w, x.x, a.x);
+    a.y = fmaf(w, x.y, a.y);
+    a.z = fmaf(w, x.z, a.z);
+    a.w = fmaf(w, x.w, a.w);
+}
+// two complex64 points times one phase
+__device__ __forceinline__ float4 cmul4(const float4 &a, float pr, float pi)
+{
+    return make_float4(a.x * pr - a.y * pi, a.x * pi + a.y * pr, a.z * pr - a.w * pi, a.z * pi + a.w * pr);
+}
+template <bool F32>
+struct FdVec;
+template <>
+struct FdVec<false> {
+    typedef double2 type;
+    typedef double scalar;
+    __device__ __forceinline__ static double2 zero() { return make_double2(0.0, 0.0); }
+};
+template <>
+struct FdVec<true> {
+    typedef float4 type;
+    typedef float scalar;
+    __device__ __forceinline__ static float4 zero() { return make_float4(0.f, 0.f, 0.f, 0.f); }
+};
 __device__ __forceinline__ double2 cmul(const double2 &a, double pr, double pi)
 {
     return make_double2(a.x * pr - a.y * pi, a.x * pi + a.y * pr);
@@ -238,7 +268,10 @@ struct TeamRange {
 //   are already in the accumulator when psi_i is in registers (x: the planes that arrived before).
 //   Each warp writes one partial (eps, norm) pair per band segment; fd_expect_finalize_sweep adds
 //   them in a fixed order (deterministic, no atomics).
-template <bool CPLX, int MODE, int ROWD, int PH, int NN, bool EX>
+// F32: float32 / complex64 data: the staging, ring and step table are unchanged (rows
+//   are counted in 8-byte units); the arithmetic is a separate body on 16-byte chunks of 4 floats
+//   (4 real points or 2 complex points), fp32 accumulation.  Plain applies only (MODE 0 / 1, no EX).
+template <bool CPLX, int MODE, int ROWD, int PH, int NN, bool EX, bool F32 = false>
 __global__ void __launch_bounds__(kMaxThreads + kProducerThreads, 1)
 fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSweepCfg cfg,
                 const double *__restrict__ psi, const double *__restrict__ v_eff,
@@ -247,10 +280,14 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
 {
     constexpr bool HAS_V = MODE != 0;
     static_assert(!(CPLX && MODE == 2), "the Jacobi sweep is real only");
+    static_assert(!(F32 && (MODE == 2 || EX)), "float32: plain applies only");
+    using VT = typename FdVec<F32>::type;  // one 16-byte chunk: double2 or float4
+    using WT = typename FdVec<F32>::scalar;
     constexpr int TY = (NN <= 3) ? 4 : 2;  // rows per thread: 2 NN + 1 accumulator planes x TY rows
                                            // must fit the registers (nn = 4..6: half-height micro tile)
     constexpr int TC = 1;              // 16-byte chunks per thread per row (lane stride 16 B)
-    constexpr int ZH = CPLX ? NN : (NN + 1) / 2;   // halo chunks per side along z
+    // halo chunks per side along z (a chunk holds 2 / 1 points in double, 4 / 2 points in float)
+    constexpr int ZH = F32 ? (NN * (CPLX ? 2 : 1) + 3) / 4 : (CPLX ? NN : (NN + 1) / 2);
     constexpr int NS = 2 * NN + 1;     // in-flight output planes (accumulator slots)
     constexpr int NP = TY * TC;
 
@@ -265,7 +302,8 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
     const int K = cfg.stages;
 
     const int nx = g.n[0], ny = g.n[1], nz = g.n[2];
-    const int rowd = ROWD ? ROWD : nz * (CPLX ? 2 : 1);  // doubles per z row of psi
+    // 8-byte units per z row of psi (doubles; for F32 two floats each)
+    const int rowd = ROWD ? ROWD : (F32 ? nz * (CPLX ? 2 : 1) / 2 : nz * (CPLX ? 2 : 1));
     const int pitch = rowd * 8;                          // bytes per z row of psi
     const int pitchv = CPLX ? pitch / 2 : pitch;         // bytes per z row of v_eff
     const int cpr = rowd >> 1;                           // 16-byte chunks per row
@@ -351,7 +389,9 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
                                  v_eff + ((long long)(me.y + (unsigned)xl) * ny + y0) * nz, tx_v, bar);
                     else
                         bulk_g2s_hint(stage0 + s * stage_bytes + (uint32_t)cfg.v_off,
-                                      v_eff + ((long long)xl * ny + y0) * nz, tx_v, bar, pol);
+                                      reinterpret_cast<const unsigned char *>(v_eff) +
+                                          ((long long)xl * ny + y0) * pitchv,
+                                      tx_v, bar, pol);
                 }
                 if (mx & kKeepL2) {
                     if (per_y && nlo > 0)
@@ -426,21 +466,21 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
         if (tactive && (r0 + i) < rows_valid) row_ok |= 1u << i;
     double *const obase = out + (long long)(y0 + r0) * rowd + zc0 * 2;
 
-    double wx[NN + 1], wy[NN + 1], wz[NN + 1];  // w[j] = scale c_j / h_d^2, j = 1..NN
+    WT wx[NN + 1], wy[NN + 1], wz[NN + 1];  // w[j] = scale c_j / h_d^2, j = 1..NN
 #pragma unroll
     for (int j = 1; j <= NN; ++j) {
-        wx[j] = g.w[0][j];
-        wy[j] = g.w[1][j];
-        wz[j] = g.w[2][j];
+        wx[j] = (WT)g.w[0][j];
+        wy[j] = (WT)g.w[1][j];
+        wz[j] = (WT)g.w[2][j];
     }
-    const double wdiag = g.wdiag;
+    const WT wdiag = (WT)g.wdiag;
 
     // ---- the sweep: one flat loop over the step table ------------------------------------------
-    double2 acc[NS][NP];
+    VT acc[NS][NP];
 #pragma unroll
     for (int a = 0; a < NS; ++a)
 #pragma unroll
-        for (int p = 0; p < NP; ++p) acc[a][p] = make_double2(0.0, 0.0);
+        for (int p = 0; p < NP; ++p) acc[a][p] = FdVec<F32>::zero();
 
     // EX: this thread's share of eps / norm of the current band segment.  One chain each: more
     // chains spill at 160 registers (float64) or run slower (complex128: measured).  Rows outside the
@@ -463,8 +503,118 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
                 const unsigned char *const sb = stage0p + st * stage_bytes;
                 const unsigned char *const ub = sb + own_off;
 
-                double2 u[NP];  // float64 path: own values of the incoming plane
-                if constexpr (CPLX) {
+                VT u[NP];  // float64 / float32 paths: own values of the incoming plane
+                if constexpr (F32) {
+                    // ---- float32 / complex64: 16-byte chunk = 4 floats = 4 real or 2 complex points
+                    constexpr int ST = CPLX ? 2 : 1;  // floats per point
+                    const float pxr = (float)g.ph_re[0], pxi = (float)g.ph_im[0];
+                    const float pyr = (float)g.ph_re[1], pyi = (float)g.ph_im[1];
+                    const float pzr = (float)g.ph_re[2], pzi = (float)g.ph_im[2];
+                    if (!(m.x & kZero)) {
+#pragma unroll
+                        for (int i = 0; i < TY; ++i) {
+                            u[i] = lds128f(ub + (NN + i) * pitch);
+                            if constexpr (CPLX) {
+                                if (yhi && r0 + NN + i >= nlo + nmid) u[i] = cmul4(u[i], pyr, pyi);
+                                if (xphase && (m.x & (kWrapLo | kWrapHi)))
+                                    u[i] = cmul4(u[i], pxr, (m.x & kWrapLo) ? -pxi : pxi);
+                            }
+                        }
+                    } else {
+#pragma unroll
+                        for (int i = 0; i < TY; ++i) u[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+                    }
+                    // x taps, oldest output first: it is complete after this and leaves
+#pragma unroll
+                    for (int i = 0; i < TY; ++i) fma4(acc[(J + NN + 1) % NS][i], wx[NN], u[i]);
+                    if (m.x & kOut) {
+                        double *o = obase + (long long)(m.y + (m.x & kXMask) - 2 * NN) * plane_d;
+#pragma unroll
+                        for (int i = 0; i < TY; ++i)
+                            if (row_ok & (1u << i))
+                                __stcs(reinterpret_cast<float4 *>(o + i * rowd), acc[(J + NN + 1) % NS][i]);
+                    }
+#pragma unroll
+                    for (int i = 0; i < TY; ++i)
+#pragma unroll
+                        for (int d = 1; d < NN; ++d) {
+                            fma4(acc[(J + NS - d) % NS][i], wx[d], u[i]);
+                            fma4(acc[(J + d) % NS][i], wx[d], u[i]);
+                        }
+                    if (m.x & kCentre) {
+                        // diagonal (+ v_eff: one float per point)
+#pragma unroll
+                        for (int i = 0; i < TY; ++i) {
+                            float4 d4 = make_float4(wdiag, wdiag, wdiag, wdiag);
+                            if (HAS_V) {
+                                if constexpr (CPLX) {
+                                    const float2 vv = *reinterpret_cast<const float2 *>(sb + v_off + i * pitchv);
+                                    d4.x += vv.x; d4.y += vv.x; d4.z += vv.y; d4.w += vv.y;
+                                } else {
+                                    const float4 vv = lds128f(sb + v_off + i * pitchv);
+                                    d4.x += vv.x; d4.y += vv.y; d4.z += vv.z; d4.w += vv.w;
+                                }
+                            }
+                            acc[J][i].x = fmaf(d4.x, u[i].x, acc[J][i].x);
+                            acc[J][i].y = fmaf(d4.y, u[i].y, acc[J][i].y);
+                            acc[J][i].z = fmaf(d4.z, u[i].z, acc[J][i].z);
+                            acc[J][i].w = fmaf(d4.w, u[i].w, acc[J][i].w);
+                        }
+                        // y taps: halo rows of the thread's column
+#pragma unroll
+                        for (int rr = 0; rr < TY + 2 * NN; ++rr) {
+                            if (rr >= NN && rr < NN + TY) continue;  // own rows: already in u
+                            float4 c = lds128f(ub + rr * pitch);
+                            if constexpr (CPLX) {
+                                if (rr < NN) {
+                                    if (ylo && r0 + rr < nlo) c = cmul4(c, pyr, -pyi);
+                                } else if (yhi && r0 + rr >= nlo + nmid) {
+                                    c = cmul4(c, pyr, pyi);
+                                }
+                            }
+#pragma unroll
+                            for (int i = 0; i < TY; ++i) {
+                                const int d = rr - NN - i;
+                                const int ad = d < 0 ? -d : d;
+                                if (ad >= 1 && ad <= NN) fma4(acc[J][i], wy[ad], c);
+                            }
+                        }
+#pragma unroll
+                        for (int i = 0; i < TY; ++i)
+#pragma unroll
+                            for (int i2 = 0; i2 < TY; ++i2) {
+                                const int ad = i2 > i ? i2 - i : i - i2;
+                                if (ad >= 1 && ad <= NN) fma4(acc[J][i], wy[ad], u[i2]);
+                            }
+                        // z taps: window = ZH chunks | own chunk | ZH chunks, point stride ST floats
+#pragma unroll
+                        for (int i = 0; i < TY; ++i) {
+                            float w[4 * (2 * ZH + 1)];
+#pragma unroll
+                            for (int k = 0; k < 2 * ZH; ++k) {
+                                float4 t = lds128f(sb + hb[k] + i * pitch);
+                                if constexpr (CPLX) {
+                                    if (zphase) {
+                                        const int wbits = (zwrap >> (2 * k)) & 3;
+                                        if (wbits == 1) t = cmul4(t, pzr, -pzi);
+                                        if (wbits == 2) t = cmul4(t, pzr, pzi);
+                                    }
+                                }
+                                const int base = 4 * (k < ZH ? k : k + 1);
+                                w[base] = t.x; w[base + 1] = t.y; w[base + 2] = t.z; w[base + 3] = t.w;
+                            }
+                            w[4 * ZH] = u[i].x; w[4 * ZH + 1] = u[i].y; w[4 * ZH + 2] = u[i].z; w[4 * ZH + 3] = u[i].w;
+                            float4 &a = acc[J][i];
+#pragma unroll
+                            for (int j = 1; j <= NN; ++j) {
+                                a.x = fmaf(wz[j], w[4 * ZH + 0 - j * ST] + w[4 * ZH + 0 + j * ST], a.x);
+                                a.y = fmaf(wz[j], w[4 * ZH + 1 - j * ST] + w[4 * ZH + 1 + j * ST], a.y);
+                                a.z = fmaf(wz[j], w[4 * ZH + 2 - j * ST] + w[4 * ZH + 2 + j * ST], a.z);
+                                a.w = fmaf(wz[j], w[4 * ZH + 3 - j * ST] + w[4 * ZH + 3 + j * ST], a.w);
+                            }
+                        }
+                    }
+                } else if constexpr (CPLX) {
                     // complex128: the rows of the thread's column stream through one register
                     // pair (no copy of the own values is kept: at 168 registers that is what
                     // lets the loads run ahead; measured +8 % on cfg4, -9 % for float64)
@@ -798,8 +948,13 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
                 __syncwarp();
                 if (elect_one()) mbar_arrive(empty_bar + 8 * st);
 
-                // ---- float64 path: the output NN planes ahead is born
-                if constexpr (!CPLX) {
+                // ---- float64 / float32 paths: the output NN planes ahead is born
+                if constexpr (F32) {
+#pragma unroll
+                    for (int p = 0; p < NP; ++p)
+                        acc[(J + NN) % NS][p] = make_float4(wx[NN] * u[p].x, wx[NN] * u[p].y,
+                                                            wx[NN] * u[p].z, wx[NN] * u[p].w);
+                } else if constexpr (!CPLX) {
 #pragma unroll
                     for (int p = 0; p < NP; ++p) acc[(J + NN) % NS][p] = mul2(wx[NN], u[p]);
                 }

@@ -15,7 +15,7 @@ import os
 from typing import Optional, Sequence
 
 FD_BC_ZERO, FD_BC_PERIODIC = 0, 1
-FD_F64, FD_C128 = 0, 1
+FD_F64, FD_C128, FD_F32, FD_C64 = 0, 1, 2, 3
 FD_OK = 0
 FD_KERNEL_AUTO, FD_KERNEL_GENERIC, FD_KERNEL_SWEEP = 0, 1, 2
 

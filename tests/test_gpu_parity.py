@@ -732,3 +732,88 @@ def test_sweep_kernel_higher_orders(oracle, fd, nn):
         assert np.max(np.abs(eps.cpu().numpy() - w_eps.real)) <= parity_tol(cfg.h, nn, psi, v) * psi[0].size * np.abs(psi).max()
     finally:
         fd.fd_destroy(plan)
+
+
+# ------------------------------------------------------------------------------ f1: float32 / complex64
+
+def tol_f32(h, nn, psi, v):
+    """fp32 accumulation of the 6 nn + 2 terms with fp32-rounded weights: |err| <= gamma_n sum|w x|,
+    gamma_n = n u / (1 - n u), n = 6 nn + 4, u = 2^-24  (nn = 3: 1.3e-6; reading R18),
+    taken as 2e-6 (max|psi| S + max|v psi|), the north_star scale."""
+    return 2e-6 / 1e-12 * parity_tol(h, nn, psi.astype(np.complex128 if np.iscomplexobj(psi) else np.float64),
+                                     None if v is None else v.astype(np.float64))
+
+
+def f32_apply(fd, cfg, psi32, v32, kinetic=False, tyc=0):
+    k = cfg.k if cfg.complex else None
+    plan = fd.fd_create(cfg.shape, cfg.h, cfg.nn, cfg.bc, k, fd.FD_C64 if cfg.complex else fd.FD_F32, 0)
+    try:
+        assert fd.fd_plan_kernel_for(plan, psi32.shape[0]) == fd.FD_KERNEL_SWEEP
+        if tyc:
+            fd.fd_plan_set_kernel(plan, fd.FD_KERNEL_SWEEP, tyc)
+        d_psi = torch.from_numpy(psi32).cuda()
+        d_out = torch.full_like(d_psi, float("nan"))
+        if kinetic:
+            fd.fd_apply_kinetic(plan, d_psi, d_out)
+        else:
+            fd.fd_apply_hamiltonian(plan, d_psi, torch.from_numpy(v32).cuda(), d_out)
+        torch.cuda.synchronize()
+        return d_out.cpu().numpy()
+    finally:
+        fd.fd_destroy(plan)
+
+
+@pytest.mark.parametrize("nn", [1, 2, 3])
+def test_float32_and_complex64_sweep(oracle, fd, nn):
+    """single precision on the sweep kernel against the fp64 oracle on the same (fp32-rounded)
+    inputs: all BC mixes, ragged tiles, complex64 with Bloch phases on every axis, several teams"""
+    for bc in itertools.product((0, 1), repeat=3):
+        cfg = W.custom((10, 26, 16), (0.2, 0.23, 0.17), bc, nbands=5, nn=nn)
+        psi32, v32 = W.make_psi(cfg).astype(np.float32), W.make_veff(cfg).astype(np.float32)
+        for kin in (False, True):
+            got = f32_apply(fd, cfg, psi32, v32, kinetic=kin, tyc=8)
+            want = oracle.apply(cfg.shape, cfg.h, nn, bc, None, psi32.astype(np.float64),
+                                None if kin else v32.astype(np.float64))
+            assert got.dtype == np.float32 and np.isfinite(got).all()
+            assert np.max(np.abs(got - want)) <= tol_f32(cfg.h, nn, psi32, None if kin else v32)
+        k = tuple(kk if b else 0.0 for kk, b in zip((0.25, 0.125, -0.3), bc))
+        ck = W.custom((10, 22, 12), (0.2, 0.23, 0.17), bc, k=k, complex_=True, nbands=4, nn=nn)
+        psi64c, v32 = W.make_psi(ck).astype(np.complex64), W.make_veff(ck).astype(np.float32)
+        got = f32_apply(fd, ck, psi64c, v32, tyc=8)
+        want = oracle.apply(ck.shape, ck.h, nn, bc, k, psi64c.astype(np.complex128), v32.astype(np.float64))
+        assert got.dtype == np.complex64
+        assert np.max(np.abs(got - want)) <= tol_f32(ck.h, nn, psi64c, v32)
+    cfg = W.custom((40, 48, 64), (0.2, 0.2, 0.18), (1, 1, 0), nbands=40, nn=nn)
+    psi32, v32 = W.make_psi(cfg).astype(np.float32), W.make_veff(cfg).astype(np.float32)
+    got = f32_apply(fd, cfg, psi32, v32)
+    want = oracle.apply(cfg.shape, cfg.h, nn, cfg.bc, None, psi32.astype(np.float64), v32.astype(np.float64))
+    assert np.max(np.abs(got - want)) <= tol_f32(cfg.h, nn, psi32, v32)
+
+
+def test_float32_full_size_cfg3_grid_and_unsupported_forms(oracle, fd):
+    cfg = W.get(3).with_bands(64)
+    psi32, v32 = W.make_psi(cfg).astype(np.float32), W.make_veff(cfg).astype(np.float32)
+    got = f32_apply(fd, cfg, psi32, v32)
+    for b in (0, 63):
+        want = oracle.apply(cfg.shape, cfg.h, 3, cfg.bc, None, psi32[b:b + 1].astype(np.float64),
+                            v32.astype(np.float64))
+        assert np.max(np.abs(got[b:b + 1] - want)) <= tol_f32(cfg.h, 3, psi32, v32)
+    # the error is single-precision sized, not double-precision sized: the dtype really is fp32
+    assert np.max(np.abs(got[:1] - oracle.apply(cfg.shape, cfg.h, 3, cfg.bc, None,
+                                                 psi32[:1].astype(np.float64), v32.astype(np.float64)))) \
+        > 1e3 * parity_tol(cfg.h, 3, psi32[:1].astype(np.float64), v32.astype(np.float64))
+    for shape, nn, dt in [((8, 8, 10), 3, fd.FD_F32), ((8, 8, 9), 3, fd.FD_C64), ((12, 12, 12), 4, fd.FD_F32),
+                          ((6, 12, 12), 3, fd.FD_F32)]:
+        with pytest.raises(fd.FDError) as ei:
+            fd.fd_create(shape, (0.3,) * 3, nn, (1, 1, 1), None, dt, 0)
+        assert ei.value.status == -2
+    plan = fd.fd_create((8, 8, 8), (0.3,) * 3, 3, (1, 1, 1), None, fd.FD_F32, 0)
+    try:
+        with pytest.raises(fd.FDError) as ei:
+            fd.fd_plan_set_kernel(plan, fd.FD_KERNEL_GENERIC)
+        assert ei.value.status == -2
+        with pytest.raises(fd.FDError) as ei:
+            fd.fd_expect_workspace_bytes(plan, 4)
+        assert ei.value.status == -2
+    finally:
+        fd.fd_destroy(plan)
