@@ -60,6 +60,60 @@ __device__ __forceinline__ void stage_rows(double *dst, const double *__restrict
     }
 }
 
+// The same, asynchronously: every in-range word is an 8-byte cp.async (LDGSTS: no registers, the
+// thread goes on), zeros are stored directly; the caller commits the group and waits for it one
+// plane later, so the loads of plane t + 1 overlap the passes over plane t.
+__device__ __forceinline__ void cp_async8(double *dst, const double *src)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(
+                     static_cast<uint32_t>(__cvta_generic_to_shared(dst))),
+                 "l"(src)
+                 : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait()
+{
+    asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
+}
+__device__ __forceinline__ void cp_async16(double *dst, const double *src)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(
+                     static_cast<uint32_t>(__cvta_generic_to_shared(dst))),
+                 "l"(src)
+                 : "memory");
+}
+// pitch >= n + 2 pad: words per staged row (the caller may add slack / keep it even)
+__device__ __forceinline__ void stage_rows_async(double *dst, const double *__restrict__ plane,
+                                                 int rows, int y0, int ny, int per_y, int n, int pad,
+                                                 int per_z, int pitch)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    // 16-byte copies when every source row and every destination row start is 16-byte aligned
+    const bool vec = !(n & 1) && !(pad & 1) && !(pitch & 1) &&
+                     !(reinterpret_cast<uintptr_t>(plane) & 15);
+    for (int rr = warp; rr < rows; rr += kThreads / 32) {
+        const int y = wrap_or_zero(y0 + rr, ny, per_y);
+        double *d = dst + rr * pitch;
+        if (y < 0) {
+            for (int z = lane; z < n + 2 * pad; z += 32) d[z] = 0.0;
+            continue;
+        }
+        const double *srow = plane + (long long)y * n;
+        if (vec) {
+            for (int z = 2 * lane; z < n; z += 64) cp_async16(d + pad + z, srow + z);
+        } else {
+            for (int z = lane; z < n; z += 32) cp_async8(d + pad + z, srow + z);
+        }
+        if (lane < 2 * pad) {  // pad <= 5: one lane per halo word
+            const int zp = (lane < pad) ? lane : n + lane;          // padded index
+            const int z = wrap_or_zero(zp - pad, n, per_z);
+            if (z < 0) d[zp] = 0.0;
+            else cp_async8(d + zp, srow + z);
+        }
+    }
+}
+
 // ---------------------------------------------------------------------------------- restriction
 // blockIdx.x: coarse y tile (jt rows), blockIdx.y: chunk of ic coarse x planes, blockIdx.z: band.
 // NPT: coarse points of the swept plane per thread (point e = tid + n * kThreads of the jt x kc tile).
@@ -71,10 +125,14 @@ fd_restrict_kernel(const __grid_constant__ TGeom g, const double *__restrict__ f
     constexpr int M = 2 * P - 1;  // reach of the 1-D restriction in fine points
     extern __shared__ double sm[];
     const int nzf = g.nf[2], kc = g.nc[2];
-    const int fp = nzf + 2 * M;               // padded fine row
+    // z halo of pad >= M words per side, chosen so that the word under coarse point k sits at the even
+    // index 2 P + 2 k of the staged row (16-byte window loads in the z pass); + 4 words of slack for
+    // the window of the last run
+    const int pad = M + 1 - g.off[2];
+    const int fp = (nzf + 2 * pad + 4 + 1) & ~1;  // words per staged fine row
     const int rows = 2 * jt - 1 + 2 * M;      // fine rows staged per plane
-    double *F = sm;                           // [rows][fp]
-    double *T = sm + (size_t)rows * fp;       // [rows][kc]  z-restricted rows
+    double *F0 = sm;                          // 2 x [rows][fp]: the plane in use and the plane in flight
+    double *T = sm + 2 * (size_t)rows * fp;   // [rows][kc]  z-restricted rows
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int J0 = blockIdx.x * jt, nj = min(jt, g.nc[1] - J0);
     const int I0 = blockIdx.y * ic, ni = min(ic, g.nc[0] - I0);
@@ -104,19 +162,60 @@ fd_restrict_kernel(const __grid_constant__ TGeom g, const double *__restrict__ f
 #pragma unroll
         for (int n = 0; n < NPT; ++n) acc[a][n] = 0.0;
 
-    // y-z restriction of fine plane xf (already wrapped into range) into s[] for the owned points
-    auto plane = [&](int xf, double (&s)[NPT]) {
-        __syncthreads();  // the previous plane's T / F are no longer read
-        stage_rows(F, fb + (long long)xf * g.nf[1] * nzf, rows, yf0, g.nf[1], g.bc[1], nzf, M, g.bc[2]);
-        __syncthreads();
+    // The planes the sweep consumes, in order: step t = 2 (c - c0) + phase, phase 0 = the odd plane
+    // d = 2c + 1, phase 1 = the even plane d = 2c + 2 (used only when coarse c + 1 is in the chunk).
+    const int c0 = I0 - P, nsteps = 2 * (ni + 2 * P - 1);
+    auto plane_of = [&](int t) -> int {  // fine x index of step t, or -1 when the step has no plane
+        const int c = c0 + (t >> 1);
+        if ((t & 1) && !(c + 1 >= I0 && c + 1 < I0 + ni)) return -1;
+        return wrap_or_zero(2 * c + 1 + (t & 1) + g.off[0], g.nf[0], g.bc[0]);
+    };
+    auto next_plane = [&](int t) -> int {  // first step after t that has a plane (nsteps: none)
+        for (++t; t < nsteps && plane_of(t) < 0; ++t) {
+        }
+        return t;
+    };
+    auto issue = [&](int t, int buf) {
+        stage_rows_async(F0 + (size_t)buf * rows * fp, fb + (long long)plane_of(t) * g.nf[1] * nzf, rows,
+                         yf0, g.nf[1], g.bc[1], nzf, pad, g.bc[2], fp);
+        cp_async_commit();
+    };
+    int t_next = next_plane(-1), buf = 0;  // the plane in flight into F0[buf]
+    if (t_next < nsteps) issue(t_next, 0);
+
+    // y-z restriction of the next plane of the sequence into s[] for the owned points
+    auto plane = [&](double (&s)[NPT]) {
+        const double *F = F0 + (size_t)buf * rows * fp;
+        const int t_after = next_plane(t_next);
+        if (t_after < nsteps) {  // F0[buf ^ 1] was last read before the previous plane's second barrier
+            issue(t_after, buf ^ 1);
+            cp_async_wait<1>();
+        } else {
+            cp_async_wait<0>();
+        }
+        t_next = t_after;
+        buf ^= 1;
+        __syncthreads();  // this plane has landed for every thread; the previous T is no longer read
+        // z pass: a lane takes runs of 3 adjacent coarse points; their 4 P + 4 fine words start at the
+        // even word 2 k0 of the staged row: 2 P + 2 conflict-free 16-byte loads for 3 outputs
         for (int rr = warp; rr < rows; rr += kThreads / 32) {
-            const double *row = F + rr * fp + M + oz;
-            for (int k = lane; k < kc; k += 32) {
-                double t = r[0] * row[2 * k];
+            const double *row = F + rr * fp;
+            for (int k0 = 3 * lane; k0 < kc; k0 += 96) {
+                double win[4 * P + 4];
 #pragma unroll
-                for (int j = 1; j <= P; ++j)
-                    t = fma(r[j], row[2 * k - (2 * j - 1)] + row[2 * k + (2 * j - 1)], t);
-                T[rr * kc + k] = t;
+                for (int i = 0; i < 2 * P + 2; ++i) {
+                    const double2 w2 = *reinterpret_cast<const double2 *>(row + 2 * k0 + 2 * i);
+                    win[2 * i] = w2.x;
+                    win[2 * i + 1] = w2.y;
+                }
+#pragma unroll
+                for (int q = 0; q < 3; ++q) {
+                    double t = r[0] * win[2 * P + 2 * q];
+#pragma unroll
+                    for (int j = 1; j <= P; ++j)
+                        t = fma(r[j], win[2 * P + 2 * q - (2 * j - 1)] + win[2 * P + 2 * q + (2 * j - 1)], t);
+                    if (k0 + q < kc) T[rr * kc + k0 + q] = t;
+                }
             }
         }
         __syncthreads();
@@ -136,9 +235,8 @@ fd_restrict_kernel(const __grid_constant__ TGeom g, const double *__restrict__ f
     for (int c = I0 - P; c <= I0 + ni + P - 2; ++c) {
         double s[NPT];
         {
-            const int xf = wrap_or_zero(2 * c + 1 + g.off[0], g.nf[0], g.bc[0]);
-            if (xf >= 0) {
-                plane(xf, s);
+            if (plane_of(2 * (c - c0)) >= 0) {
+                plane(s);
 #pragma unroll
                 for (int j = 1; j <= P; ++j)
 #pragma unroll
@@ -162,13 +260,10 @@ fd_restrict_kernel(const __grid_constant__ TGeom g, const double *__restrict__ f
 #pragma unroll
         for (int n = 0; n < NPT; ++n) acc[2 * P - 1][n] = 0.0;
         // even plane on coarse c + 1 (slot P - 1 after the shift)
-        if (c + 1 >= I0 && c + 1 < I0 + ni) {
-            const int xf = wrap_or_zero(2 * c + 2 + g.off[0], g.nf[0], g.bc[0]);
-            if (xf >= 0) {
-                plane(xf, s);
+        if (plane_of(2 * (c - c0) + 1) >= 0) {
+            plane(s);
 #pragma unroll
-                for (int n = 0; n < NPT; ++n) acc[P - 1][n] = fma(r[0], s[n], acc[P - 1][n]);
-            }
+            for (int n = 0; n < NPT; ++n) acc[P - 1][n] = fma(r[0], s[n], acc[P - 1][n]);
         }
     }
 }
@@ -186,8 +281,8 @@ fd_interp_kernel(const __grid_constant__ TGeom g, const double *__restrict__ coa
     const int nzf = g.nf[2], kc = g.nc[2];
     const int cp = kc + 2 * P;                // padded coarse row
     const int rows = jt + 2 * P;              // coarse rows staged per plane: J0 - P .. J0 + jt + P - 1
-    double *C = sm;                           // [rows][cp]
-    double *T = sm + (size_t)rows * cp;       // [rows][nzf]  z-interpolated rows
+    double *C0 = sm;                          // 2 x [rows][cp]: the plane in use and the plane in flight
+    double *T = sm + 2 * (size_t)rows * cp;   // [rows][nzf]  z-interpolated rows
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int J0 = blockIdx.x * jt, nj = min(jt, g.nc[1] - J0);
     const int I0 = blockIdx.y * ic, ni = min(ic, g.nc[0] - I0);
@@ -226,9 +321,35 @@ fd_interp_kernel(const __grid_constant__ TGeom g, const double *__restrict__ coa
 #pragma unroll
         for (int n = 0; n < NPT; ++n) sq[a][n] = 0.0;
 
-    auto plane = [&](int xc, double (&s)[NPT]) {
-        __syncthreads();
-        stage_rows(C, cb + (long long)xc * g.nc[1] * kc, rows, J0 - P, g.nc[1], g.bc[1], kc, P, g.bc[2]);
+    // the chunk owns the even planes e_x = 2 i, i in [I0, I0 + ni), and the odd planes e_x = 2 c + 1,
+    // c in [c_first, I0 + ni): c_first = -1 for the first chunk on a zero-BC axis (the wall), else I0
+    const int c_first = (I0 == 0 && ox == 1) ? -1 : I0;
+    const int i_lo = c_first + 1 - P, i_hi = I0 + ni - 1 + P;  // coarse planes the sweep brings in
+    auto next_plane = [&](int i) -> int {  // first plane after i that exists (i_hi + 1: none)
+        for (++i; i <= i_hi && wrap_or_zero(i, g.nc[0], g.bc[0]) < 0; ++i) {
+        }
+        return i;
+    };
+    auto issue = [&](int i, int buf) {
+        stage_rows_async(C0 + (size_t)buf * rows * cp,
+                         cb + (long long)wrap_or_zero(i, g.nc[0], g.bc[0]) * g.nc[1] * kc, rows, J0 - P,
+                         g.nc[1], g.bc[1], kc, P, g.bc[2], cp);
+        cp_async_commit();
+    };
+    int i_next = next_plane(i_lo - 1), buf = 0;
+    if (i_next <= i_hi) issue(i_next, 0);
+
+    auto plane = [&](double (&s)[NPT]) {
+        const double *C = C0 + (size_t)buf * rows * cp;
+        const int i_after = next_plane(i_next);
+        if (i_after <= i_hi) {
+            issue(i_after, buf ^ 1);
+            cp_async_wait<1>();
+        } else {
+            cp_async_wait<0>();
+        }
+        i_next = i_after;
+        buf ^= 1;
         __syncthreads();
         for (int rr = warp; rr < rows; rr += kThreads / 32) {
             const double *row = C + rr * cp + P;
@@ -269,14 +390,11 @@ fd_interp_kernel(const __grid_constant__ TGeom g, const double *__restrict__ coa
             if (foff[n] >= 0) __stcs(fpx + foff[n], s[n]);
     };
 
-    // the chunk owns the even planes e_x = 2 i, i in [I0, I0 + ni), and the odd planes e_x = 2 c + 1,
-    // c in [c_first, I0 + ni): c_first = -1 for the first chunk on a zero-BC axis (the wall), else I0
-    const int c_first = (I0 == 0 && ox == 1) ? -1 : I0;
-    for (int i = c_first + 1 - P; i <= I0 + ni - 1 + P; ++i) {
+    for (int i = i_lo; i <= i_hi; ++i) {
         double s[NPT];
         const int xc = wrap_or_zero(i, g.nc[0], g.bc[0]);
         if (xc >= 0) {
-            plane(xc, s);
+            plane(s);
         } else {
 #pragma unroll
             for (int n = 0; n < NPT; ++n) s[n] = 0.0;
@@ -396,9 +514,10 @@ cudaError_t launch(bool interp, const TGeom &g, const double *src, double *dst, 
     if (pts > kThreads * kMaxPt) return cudaErrorInvalidConfiguration;
     size_t smem;
     if (interp)
-        smem = sizeof(double) * ((size_t)(jt + 2 * P) * (g.nc[2] + 2 * P) + (size_t)(jt + 2 * P) * g.nf[2]);
+        smem = sizeof(double) * ((size_t)(jt + 2 * P) * 2 * (g.nc[2] + 2 * P) + (size_t)(jt + 2 * P) * g.nf[2]);
     else
-        smem = sizeof(double) * (size_t)(2 * jt - 1 + 2 * (2 * P - 1)) * (g.nf[2] + 2 * (2 * P - 1) + g.nc[2]);
+        smem = sizeof(double) * (size_t)(2 * jt - 1 + 2 * (2 * P - 1)) *
+               (2 * (size_t)((g.nf[2] + 2 * (2 * P - g.off[2]) + 5) & ~1) + g.nc[2]);
     if (smem > (size_t)kFdSweepSmemMax) return cudaErrorInvalidConfiguration;
     const int npt = (pts + kThreads - 1) / kThreads;
     if (npt <= 1) return launch_npt<P, 1>(interp, g, src, dst, nbands, jt, ic, smem, stream);
