@@ -114,10 +114,13 @@ fd_paw_project_kernel(const PawAtom *__restrict__ atoms, const int *__restrict__
         Acc<CPLX> acc[NB];
 #pragma unroll
         for (int b = 0; b < NB; ++b) acc[b].zero();
+        // dropped points (zero-BC clipping) take weight 0 at a valid address: no branch in the loop, so
+        // the unrolled iterations keep several gathers in flight (the loop is latency bound otherwise)
+#pragma unroll 4
         for (int r = lane; r < at.npts; r += 32) {
-            const int gi = ix[r];
-            if (gi < 0) continue;
-            const double w = p[r];
+            const int gr = ix[r];
+            const int gi = gr < 0 ? 0 : gr;
+            const double w = gr < 0 ? 0.0 : p[r];
             if constexpr (CPLX) {
                 double pr = 1.0, pi = 0.0;
                 if (code) phase_of(code[at.idx_off + r], ph, pr, pi);
@@ -189,6 +192,7 @@ fd_paw_add_kernel(const PawAtom *__restrict__ atoms, const int *__restrict__ col
         double sx[NB], sy[NB];
 #pragma unroll
         for (int b = 0; b < NB; ++b) sx[b] = sy[b] = 0.0;
+#pragma unroll 4
         for (int i = 0; i < at.ni; ++i) {
             const double w = proj[at.proj_off + (long long)i * at.npts + r];
 #pragma unroll
