@@ -159,7 +159,7 @@ FD_API int fd_apply_hamiltonian_host_ws(const fd_plan *plan, fd_workspace *ws, c
  *     eps[b]  = Re sum_i conj(psi_b[i]) (H psi)_b[i]     (H is Hermitian: the imaginary part is zero)
  *     norm[b] = sum_i |psi_b[i]|^2                         (plain grid sums; x h_x h_y h_z = integrals)
  *   eps, norm   device pointers, double [nbands]
- *   workspace   device pointer, 8-byte aligned, >= fd_expect_workspace_bytes(plan, nbands) bytes,
+ *   workspace   device pointer, 16-byte aligned, >= fd_expect_workspace_bytes(plan, nbands) bytes,
  *               owned by the caller, scratch (per-warp partial sums; reduced in a fixed order by a
  *               second small launch: results are bit-reproducible run to run, no atomics)
  *   Other arguments and errors as fd_apply_hamiltonian; FD_ERR_INVALID also for a short workspace,

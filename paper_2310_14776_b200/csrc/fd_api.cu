@@ -422,7 +422,7 @@ int fd_apply_hamiltonian_expect(const fd_plan *plan, const void *psi, const doub
     const int rc = check_apply_args(plan, psi, v_eff, false, out, nbands);
     if (rc != FD_OK || nbands == 0) return rc;
     if (!eps || !norm || !workspace) return FD_ERR_INVALID;
-    if (((uintptr_t)eps | (uintptr_t)norm | (uintptr_t)workspace) & 7) return FD_ERR_INVALID;
+    if ((((uintptr_t)eps | (uintptr_t)norm) & 7) || ((uintptr_t)workspace & 15)) return FD_ERR_INVALID;
     if (workspace_bytes < fd_expect_workspace_bytes(plan, nbands)) return FD_ERR_INVALID;
     const size_t nb = (size_t)plan->g.n[0] * plan->g.n[1] * plan->g.n[2] * (size_t)nbands *
                       (plan->g.cplx ? 16 : 8);

@@ -7,8 +7,9 @@
 // are whatever the caller supplies (synthetic in tests and bench).
 //
 // Two kernels.  project: gather psi over each atom's box (an index table built at fd_paw_create
-// resolves wrap / zero-BC clipping once), P_b[a,i] = dv sum_r p~_i(r) psi^_b(r); one warp per
-// projector function, lanes over box points, fixed-order warp reduction (deterministic).
+// resolves wrap / zero-BC clipping once), P_b[a,i] = dv sum_r p~_i(r) psi^_b(r); one warp per 4 bands
+// of an atom, lanes over box points, 8 projector functions at a time in registers, fixed-order warp
+// reduction (deterministic).
 // add: out_b(r) += conj(phase) sum_i p~_i(r) (dO P_b)_i, one thread per box point; atoms are greedily
 // coloured at create so that the boxes of one launch are disjoint: plain read-modify-write, no
 // atomics, results independent of scheduling.
@@ -97,8 +98,12 @@ __device__ __forceinline__ void phase_of(unsigned code, const Phases &ph, double
         }
 }
 
-// grid (atoms, band tiles); coef[b][coef_off + i] = dv sum_r p~_i(r) psi^_b(r)
-template <bool CPLX, int NB>
+// grid (atoms, tiles of 8 NB bands); coef[b][coef_off + i] = dv sum_r p~_i(r) psi^_b(r).
+// A warp owns NB bands of the atom: lanes run over the box points, every lane keeps NI x NB partial
+// sums (psi is gathered once per point and meets NI projector values), projector functions go by
+// in chunks of NI; fixed shuffle tree at the end of a chunk.  The 8 warps of a CTA share the atom's
+// projector values through L1.
+template <bool CPLX, int NB, int NI>
 __global__ void __launch_bounds__(kPawThreads)
 fd_paw_project_kernel(const PawAtom *__restrict__ atoms, const int *__restrict__ idx,
                       const unsigned char *__restrict__ code, const double *__restrict__ proj,
@@ -106,50 +111,65 @@ fd_paw_project_kernel(const PawAtom *__restrict__ atoms, const int *__restrict__
                       long long nbands, int ntot, double dv, const Phases ph)
 {
     const PawAtom at = atoms[blockIdx.x];
-    const long long b0 = (long long)blockIdx.y * NB;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const long long b0 = ((long long)blockIdx.y * (kPawThreads / 32) + warp) * NB;
+    if (b0 >= nbands) return;
     const int *ix = idx + at.idx_off;
-    for (int i = warp; i < at.ni; i += kPawThreads / 32) {
-        const double *p = proj + at.proj_off + (long long)i * at.npts;
-        Acc<CPLX> acc[NB];
+    const double *pb[NB];
 #pragma unroll
-        for (int b = 0; b < NB; ++b) acc[b].zero();
-        // dropped points (zero-BC clipping) take weight 0 at a valid address: no branch in the loop, so
-        // the unrolled iterations keep several gathers in flight (the loop is latency bound otherwise)
-#pragma unroll 4
+    for (int b = 0; b < NB; ++b)  // bands past the end re-read the last one and are not written
+        pb[b] = psi + ((b0 + b < nbands) ? (b0 + b) : (nbands - 1)) * band_d;
+    for (int i0 = 0; i0 < at.ni; i0 += NI) {
+        const double *p = proj + at.proj_off + (long long)i0 * at.npts;
+        Acc<CPLX> acc[NI][NB];
+#pragma unroll
+        for (int i = 0; i < NI; ++i)
+#pragma unroll
+            for (int b = 0; b < NB; ++b) acc[i][b].zero();
+        // dropped points (zero-BC clipping) take weight 0 at a valid address: no branch in the loop
+#pragma unroll 2
         for (int r = lane; r < at.npts; r += 32) {
             const int gr = ix[r];
             const int gi = gr < 0 ? 0 : gr;
-            const double w = gr < 0 ? 0.0 : p[r];
+            Acc<CPLX> v[NB];
             if constexpr (CPLX) {
                 double pr = 1.0, pi = 0.0;
                 if (code) phase_of(code[at.idx_off + r], ph, pr, pi);
 #pragma unroll
-                for (int b = 0; b < NB; ++b)
-                    if (b0 + b < nbands) {
-                        const double2 v = *reinterpret_cast<const double2 *>(psi + (b0 + b) * band_d + 2LL * gi);
-                        acc[b].x = fma(w, v.x * pr - v.y * pi, acc[b].x);
-                        acc[b].y = fma(w, v.x * pi + v.y * pr, acc[b].y);
-                    }
+                for (int b = 0; b < NB; ++b) {
+                    const double2 t = *reinterpret_cast<const double2 *>(pb[b] + 2LL * gi);
+                    v[b].x = t.x * pr - t.y * pi;
+                    v[b].y = t.x * pi + t.y * pr;
+                }
             } else {
 #pragma unroll
-                for (int b = 0; b < NB; ++b)
-                    if (b0 + b < nbands) acc[b].x = fma(w, psi[(b0 + b) * band_d + gi], acc[b].x);
+                for (int b = 0; b < NB; ++b) v[b].x = pb[b][gi];
             }
-        }
 #pragma unroll
-        for (int b = 0; b < NB; ++b) {
-            acc[b].reduce();
-            if (lane == 0 && b0 + b < nbands) {
-                double *c = coef + ((b0 + b) * ntot + at.coef_off + i) * (CPLX ? 2 : 1);
-                if constexpr (CPLX) {
-                    c[0] = dv * (acc[b].x * at.ph0_re - acc[b].y * at.ph0_im);
-                    c[1] = dv * (acc[b].x * at.ph0_im + acc[b].y * at.ph0_re);
-                } else {
-                    c[0] = dv * acc[b].x;
+            for (int i = 0; i < NI; ++i) {
+                const double w = (gr < 0 || i0 + i >= at.ni) ? 0.0 : p[(long long)i * at.npts + r];
+#pragma unroll
+                for (int b = 0; b < NB; ++b) {
+                    acc[i][b].x = fma(w, v[b].x, acc[i][b].x);
+                    if constexpr (CPLX) acc[i][b].y = fma(w, v[b].y, acc[i][b].y);
                 }
             }
         }
+#pragma unroll
+        for (int i = 0; i < NI; ++i)
+#pragma unroll
+            for (int b = 0; b < NB; ++b) {
+                acc[i][b].reduce();
+                if (lane == 0 && i0 + i < at.ni && b0 + b < nbands) {
+                    double *c = coef + ((b0 + b) * ntot + at.coef_off + i0 + i) * (CPLX ? 2 : 1);
+                    if constexpr (CPLX) {
+                        c[0] = dv * (acc[i][b].x * at.ph0_re - acc[i][b].y * at.ph0_im);
+                        c[1] = dv * (acc[i][b].x * at.ph0_im + acc[i][b].y * at.ph0_re);
+                    } else {
+                        c[0] = dv * acc[i][b].x;
+                    }
+                }
+            }
     }
 }
 
@@ -188,7 +208,7 @@ fd_paw_add_kernel(const PawAtom *__restrict__ atoms, const int *__restrict__ col
     const int *ix = idx + at.idx_off;
     for (int r = threadIdx.x; r < at.npts; r += kPawThreads) {
         const int gi = ix[r];
-        if (gi < 0) continue;
+        if (gi < 0) continue;  // dropped by zero-BC clipping
         double sx[NB], sy[NB];
 #pragma unroll
         for (int b = 0; b < NB; ++b) sx[b] = sy[b] = 0.0;
@@ -402,17 +422,17 @@ cudaError_t fd_paw_launch_project(const fd_paw *w, const void *psi, void *coef, 
         ph.im[d] = w->ph_im[d];
     }
     const long long band_d = (long long)w->npoints * (w->cplx ? 2 : 1);
-    const int NB = w->cplx ? 2 : 4;
-    for (int64_t b0 = 0; b0 < nbands; b0 += 65535LL * NB) {
-        const int64_t nb = (nbands - b0 < 65535LL * NB) ? nbands - b0 : 65535LL * NB;
-        const dim3 grid((unsigned)w->natoms, (unsigned)((nb + NB - 1) / NB));
+    const int tile = (w->cplx ? 2 : 4) * (kPawThreads / 32);  // bands per CTA
+    for (int64_t b0 = 0; b0 < nbands; b0 += 65535LL * tile) {
+        const int64_t nb = (nbands - b0 < 65535LL * tile) ? nbands - b0 : 65535LL * tile;
+        const dim3 grid((unsigned)w->natoms, (unsigned)((nb + tile - 1) / tile));
         const double *p = static_cast<const double *>(psi) + b0 * band_d;
         double *c = static_cast<double *>(coef) + b0 * w->ntot * (w->cplx ? 2 : 1);
         if (w->cplx)
-            fd_paw_project_kernel<true, 2><<<grid, kPawThreads, 0, stream>>>(
+            fd_paw_project_kernel<true, 2, 8><<<grid, kPawThreads, 0, stream>>>(
                 w->atoms, w->idx, w->code, w->proj, p, c, band_d, nb, w->ntot, w->dv, ph);
         else
-            fd_paw_project_kernel<false, 4><<<grid, kPawThreads, 0, stream>>>(
+            fd_paw_project_kernel<false, 4, 8><<<grid, kPawThreads, 0, stream>>>(
                 w->atoms, w->idx, w->code, w->proj, p, c, band_d, nb, w->ntot, w->dv, ph);
         cudaError_t e = cudaPeekAtLastError();
         if (e != cudaSuccess) return e;

@@ -141,25 +141,36 @@ long long team_quota(const fd_plan *plan, long long total)
 int64_t bands_per_launch(const fd_plan *plan) { return (1LL << kPlaneBits) / plan->g.n[0]; }
 
 // Sums the per-warp partials of the EX sweep kernel (layout: FdSweepAux) band by band in a fixed
-// order: team by team, y tile by y tile, warp by warp.  One thread per band.
+// order.  One warp per band: lane l adds the entries l, l + 32, ... of each team's block in order,
+// then a fixed shuffle tree: the same association every run, no atomics.
 __global__ void fd_expect_finalize_sweep(const double *__restrict__ ws, double *__restrict__ eps,
                                          double *__restrict__ norm, int nbands, int nx,
                                          long long quota, int maxseg, int nytiles, int nwarps)
 {
-    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    const int b = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    const int lane = threadIdx.x & 31;
     if (b >= nbands) return;
     const long long l_lo = (long long)b * nx, l_hi = l_lo + nx - 1;
     double e = 0.0, n = 0.0;
     for (long long t = l_lo / quota; t <= l_hi / quota; ++t) {
         const long long seg = b - (t * quota) / nx;  // this band's segment index inside team t
-        const double *w = ws + 2 * ((t * maxseg + seg) * nytiles) * (long long)nwarps;
-        for (int i = 0; i < nytiles * nwarps; ++i) {
-            e += w[2 * i];
-            n += w[2 * i + 1];
+        const double2 *w = reinterpret_cast<const double2 *>(ws) +
+                           ((t * maxseg + seg) * nytiles) * (long long)nwarps;
+        for (int i = lane; i < nytiles * nwarps; i += 32) {
+            const double2 v = w[i];
+            e += v.x;
+            n += v.y;
         }
     }
-    eps[b] = e;
-    norm[b] = n;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        e += __shfl_xor_sync(0xffffffffu, e, o);
+        n += __shfl_xor_sync(0xffffffffu, n, o);
+    }
+    if (lane == 0) {
+        eps[b] = e;
+        norm[b] = n;
+    }
 }
 
 }  // namespace
@@ -237,7 +248,7 @@ cudaError_t fd_launch_sweep(const fd_plan *plan, const FdGeom &g, int mode, cons
         if (e != cudaSuccess) return e;
         if (nlaunches) ++*nlaunches;
         if (ex) {
-            fd_expect_finalize_sweep<<<dim3((unsigned)((nb + 127) / 128)), dim3(128), 0, stream>>>(
+            fd_expect_finalize_sweep<<<dim3((unsigned)((nb + 3) / 4)), dim3(128), 0, stream>>>(
                 ws, eps + b0, norm + b0, (int)nb, g.n[0], quota, aux.maxseg, c.nytiles,
                 c.threads / 32);
             e = cudaPeekAtLastError();
