@@ -272,12 +272,16 @@ FD_API const char *fd_strerror(int status);
  *   to fill its persistent CTAs to the generic kernel unless it was forced).
  * fd_plan_kernel_for: family an apply of `nbands` bands will launch.
  * fd_plan_launches: kernels launched by this plan so far (for bench.py's gpu_launches).
- * fd_plan_get_weights: the 3*(nn+1) doubles w_d[j] = -1/2 c_j / h_d^2 (d-major) the kernels use. */
+ * fd_plan_get_weights: the 3*(nn+1) doubles w_d[j] = -1/2 c_j / h_d^2 (d-major) the kernels use.
+ * fd_plan_get_info: info[0..2] = nx, ny, nz; [3] = nn; [4] = dtype (FD_F64 ...); [5] = device;
+ *   [6] = bc bits (x | y << 1 | z << 2); [7] = kernel family.  Lets a binding check the arrays it is
+ *   handed against the plan before it passes raw pointers on. */
 FD_API int fd_plan_set_kernel(fd_plan *plan, int32_t kernel, int32_t param);
 FD_API int fd_plan_get_kernel(const fd_plan *plan);
 FD_API int fd_plan_kernel_for(const fd_plan *plan, int64_t nbands);
 FD_API int64_t fd_plan_launches(const fd_plan *plan);
 FD_API int fd_plan_get_weights(const fd_plan *plan, double *w, int32_t capacity);
+FD_API int fd_plan_get_info(const fd_plan *plan, int32_t info[8]);
 
 #ifdef __cplusplus
 }

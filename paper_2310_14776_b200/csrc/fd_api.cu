@@ -668,6 +668,21 @@ int fd_plan_set_kernel(fd_plan *plan, int32_t kernel, int32_t param)
 
 int fd_plan_get_kernel(const fd_plan *plan) { return plan ? plan->kernel : FD_ERR_INVALID; }
 
+int fd_plan_get_info(const fd_plan *plan, int32_t info[8])
+{
+    if (!plan || !info) return FD_ERR_INVALID;
+    const FdGeom &g = plan->g;
+    info[0] = g.n[0];
+    info[1] = g.n[1];
+    info[2] = g.n[2];
+    info[3] = g.nn;
+    info[4] = g.f32 ? (g.cplx ? FD_C64 : FD_F32) : (g.cplx ? FD_C128 : FD_F64);
+    info[5] = plan->device;
+    info[6] = g.bc[0] | (g.bc[1] << 1) | (g.bc[2] << 2);
+    info[7] = plan->kernel;
+    return FD_OK;
+}
+
 int fd_plan_kernel_for(const fd_plan *plan, int64_t nbands)
 {
     if (!plan || nbands < 0) return FD_ERR_INVALID;

@@ -30,7 +30,7 @@ EXPORTED_SYMBOLS = [
     "fd_paw_create", "fd_paw_destroy", "fd_paw_nproj_total", "fd_paw_project", "fd_paw_add_nonlocal",
     "fd_apply_hamiltonian_paw", "fd_apply_overlap",
     "fd_destroy", "fd_strerror", "fd_plan_set_kernel", "fd_plan_get_kernel", "fd_plan_kernel_for", "fd_plan_launches",
-    "fd_plan_get_weights",
+    "fd_plan_get_weights", "fd_plan_get_info",
 ]
 
 
@@ -112,6 +112,8 @@ def load_library() -> ctypes.CDLL:
     lib.fd_plan_launches.restype = ctypes.c_int64
     lib.fd_plan_get_weights.argtypes = [vp, f64p, i32]
     lib.fd_plan_get_weights.restype = ctypes.c_int
+    lib.fd_plan_get_info.argtypes = [vp, i32p]
+    lib.fd_plan_get_info.restype = ctypes.c_int
     _lib = lib
     return lib
 
@@ -173,8 +175,54 @@ def _dev_ptr(t) -> ctypes.c_void_p:
     return ctypes.c_void_p(t.data_ptr())
 
 
+def fd_plan_get_info(plan) -> dict:
+    """shape, nn, dtype, device, bc and kernel family of a plan (include/fdham.h)."""
+    buf = (ctypes.c_int32 * 8)()
+    _check(load_library().fd_plan_get_info(plan, buf), "fd_plan_get_info")
+    return {"shape": (buf[0], buf[1], buf[2]), "nn": buf[3], "dtype": buf[4], "device": buf[5],
+            "bc": (buf[6] & 1, (buf[6] >> 1) & 1, (buf[6] >> 2) & 1), "kernel": buf[7]}
+
+
+def _torch_dtypes(dtype: int):
+    """(torch dtype of psi / out, torch dtype of v_eff) for an FD_* dtype."""
+    import torch
+    return {FD_F64: (torch.float64, torch.float64), FD_C128: (torch.complex128, torch.float64),
+            FD_F32: (torch.float32, torch.float32), FD_C64: (torch.complex64, torch.float32)}[dtype]
+
+
+def _check_arrays(plan, where: str, batch=(), grid=(), real=()):
+    """The C ABI takes raw pointers: a tensor of the wrong shape, dtype or device would become an
+    out-of-bounds access on the device, so the binding checks them against the plan first.
+    batch: tensors [nbands, nx, ny, nz] of the plan's dtype (same nbands); grid: [nx, ny, nz] of the
+    plan's real dtype; real: batch-shaped tensors of the plan's real dtype."""
+    info = fd_plan_get_info(plan)
+    shape, (tdt, rdt) = tuple(info["shape"]), _torch_dtypes(info["dtype"])
+    nb = None
+    for kind, tensors, want_dt in (("batch", batch, tdt), ("real", real, rdt)):
+        for t in tensors:
+            if t is None:
+                continue
+            if t.dim() != 4 or tuple(t.shape[1:]) != shape:
+                raise ValueError(f"{where}: expected [nbands, {shape}], got {tuple(t.shape)}")
+            if t.dtype != want_dt:
+                raise ValueError(f"{where}: expected dtype {want_dt}, got {t.dtype}")
+            if nb is not None and t.shape[0] != nb:
+                raise ValueError(f"{where}: band counts differ ({t.shape[0]} vs {nb})")
+            nb = t.shape[0]
+            if t.device.index != info["device"]:
+                raise ValueError(f"{where}: tensor on cuda:{t.device.index}, plan on cuda:{info['device']}")
+    for t in grid:
+        if t is None:
+            continue
+        if tuple(t.shape) != shape or t.dtype != rdt:
+            raise ValueError(f"{where}: v_eff must be {rdt} {shape}, got {t.dtype} {tuple(t.shape)}")
+        if t.device.index != info["device"]:
+            raise ValueError(f"{where}: tensor on cuda:{t.device.index}, plan on cuda:{info['device']}")
+
+
 def fd_apply_kinetic(plan, psi, out, stream=None) -> None:
     """out = T psi for torch CUDA tensors psi/out [nbands,nx,ny,nz] (float64 or complex128)."""
+    _check_arrays(plan, "fd_apply_kinetic", batch=(psi, out))
     rc = load_library().fd_apply_kinetic(plan, _dev_ptr(psi), _dev_ptr(out), int(psi.shape[0]),
                                          _stream_ptr(stream))
     _check(rc, "fd_apply_kinetic")
@@ -182,6 +230,7 @@ def fd_apply_kinetic(plan, psi, out, stream=None) -> None:
 
 def fd_apply_hamiltonian(plan, psi, v_eff, out, stream=None) -> None:
     """out = T psi + v_eff psi; v_eff is a float64 CUDA tensor [nx,ny,nz]."""
+    _check_arrays(plan, "fd_apply_hamiltonian", batch=(psi, out), grid=(v_eff,))
     rc = load_library().fd_apply_hamiltonian(plan, _dev_ptr(psi), _dev_ptr(v_eff), _dev_ptr(out),
                                              int(psi.shape[0]), _stream_ptr(stream))
     _check(rc, "fd_apply_hamiltonian")
@@ -238,6 +287,10 @@ def fd_apply_hamiltonian_expect(plan, psi, v_eff, out, eps, norm, workspace, str
     """out = H psi (v_eff None: T psi), eps[b] = Re <psi_b|H psi_b>, norm[b] = <psi_b|psi_b> (grid
     sums) in one pass; eps/norm float64 CUDA tensors [nbands], workspace a CUDA byte/float64 tensor
     of at least fd_expect_workspace_bytes(plan, nbands) bytes."""
+    _check_arrays(plan, "fd_apply_hamiltonian_expect", batch=(psi, out), grid=(v_eff,))
+    for name, t in (("eps", eps), ("norm", norm)):
+        if tuple(t.shape) != (psi.shape[0],) or str(t.dtype) != "torch.float64":
+            raise ValueError(f"fd_apply_hamiltonian_expect: {name} must be float64 [nbands]")
     rc = load_library().fd_apply_hamiltonian_expect(
         plan, _dev_ptr(psi), _dev_ptr(v_eff) if v_eff is not None else ctypes.c_void_p(0),
         _dev_ptr(out), _dev_ptr(eps), _dev_ptr(norm), int(psi.shape[0]), _dev_ptr(workspace),
@@ -247,6 +300,7 @@ def fd_apply_hamiltonian_expect(plan, psi, v_eff, out, eps, norm, workspace, str
 
 def fd_residual(plan, psi, hpsi, eps, norm, r, stream=None) -> None:
     """r_b = hpsi_b - (eps[b] / norm[b]) psi_b; r may be hpsi itself."""
+    _check_arrays(plan, "fd_residual", batch=(psi, hpsi, r))
     rc = load_library().fd_residual(plan, _dev_ptr(psi), _dev_ptr(hpsi), _dev_ptr(eps),
                                     _dev_ptr(norm), _dev_ptr(r), int(psi.shape[0]),
                                     _stream_ptr(stream))
@@ -255,6 +309,7 @@ def fd_residual(plan, psi, hpsi, eps, norm, r, stream=None) -> None:
 
 def fd_jacobi_sweep(plan, phi, rhs, out, omega: float, stream=None) -> None:
     """out = phi + omega (rhs - A phi) / A_ii for the plan's A = scale lap_FD (fd_create_scaled)."""
+    _check_arrays(plan, "fd_jacobi_sweep", batch=(phi, rhs, out))
     rc = load_library().fd_jacobi_sweep(plan, _dev_ptr(phi), _dev_ptr(rhs), _dev_ptr(out),
                                         int(phi.shape[0]), float(omega), _stream_ptr(stream))
     _check(rc, "fd_jacobi_sweep")
@@ -265,8 +320,20 @@ def coarse_shape(shape_fine: Sequence[int], bc: Sequence[int]):
     return tuple(int(n) // 2 if b else (int(n) - 1) // 2 for n, b in zip(shape_fine, bc))
 
 
+def _check_transfer(shape_fine, bc, fine, coarse, where: str) -> None:
+    nf, nc = tuple(int(n) for n in shape_fine), coarse_shape(shape_fine, bc)
+    if not all((n % 2 == 0 and n >= 2) if b else (n % 2 == 1 and n >= 3) for n, b in zip(nf, bc)):
+        return  # not a valid fine grid: the library reports it (FD_ERR_INVALID)
+    for t, shp, name in ((fine, nf, "fine"), (coarse, nc, "coarse")):
+        if t.dim() != 4 or tuple(t.shape[1:]) != shp or str(t.dtype) != "torch.float64":
+            raise ValueError(f"{where}: {name} must be float64 [nbands, {shp}], got {t.dtype} {tuple(t.shape)}")
+    if fine.shape[0] != coarse.shape[0] or fine.device != coarse.device:
+        raise ValueError(f"{where}: fine and coarse differ in band count or device")
+
+
 def fd_restrict(shape_fine, bc, p: int, fine, coarse, stream=None) -> None:
     """coarse[nbands, nc] <- fine[nbands, nf] (float64 CUDA tensors; include/fdham.h)."""
+    _check_transfer(shape_fine, bc, fine, coarse, "fd_restrict")
     rc = load_library().fd_restrict((ctypes.c_int32 * 3)(*[int(s) for s in shape_fine]),
                                     (ctypes.c_int32 * 3)(*[int(b) for b in bc]), int(p),
                                     _dev_ptr(fine), _dev_ptr(coarse), int(fine.shape[0]),
@@ -276,6 +343,7 @@ def fd_restrict(shape_fine, bc, p: int, fine, coarse, stream=None) -> None:
 
 def fd_interpolate(shape_fine, bc, p: int, coarse, fine, stream=None) -> None:
     """fine[nbands, nf] <- coarse[nbands, nc] (float64 CUDA tensors; include/fdham.h)."""
+    _check_transfer(shape_fine, bc, fine, coarse, "fd_interpolate")
     rc = load_library().fd_interpolate((ctypes.c_int32 * 3)(*[int(s) for s in shape_fine]),
                                        (ctypes.c_int32 * 3)(*[int(b) for b in bc]), int(p),
                                        _dev_ptr(coarse), _dev_ptr(fine), int(coarse.shape[0]),
@@ -320,8 +388,16 @@ def fd_paw_nproj_total(paw) -> int:
     return n
 
 
+def _check_coef(paw, psi, coef, where: str) -> None:
+    ntot = fd_paw_nproj_total(paw)
+    if tuple(coef.shape) != (psi.shape[0], ntot) or coef.dtype != psi.dtype or coef.device != psi.device:
+        raise ValueError(f"{where}: coef must be {psi.dtype} [{psi.shape[0]}, {ntot}] on {psi.device}")
+
+
 def fd_paw_project(plan, paw, psi, coef, stream=None) -> None:
     """coef[nbands, sum n_i] = dv <p~|psi> (dtype of psi)."""
+    _check_arrays(plan, "fd_paw_project", batch=(psi,))
+    _check_coef(paw, psi, coef, "fd_paw_project")
     rc = load_library().fd_paw_project(plan, paw, _dev_ptr(psi), _dev_ptr(coef), int(psi.shape[0]),
                                        _stream_ptr(stream))
     _check(rc, "fd_paw_project")
@@ -329,6 +405,8 @@ def fd_paw_project(plan, paw, psi, coef, stream=None) -> None:
 
 def fd_paw_add_nonlocal(plan, paw, psi, out, coef, stream=None) -> None:
     """out += sum |p~> Delta H <p~|psi>; coef is scratch [nbands, sum n_i]."""
+    _check_arrays(plan, "fd_paw_add_nonlocal", batch=(psi, out))
+    _check_coef(paw, psi, coef, "fd_paw_add_nonlocal")
     rc = load_library().fd_paw_add_nonlocal(plan, paw, _dev_ptr(psi), _dev_ptr(out), _dev_ptr(coef),
                                             int(psi.shape[0]), _stream_ptr(stream))
     _check(rc, "fd_paw_add_nonlocal")
@@ -336,6 +414,8 @@ def fd_paw_add_nonlocal(plan, paw, psi, out, coef, stream=None) -> None:
 
 def fd_apply_hamiltonian_paw(plan, paw, psi, v_eff, out, coef, stream=None) -> None:
     """out = -1/2 lap psi + v_eff psi + sum |p~> Delta H <p~|psi> (Eq. 6 complete)."""
+    _check_arrays(plan, "fd_apply_hamiltonian_paw", batch=(psi, out), grid=(v_eff,))
+    _check_coef(paw, psi, coef, "fd_apply_hamiltonian_paw")
     rc = load_library().fd_apply_hamiltonian_paw(
         plan, paw, _dev_ptr(psi), _dev_ptr(v_eff) if v_eff is not None else ctypes.c_void_p(0),
         _dev_ptr(out), _dev_ptr(coef), int(psi.shape[0]), _stream_ptr(stream))
@@ -344,6 +424,8 @@ def fd_apply_hamiltonian_paw(plan, paw, psi, v_eff, out, coef, stream=None) -> N
 
 def fd_apply_overlap(plan, paw, psi, out, coef, stream=None) -> None:
     """out = psi + sum |p~> Delta S <p~|psi> (Eq. 7)."""
+    _check_arrays(plan, "fd_apply_overlap", batch=(psi, out))
+    _check_coef(paw, psi, coef, "fd_apply_overlap")
     rc = load_library().fd_apply_overlap(plan, paw, _dev_ptr(psi), _dev_ptr(out), _dev_ptr(coef),
                                          int(psi.shape[0]), _stream_ptr(stream))
     _check(rc, "fd_apply_overlap")

@@ -314,10 +314,12 @@ def test_jacobi_full_size_grid_sampled(oracle, fd):
 def test_jacobi_rejects_complex_plans(fd):
     plan = fd.fd_create((8, 8, 8), (0.4,) * 3, dtype=fd.FD_C128)
     try:
-        x = torch.zeros((1, 8, 8, 8), dtype=torch.float64, device="cuda")
+        x = torch.zeros((1, 8, 8, 8), dtype=torch.complex128, device="cuda")
         with pytest.raises(fd.FDError) as ei:
             fd.fd_jacobi_sweep(plan, x, x.clone(), x.clone(), 1.0)
         assert ei.value.status == -2
+        with pytest.raises(ValueError):            # the binding checks dtypes against the plan
+            fd.fd_jacobi_sweep(plan, x.real.contiguous(), x.real.contiguous(), x.real.contiguous(), 1.0)
     finally:
         fd.fd_destroy(plan)
 
@@ -516,7 +518,7 @@ def test_paw_create_errors(fd):
         pw = fd.fd_paw_create(plan, [[0, 0, 0]], [[2, 2, 2]], [1], np.ones(8), np.ones(1))
         try:
             x = torch.zeros((1, 8, 8, 10), dtype=torch.float64, device="cuda")
-            c = torch.zeros((1, 2), dtype=torch.float64, device="cuda")
+            c = torch.zeros((1, 1), dtype=torch.float64, device="cuda")
             with pytest.raises(fd.FDError) as ei:                  # paw of another grid
                 fd.fd_paw_project(other, pw, x, c)
             assert ei.value.status == -1

@@ -817,3 +817,66 @@ def test_float32_full_size_cfg3_grid_and_unsupported_forms(oracle, fd):
         assert ei.value.status == -2
     finally:
         fd.fd_destroy(plan)
+
+
+def test_binding_rejects_arrays_that_do_not_match_the_plan(fd):
+    """The C ABI takes raw pointers; the binding checks shape, dtype and band counts first."""
+    plan = fd.fd_create((8, 10, 12), (0.4,) * 3)
+    try:
+        info = fd.fd_plan_get_info(plan)
+        assert info["shape"] == (8, 10, 12) and info["nn"] == 3 and info["dtype"] == fd.FD_F64
+        assert info["bc"] == (1, 1, 1) and info["device"] == 0
+        good = torch.zeros((2, 8, 10, 12), dtype=torch.float64, device="cuda")
+        v = torch.zeros((8, 10, 12), dtype=torch.float64, device="cuda")
+        fd.fd_apply_hamiltonian(plan, good, v, torch.empty_like(good))
+        for bad_psi, bad_out, bad_v in [
+                (torch.zeros((2, 8, 10, 10), dtype=torch.float64, device="cuda"), good, v),   # shape
+                (good, torch.zeros((1, 8, 10, 12), dtype=torch.float64, device="cuda"), v),   # band count
+                (good.to(torch.float32), good, v),                                            # dtype
+                (good, torch.empty_like(good), v[:4]),                                        # v_eff shape
+                (good, torch.empty_like(good), v.to(torch.float32))]:                        # v_eff dtype
+            with pytest.raises(ValueError):
+                fd.fd_apply_hamiltonian(plan, bad_psi, bad_v, bad_out)
+        with pytest.raises(ValueError):
+            fd.fd_apply_kinetic(plan, good, good.cpu())
+        torch.cuda.synchronize()
+    finally:
+        fd.fd_destroy(plan)
+
+
+def test_per_batch_kernel_choice_is_near_the_faster_kernel(fd):
+    """fd_plan_kernel_for's crossover (two B200 constants in fd_api.cu): whatever it picks must be
+    within 1.6x of the faster family for small and medium batches, and the sweep kernel for big ones."""
+    def time_plan(plan, psi, v, out, n=30):
+        for _ in range(5):
+            fd.fd_apply_hamiltonian(plan, psi, v, out)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(n):
+            fd.fd_apply_hamiltonian(plan, psi, v, out)
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / n
+    for shape, nb in [((24, 24, 24), 8), ((24, 24, 24), 64), ((48, 48, 48), 8), ((48, 48, 48), 64),
+                      ((32, 32, 32), 2)]:
+        psi = torch.randn((nb,) + shape, dtype=torch.float64, device="cuda")
+        v = torch.rand(shape, dtype=torch.float64, device="cuda")
+        out = torch.empty_like(psi)
+        times = {}
+        for kern in ("auto", fd.FD_KERNEL_SWEEP, fd.FD_KERNEL_GENERIC):
+            plan = fd.fd_create(shape, (0.4,) * 3)
+            try:
+                if kern != "auto":
+                    fd.fd_plan_set_kernel(plan, kern)
+                times[kern] = time_plan(plan, psi, v, out)
+            finally:
+                fd.fd_destroy(plan)
+        best = min(times[fd.FD_KERNEL_SWEEP], times[fd.FD_KERNEL_GENERIC])
+        assert times["auto"] <= 1.6 * best + 0.002, (shape, nb, times)
+    plan = fd.fd_create((96, 96, 96), (0.4,) * 3)
+    try:
+        assert fd.fd_plan_kernel_for(plan, 256) == fd.FD_KERNEL_SWEEP
+        assert fd.fd_plan_kernel_for(plan, 16) == fd.FD_KERNEL_SWEEP
+    finally:
+        fd.fd_destroy(plan)
