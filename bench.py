@@ -142,6 +142,18 @@ def _cfg(name):
     return W.get(name)
 
 
+def config_dict(cfg, world: int) -> dict:
+    """The `config` object of the JSON line: identical in both arms (ours / --impl reference)."""
+    return {"workload": cfg.name, "grid": list(cfg.shape), "nbands": cfg.nbands,
+            "bc": list(cfg.bc), "k": list(cfg.k), "nn": cfg.nn,
+            "h_angstrom": list(cfg.h_angstrom),
+            "parallelism": "replicas only" if world > 1 else "single GPU",
+            "l2": "inputs+outputs %.2f GB >> 126 MB L2, no flush between steps" % (cfg.min_bytes / 1e9)
+                  if cfg.min_bytes > (256 << 20) else
+                  "inputs+outputs %.1f MB fit the 126 MB L2: hot figure; see other_workloads for the "
+                  "rotating-buffer cold figure" % (cfg.min_bytes / 1e6)}
+
+
 def cpu_oracle_rate(cfg, budget_s: float = 10.0, max_bands: int | None = None):
     """Time the CPU oracle (as it stands) on a bounded sample of the workload: OpenMP over bands on
     all host cores (the reported `value`) and one thread (`value_1thread`, a third of the budget)."""
@@ -206,8 +218,7 @@ def run_reference(args):
         "n_gpus": args.gpus, "steps": done, "warmup": args.warmup,
         "ms_per_step": el / done * 1e3, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "c128" if cfg.complex else "f64", "data": "synthetic",
-        "config": {"workload": cfg.name, "grid": list(cfg.shape), "nbands": cfg.nbands,
-                   "sample": sample},
+        "config": config_dict(cfg, int(os.environ.get("WORLD_SIZE", "1"))),
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
                          "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -530,12 +541,7 @@ def run_ours(args):
             "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "c128" if cfg.complex else "f64",
             "data": "synthetic",
-            "config": {"workload": cfg.name, "grid": list(cfg.shape), "nbands": cfg.nbands,
-                       "bc": list(cfg.bc), "k": list(cfg.k), "nn": cfg.nn,
-                       "h_angstrom": list(cfg.h_angstrom), "kernel": kernel,
-                       "parallelism": "replicas only" if world > 1 else "single GPU",
-                       "l2": "inputs+outputs %.2f GB >> 126 MB L2, no flush between steps"
-                             % (cfg.min_bytes / 1e9)},
+            "config": config_dict(cfg, world), "kernel": kernel,
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
             "roofline": roofline, "cpu_baseline": cpu, "sustained": sustained, "parity": parity,
             "next_rows": rows, "other_workloads": others,
