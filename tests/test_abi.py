@@ -89,3 +89,20 @@ def test_product_path_does_not_import_oracle():
             if f.endswith((".py", ".cu", ".h", ".cpp")):
                 src = open(os.path.join(dirpath, f)).read()
                 assert "oracle" not in src.replace("no CPU", ""), f
+
+
+def test_c_abi_from_plain_c(lib, tmp_path):
+    """include/fdham.h compiles as C99 (-Wall -Wextra -pedantic -Werror) and libfdham.so links and
+    runs from a C program with no C++ / torch dependency."""
+    import subprocess
+    from paper_2310_14776_b200 import fdham
+    exe = tmp_path / "c_abi_check"
+    libdir = os.path.dirname(fdham.LIB_PATH)
+    cmd = ["gcc", "-std=c99", "-Wall", "-Wextra", "-pedantic", "-Werror", "-I", os.path.join(ROOT, "include"),
+           os.path.join(ROOT, "tests", "c_abi_check.c"), "-o", str(exe), "-L", libdir, "-lfdham",
+           "-Wl,-rpath," + libdir]
+    res = subprocess.run(cmd, capture_output=True, text=True)
+    assert res.returncode == 0, res.stderr
+    run = subprocess.run([str(exe)], capture_output=True, text=True, timeout=120)
+    assert run.returncode == 0, (run.returncode, run.stdout, run.stderr)
+    assert "c_abi_check" in run.stdout
