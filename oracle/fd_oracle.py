@@ -281,3 +281,50 @@ def paw_apply(shape, h, bc, k, psi: np.ndarray, box_start, box_size, nproj, proj
     if rc != 0:
         raise ValueError("fd_oracle_paw_apply: invalid argument")
     return (res, coef) if want_coef else res
+
+
+# ------------------------------------------------------------------------------ multigrid V-cycle
+
+def mg_levels(shape, bc, nn: int, max_levels: int = 16):
+    """Grid hierarchy of the V-cycle: level 0 = `shape`; a level is coarsened (n/2 on periodic axes,
+    (n-1)/2 on zero-BC axes, fd_oracle.c: fd_oracle_restrict) while every axis allows it (even >= 2
+    periodic / odd >= 3 zero-BC) and every coarse axis keeps at least max(nn, 2) points."""
+    levels = [tuple(int(n) for n in shape)]
+    while len(levels) < max_levels:
+        s = levels[-1]
+        if not all((n % 2 == 0 and n >= 2) if b else (n % 2 == 1 and n >= 3) for n, b in zip(s, bc)):
+            break
+        c = coarse_shape(s, bc)
+        if min(c) < max(nn, 2):
+            break
+        levels.append(c)
+    return levels
+
+
+def vcycle(shape, h, nn: int, bc, p: int, phi: np.ndarray, rhs: np.ndarray, nu1: int = 2,
+           nu2: int = 2, nu_coarse: int = 8, omega: float = 2.0 / 3.0, scale: float = 1.0,
+           max_levels: int = 16, _level: int = 0, _levels=None) -> np.ndarray:
+    """One multigrid V-cycle for (scale lap_FD) phi = rhs ("multigrid ... Jacobi"
+    Poisson solvers; PAPER.md:93, :150 grid transfer), the textbook algorithm step by step:
+        nu1 weighted-Jacobi sweeps;  r = rhs - A phi;  rhs_c = R r,  e_c = 0;
+        e_c <- V-cycle on the coarse grid (spacing 2h; nu_coarse sweeps on the coarsest grid);
+        phi += I e_c;  nu2 weighted-Jacobi sweeps.
+    Every step is the oracle function of that step (jacobi, apply, restrict, interpolate)."""
+    if _levels is None:
+        _levels = mg_levels(shape, bc, nn, max_levels)
+    phi = np.array(phi, dtype=np.float64, copy=True)
+    hl = tuple(x * (2 ** _level) for x in h)
+    if _level == len(_levels) - 1:
+        for _ in range(nu_coarse):
+            phi = jacobi(shape, hl, nn, bc, phi, rhs, omega, scale)
+        return phi
+    for _ in range(nu1):
+        phi = jacobi(shape, hl, nn, bc, phi, rhs, omega, scale)
+    r = rhs - apply(shape, hl, nn, bc, None, phi, None, scale=scale)
+    rhs_c = restrict(shape, bc, p, r)
+    e_c = vcycle(_levels[_level + 1], h, nn, bc, p, np.zeros_like(rhs_c), rhs_c, nu1, nu2, nu_coarse,
+                 omega, scale, max_levels, _level + 1, _levels)
+    phi = phi + interpolate(shape, bc, p, e_c)
+    for _ in range(nu2):
+        phi = jacobi(shape, hl, nn, bc, phi, rhs, omega, scale)
+    return phi
