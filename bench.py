@@ -339,6 +339,21 @@ def next_rows(torch, W, fd, cfg, plan, d_psi, d_v, d_out, stream, plain_ms, peak
         ms = _time_stream(torch, stream, lambda: fd.fd_interpolate(nf, cfg.bc, 3, coarse, fine, stream), 10, 2)
         rows["f3_interpolate"] = entry(ms, tb, what="order p = 3, %s -> %s, %d arrays" % (cfg.shape, nf, nt))
         del fine
+        # one multigrid V-cycle on this grid (2 + 2 sweeps per level, 8 on the coarsest, p = 3)
+        mg = fd.fd_mg_create(cfg.shape, cfg.h, cfg.nn, cfg.bc, 3, 16, nt, torch.cuda.current_device())
+        nlev = fd.fd_mg_levels(mg)
+        rhs = torch.empty((nt,) + cfg.shape, dtype=torch.float64, device="cuda").normal_()
+        rhs -= rhs.mean(dim=(1, 2, 3), keepdim=True)
+        phi = torch.zeros_like(rhs)
+        ms = _time_stream(torch, stream, lambda: fd.fd_mg_vcycle(mg, phi, rhs, 2, 2, 8, 2.0 / 3.0, stream), 10, 2)
+        # per fine-level point: 4 sweeps x 24 B + residual 24 + restrict 9 + interpolate 9 + add 24;
+        # levels shrink by 8; the coarsest level does 8 sweeps
+        pts = [P / 8 ** l for l in range(nlev)]
+        vb = nt * (sum(p_ * (4 * 24 + 66) for p_ in pts[:-1]) + pts[-1] * 8 * 24)
+        rows["f3_vcycle"] = entry(ms, vb, what="multigrid V-cycle, %d levels, %d right-hand sides, "
+                                                "2 + 2 Jacobi sweeps per level, p = 3" % (nlev, nt))
+        fd.fd_mg_destroy(mg)
+        del rhs, phi
     # PAW non-local term: ~1 atom per (9 A)^3 ... synthetic set of 128 atoms x (13 | 11) functions
     paw = W.make_paw(cfg, 128, nproj=13, radius_angstrom=1.1)
     pw = fd.fd_paw_create(plan, paw.box_start, paw.box_size, paw.nproj, paw.proj, paw.dmat, None)

@@ -187,6 +187,13 @@ FD_API int fd_jacobi_sweep(const fd_plan *plan, const double *phi, const double 
                     int64_t nbands, double omega, void *cuda_stream);
 
 /*
+ * fd_poisson_residual -- out = rhs - A phi for the plan's A = scale lap_FD (the residual of the
+ * Poisson problem, same kernels and argument rules as fd_jacobi_sweep).
+ */
+FD_API int fd_poisson_residual(const fd_plan *plan, const double *phi, const double *rhs, double *out,
+                        int64_t nbands, void *cuda_stream);
+
+/*
  * grid transfer between a fine grid (spacing h) and the coarse grid of spacing
  * 2h ("interpolating from one uniform grid to another", the second C hot spot of PAPER.md:150;
  * multigrid).  The paper prints no weights; readings R13 / R14:
@@ -257,6 +264,28 @@ FD_API int fd_apply_hamiltonian_paw(const fd_plan *plan, const fd_paw *paw, cons
                              void *cuda_stream);
 FD_API int fd_apply_overlap(const fd_plan *plan, const fd_paw *paw, const void *psi, void *out,
                      void *coef, int64_t nbands, void *cuda_stream);
+
+/*
+ * Multigrid V-cycle for lap_FD phi = rhs on the f3 kernels ("multigrid ... Jacobi" Poisson solvers,
+ * PAPER.md:248; the grids of PAPER.md:93).  The textbook cycle, per level l (spacing 2^l h):
+ *     nu1 weighted-Jacobi sweeps;  r = rhs - A phi;  rhs_{l+1} = R r,  phi_{l+1} = 0;  recurse
+ *     (nu_coarse sweeps on the coarsest level);  phi += I phi_{l+1};  nu2 sweeps.
+ * fd_mg_create builds the hierarchy (levels are added while every axis can be coarsened -- even on
+ *   periodic, odd on zero-BC axes -- and keeps max(nn, 2) points, at most max_levels), one plan per
+ *   level and the level buffers for up to max_nbands right-hand sides (3 arrays per coarse level, one
+ *   on the finest); transfer order p = 1..3.  fd_mg_levels: number of levels.
+ * fd_mg_vcycle: one cycle IN PLACE on phi [nbands, nx, ny, nz] (device, float64, 16-byte aligned;
+ *   rhs likewise, no overlap); a sequence of kernel launches on cuda_stream, no synchronisation.
+ *   A single-level hierarchy (a grid that cannot be coarsened) does nu_coarse sweeps.  Errors as fd_jacobi_sweep / fd_restrict;
+ *   FD_ERR_INVALID for nbands > max_nbands.
+ */
+typedef struct fd_mg fd_mg;
+FD_API int fd_mg_create(fd_mg **mg, const int32_t shape[3], const double h[3], int32_t nn,
+                 const int32_t bc[3], int32_t p, int32_t max_levels, int64_t max_nbands, int32_t device);
+FD_API int fd_mg_destroy(fd_mg *mg);
+FD_API int32_t fd_mg_levels(const fd_mg *mg);
+FD_API int fd_mg_vcycle(const fd_mg *mg, double *phi, const double *rhs, int64_t nbands, int32_t nu1,
+                 int32_t nu2, int32_t nu_coarse, double omega, void *cuda_stream);
 
 /* fd_destroy -- free the plan; NULL is a no-op.  The caller must have synchronised any stream
  * still running an apply of this plan. */

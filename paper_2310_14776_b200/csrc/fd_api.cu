@@ -482,6 +482,187 @@ int fd_jacobi_sweep(const fd_plan *plan, const double *phi, const double *rhs, d
                         (cudaStream_t)cuda_stream);
 }
 
+int fd_poisson_residual(const fd_plan *plan, const double *phi, const double *rhs, double *out,
+                        int64_t nbands, void *cuda_stream)
+{
+    if (!plan || nbands < 0) return FD_ERR_INVALID;
+    if (plan->g.cplx || plan->g.f32) return FD_ERR_UNSUPPORTED;
+    if (nbands == 0) return FD_OK;
+    if (!phi || !rhs || !out) return FD_ERR_INVALID;
+    if (((uintptr_t)phi | (uintptr_t)rhs | (uintptr_t)out) & 15) return FD_ERR_INVALID;
+    const size_t nb = (size_t)plan->g.n[0] * plan->g.n[1] * plan->g.n[2] * (size_t)nbands * 8;
+    if (overlaps(out, nb, phi, nb) || overlaps(out, nb, rhs, nb)) return FD_ERR_ALIAS;
+    // out = rhs - A phi: the Jacobi form of the stencil kernels with weights -w and coefficient 1
+    FdGeom gr = plan->g;
+    for (int d = 0; d < 3; ++d)
+        for (int j = 0; j <= gr.nn; ++j) gr.w[d][j] = -plan->g.w[d][j];
+    gr.wdiag = -plan->g.wdiag;
+    gr.rhs_coef = 1.0;
+    return apply_device(plan, gr, 2, phi, rhs, out, nbands, nullptr, nullptr, nullptr,
+                        (cudaStream_t)cuda_stream);
+}
+
+// ---- multigrid V-cycle on the f3 kernels ------------------------------------------------------------
+
+struct fd_mg {
+    static const int kMaxLevels = 16;
+    int nlevels, p, device;
+    int32_t bc[3];
+    int32_t shape[kMaxLevels][3];
+    size_t npoints[kMaxLevels];
+    fd_plan *plan[kMaxLevels];
+    double *phi[kMaxLevels], *rhs[kMaxLevels], *tmp[kMaxLevels];  // phi / rhs of level 0: the caller's
+    int64_t max_nbands;
+};
+
+int fd_mg_destroy(fd_mg *mg)
+{
+    if (!mg) return FD_OK;
+    for (int l = 0; l < mg->nlevels; ++l) {
+        if (mg->plan[l]) fd_destroy(mg->plan[l]);
+        if (l > 0) {
+            cudaFree(mg->phi[l]);
+            cudaFree(mg->rhs[l]);
+        }
+        cudaFree(mg->tmp[l]);
+    }
+    cudaGetLastError();
+    delete mg;
+    return FD_OK;
+}
+
+int fd_mg_create(fd_mg **mg_out, const int32_t shape[3], const double h[3], int32_t nn,
+                 const int32_t bc[3], int32_t p, int32_t max_levels, int64_t max_nbands, int32_t device)
+{
+    if (!mg_out || !shape || !h || !bc || max_nbands < 1 || max_levels < 1) return FD_ERR_INVALID;
+    if (p < 1 || p > 3) return (p >= 1 && p <= 6) ? FD_ERR_UNSUPPORTED : FD_ERR_INVALID;
+    int cur = -1;  // the level buffers are allocated on the current device: it must be `device`
+    if (cudaGetDevice(&cur) != cudaSuccess) {
+        cudaGetLastError();
+        return FD_ERR_CUDA;
+    }
+    if (cur != device) return FD_ERR_INVALID;
+    fd_mg *mg = new (std::nothrow) fd_mg();
+    if (!mg) return FD_ERR_NOMEM;
+    memset(mg, 0, sizeof(*mg));
+    mg->p = p;
+    mg->device = device;
+    mg->max_nbands = max_nbands;
+    if (max_levels > fd_mg::kMaxLevels) max_levels = fd_mg::kMaxLevels;
+    int32_t s[3] = {shape[0], shape[1], shape[2]};
+    double hl[3] = {h[0], h[1], h[2]};
+    int rc = FD_OK;
+    for (int l = 0; l < max_levels && rc == FD_OK; ++l) {
+        for (int d = 0; d < 3; ++d) {
+            mg->bc[d] = bc[d];
+            mg->shape[l][d] = s[d];
+        }
+        mg->npoints[l] = (size_t)s[0] * s[1] * s[2];
+        rc = fd_create_scaled(&mg->plan[l], s, hl, nn, bc, nullptr, FD_F64, device, 1.0);
+        if (rc != FD_OK) break;
+        mg->nlevels = l + 1;
+        const size_t bytes = mg->npoints[l] * 8 * (size_t)max_nbands;
+        if (cudaMalloc(&mg->tmp[l], bytes) != cudaSuccess ||
+            (l > 0 && (cudaMalloc(&mg->phi[l], bytes) != cudaSuccess ||
+                       cudaMalloc(&mg->rhs[l], bytes) != cudaSuccess))) {
+            rc = FD_ERR_NOMEM;
+            break;
+        }
+        // the next level: every axis must allow coarsening and keep max(nn, 2) points
+        bool ok = true;
+        int32_t c[3];
+        for (int d = 0; d < 3; ++d) {
+            ok = ok && (bc[d] ? (s[d] % 2 == 0 && s[d] >= 2) : (s[d] % 2 == 1 && s[d] >= 3));
+            c[d] = bc[d] ? s[d] / 2 : (s[d] - 1) / 2;
+            ok = ok && c[d] >= (nn > 2 ? nn : 2);
+        }
+        if (!ok) break;
+        for (int d = 0; d < 3; ++d) {
+            s[d] = c[d];
+            hl[d] *= 2.0;
+        }
+    }
+    if (rc != FD_OK) {
+        cudaGetLastError();
+        fd_mg_destroy(mg);
+        return rc;
+    }
+    *mg_out = mg;
+    return FD_OK;
+}
+
+int32_t fd_mg_levels(const fd_mg *mg) { return mg ? mg->nlevels : FD_ERR_INVALID; }
+
+namespace {
+
+// nu weighted-Jacobi sweeps on level l, result in phi (tmp is the other buffer of the ping-pong)
+int mg_smooth(const fd_mg *mg, int l, double *phi, const double *rhs, int64_t nbands, int nu,
+              double omega, void *stream)
+{
+    double *src = phi, *dst = mg->tmp[l];
+    for (int s = 0; s < nu; ++s) {
+        const int rc = fd_jacobi_sweep(mg->plan[l], src, rhs, dst, nbands, omega, stream);
+        if (rc != FD_OK) return rc;
+        double *t = src;
+        src = dst;
+        dst = t;
+    }
+    if (src != phi &&
+        cudaMemcpyAsync(phi, src, mg->npoints[l] * 8 * (size_t)nbands, cudaMemcpyDeviceToDevice,
+                        (cudaStream_t)stream) != cudaSuccess) {
+        cudaGetLastError();
+        return FD_ERR_CUDA;
+    }
+    return FD_OK;
+}
+
+}  // namespace
+
+int fd_mg_vcycle(const fd_mg *mg, double *phi, const double *rhs, int64_t nbands, int32_t nu1,
+                 int32_t nu2, int32_t nu_coarse, double omega, void *cuda_stream)
+{
+    if (!mg || nbands < 0 || nu1 < 0 || nu2 < 0 || nu_coarse < 0 || !isfinite(omega)) return FD_ERR_INVALID;
+    if (nbands > mg->max_nbands) return FD_ERR_INVALID;
+    if (nbands == 0) return FD_OK;
+    if (!phi || !rhs) return FD_ERR_INVALID;
+    const size_t nb0 = mg->npoints[0] * 8 * (size_t)nbands;
+    if (overlaps(phi, nb0, rhs, nb0)) return FD_ERR_ALIAS;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const int L = mg->nlevels;
+    double *ph[fd_mg::kMaxLevels];
+    const double *rh[fd_mg::kMaxLevels];
+    for (int l = 0; l < L; ++l) {
+        ph[l] = l ? mg->phi[l] : phi;
+        rh[l] = l ? mg->rhs[l] : rhs;
+    }
+    int rc;
+    for (int l = 0; l + 1 < L; ++l) {  // down: smooth, residual, restrict, zero initial guess
+        if ((rc = mg_smooth(mg, l, ph[l], rh[l], nbands, nu1, omega, cuda_stream)) != FD_OK) return rc;
+        if ((rc = fd_poisson_residual(mg->plan[l], ph[l], rh[l], mg->tmp[l], nbands, cuda_stream)) != FD_OK)
+            return rc;
+        if ((rc = fd_transfer_run(0, mg->shape[l], mg->bc, mg->p, mg->tmp[l], mg->rhs[l + 1], nbands, st)) != 0)
+            return rc;
+        if (cudaMemsetAsync(mg->phi[l + 1], 0, mg->npoints[l + 1] * 8 * (size_t)nbands, st) != cudaSuccess) {
+            cudaGetLastError();
+            return FD_ERR_CUDA;
+        }
+    }
+    if ((rc = mg_smooth(mg, L - 1, ph[L - 1], rh[L - 1], nbands, nu_coarse, omega,
+                        cuda_stream)) != FD_OK)
+        return rc;
+    for (int l = L - 2; l >= 0; --l) {  // up: interpolate the correction, add, smooth
+        if ((rc = fd_transfer_run(1, mg->shape[l], mg->bc, mg->p, ph[l + 1], mg->tmp[l], nbands, st)) != 0)
+            return rc;
+        if (fd_launch_add(ph[l], mg->tmp[l], (long long)(mg->npoints[l] * (size_t)nbands),
+                          mg->plan[l]->sm_count, st) != cudaSuccess) {
+            cudaGetLastError();
+            return FD_ERR_CUDA;
+        }
+        if ((rc = mg_smooth(mg, l, ph[l], rh[l], nbands, nu2, omega, cuda_stream)) != FD_OK) return rc;
+    }
+    return FD_OK;
+}
+
 // ---- grid transfer ---------------------------------------------------------------
 
 static int transfer_call(int interp, const int32_t shape_fine[3], const int32_t bc[3], int32_t p,

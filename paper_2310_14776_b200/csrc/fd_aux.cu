@@ -104,6 +104,27 @@ fd_residual_kernel(const double *__restrict__ psi, const double *hpsi, const dou
     }
 }
 
+// y += x over n doubles (the coarse-grid correction of the V-cycle)
+__global__ void __launch_bounds__(256) fd_add_kernel(double *__restrict__ y, const double *__restrict__ x, long long n)
+{
+    const long long stride = (long long)gridDim.x * blockDim.x * 2;
+    long long i = ((long long)blockIdx.x * blockDim.x + threadIdx.x) * 2;
+    const bool vec = ((reinterpret_cast<uintptr_t>(y) | reinterpret_cast<uintptr_t>(x)) & 15) == 0;
+    for (; i + 1 < n; i += stride) {
+        if (vec) {
+            double2 a = *reinterpret_cast<double2 *>(y + i);
+            const double2 b = __ldcs(reinterpret_cast<const double2 *>(x + i));
+            a.x += b.x;
+            a.y += b.y;
+            *reinterpret_cast<double2 *>(y + i) = a;
+        } else {
+            y[i] += x[i];
+            y[i + 1] += x[i + 1];
+        }
+    }
+    if (i < n) y[i] += x[i];
+}
+
 inline int dot_chunks(const fd_plan *plan)
 {
     const long long band_d =
@@ -161,4 +182,15 @@ cudaError_t fd_launch_residual(const fd_plan *plan, const void *psi, const void 
         if (e != cudaSuccess) return e;
     }
     return cudaSuccess;
+}
+
+cudaError_t fd_launch_add(double *y, const double *x, long long n, int sm_count, cudaStream_t stream)
+{
+    if (n <= 0) return cudaSuccess;
+    long long blocks = (n / 2 + 255) / 256;
+    const long long cap = 8LL * sm_count;
+    if (blocks > cap) blocks = cap;
+    if (blocks < 1) blocks = 1;
+    fd_add_kernel<<<(unsigned)blocks, 256, 0, stream>>>(y, x, n);
+    return cudaPeekAtLastError();
 }

@@ -73,6 +73,7 @@ int64_t fd_dot_ws_bytes(const fd_plan *plan, int64_t nbands);
 cudaError_t fd_launch_dot(const fd_plan *plan, const void *psi, const void *hpsi, double *eps,
                           double *norm, double *ws, int64_t nbands, cudaStream_t stream,
                           int *nlaunches);
+cudaError_t fd_launch_add(double *y, const double *x, long long n, int sm_count, cudaStream_t stream);
 cudaError_t fd_launch_residual(const fd_plan *plan, const void *psi, const void *hpsi,
                                const double *eps, const double *norm, void *r, int64_t nbands,
                                cudaStream_t stream);

@@ -29,6 +29,7 @@ EXPORTED_SYMBOLS = [
     "fd_residual", "fd_jacobi_sweep", "fd_restrict", "fd_interpolate",
     "fd_paw_create", "fd_paw_destroy", "fd_paw_nproj_total", "fd_paw_project", "fd_paw_add_nonlocal",
     "fd_apply_hamiltonian_paw", "fd_apply_overlap",
+    "fd_poisson_residual", "fd_mg_create", "fd_mg_destroy", "fd_mg_levels", "fd_mg_vcycle",
     "fd_destroy", "fd_strerror", "fd_plan_set_kernel", "fd_plan_get_kernel", "fd_plan_kernel_for", "fd_plan_launches",
     "fd_plan_get_weights", "fd_plan_get_info",
 ]
@@ -98,6 +99,16 @@ def load_library() -> ctypes.CDLL:
     lib.fd_apply_hamiltonian_paw.restype = ctypes.c_int
     lib.fd_apply_overlap.argtypes = [vp, vp, vp, vp, vp, i64, vp]
     lib.fd_apply_overlap.restype = ctypes.c_int
+    lib.fd_poisson_residual.argtypes = [vp, vp, vp, vp, i64, vp]
+    lib.fd_poisson_residual.restype = ctypes.c_int
+    lib.fd_mg_create.argtypes = [ctypes.POINTER(vp), i32p, f64p, i32, i32p, i32, i32, i64, i32]
+    lib.fd_mg_create.restype = ctypes.c_int
+    lib.fd_mg_destroy.argtypes = [vp]
+    lib.fd_mg_destroy.restype = ctypes.c_int
+    lib.fd_mg_levels.argtypes = [vp]
+    lib.fd_mg_levels.restype = ctypes.c_int32
+    lib.fd_mg_vcycle.argtypes = [vp, vp, vp, i64, i32, i32, i32, ctypes.c_double, vp]
+    lib.fd_mg_vcycle.restype = ctypes.c_int
     lib.fd_destroy.argtypes = [vp]
     lib.fd_destroy.restype = ctypes.c_int
     lib.fd_strerror.argtypes = [ctypes.c_int]
@@ -429,6 +440,44 @@ def fd_apply_overlap(plan, paw, psi, out, coef, stream=None) -> None:
     rc = load_library().fd_apply_overlap(plan, paw, _dev_ptr(psi), _dev_ptr(out), _dev_ptr(coef),
                                          int(psi.shape[0]), _stream_ptr(stream))
     _check(rc, "fd_apply_overlap")
+
+
+def fd_poisson_residual(plan, phi, rhs, out, stream=None) -> None:
+    """out = rhs - A phi for the plan's A = scale lap_FD."""
+    _check_arrays(plan, "fd_poisson_residual", batch=(phi, rhs, out))
+    rc = load_library().fd_poisson_residual(plan, _dev_ptr(phi), _dev_ptr(rhs), _dev_ptr(out),
+                                            int(phi.shape[0]), _stream_ptr(stream))
+    _check(rc, "fd_poisson_residual")
+
+
+def fd_mg_create(shape, h, nn: int = 3, bc=(1, 1, 1), p: int = 2, max_levels: int = 16,
+                 max_nbands: int = 1, device: int = 0) -> ctypes.c_void_p:
+    """Multigrid hierarchy for lap_FD phi = rhs (include/fdham.h: fd_mg_create)."""
+    mg = ctypes.c_void_p()
+    rc = load_library().fd_mg_create(ctypes.byref(mg), (ctypes.c_int32 * 3)(*[int(s) for s in shape]),
+                                     (ctypes.c_double * 3)(*[float(x) for x in h]), int(nn),
+                                     (ctypes.c_int32 * 3)(*[int(b) for b in bc]), int(p),
+                                     int(max_levels), int(max_nbands), int(device))
+    _check(rc, "fd_mg_create")
+    return mg
+
+
+def fd_mg_destroy(mg) -> None:
+    _check(load_library().fd_mg_destroy(mg), "fd_mg_destroy")
+
+
+def fd_mg_levels(mg) -> int:
+    return int(load_library().fd_mg_levels(mg))
+
+
+def fd_mg_vcycle(mg, phi, rhs, nu1: int = 2, nu2: int = 2, nu_coarse: int = 8,
+                 omega: float = 2.0 / 3.0, stream=None) -> None:
+    """One V-cycle in place on phi (float64 CUDA tensors [nbands, nx, ny, nz])."""
+    if phi.shape != rhs.shape or phi.dtype != rhs.dtype or str(phi.dtype) != "torch.float64":
+        raise ValueError("fd_mg_vcycle: phi and rhs must be float64 tensors of the same shape")
+    rc = load_library().fd_mg_vcycle(mg, _dev_ptr(phi), _dev_ptr(rhs), int(phi.shape[0]), int(nu1),
+                                     int(nu2), int(nu_coarse), float(omega), _stream_ptr(stream))
+    _check(rc, "fd_mg_vcycle")
 
 
 def fd_plan_set_kernel(plan, kernel: int, param: int = 0) -> None:
