@@ -276,6 +276,9 @@ FD_API int fd_apply_overlap(const fd_plan *plan, const fd_paw *paw, const void *
  *   on the finest); transfer order p = 1..3.  fd_mg_levels: number of levels.
  * fd_mg_vcycle: one cycle IN PLACE on phi [nbands, nx, ny, nz] (device, float64, 16-byte aligned;
  *   rhs likewise, no overlap); a sequence of kernel launches on cuda_stream, no synchronisation.
+ *   On a non-default stream the sequence is captured into a CUDA graph the first time an argument
+ *   set (phi, rhs, nbands, nu1, nu2, nu_coarse, omega) is seen and replayed afterwards (the coarse
+ *   levels are launch bound); the last argument set is kept.  Calls on one fd_mg are serialised.
  *   A single-level hierarchy (a grid that cannot be coarsened) does nu_coarse sweeps.  Errors as fd_jacobi_sweep / fd_restrict;
  *   FD_ERR_INVALID for nbands > max_nbands.
  */

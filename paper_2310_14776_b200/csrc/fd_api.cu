@@ -2,6 +2,7 @@
 // checking, kernel dispatch, and the host-buffer (end-to-end) variant.  No CPU compute path exists
 // here on purpose: without a CUDA device every entry point fails with FD_ERR_CUDA.
 #include <math.h>
+#include <mutex>
 #include <new>
 #include <stdlib.h>
 #include <string.h>
@@ -513,11 +514,24 @@ struct fd_mg {
     fd_plan *plan[kMaxLevels];
     double *phi[kMaxLevels], *rhs[kMaxLevels], *tmp[kMaxLevels];  // phi / rhs of level 0: the caller's
     int64_t max_nbands;
+    // The cycle is ~15 launches per level and launch bound on the coarse levels: it is captured once
+    // into a CUDA graph per argument set (the last one is kept) and replayed.
+    struct GraphKey {
+        const void *phi, *rhs;
+        int64_t nbands;
+        int nu1, nu2, nu_coarse;
+        double omega;
+    };
+    mutable std::mutex graph_mutex;
+    mutable GraphKey graph_key;
+    mutable cudaGraphExec_t graph_exec;
+    mutable bool graph_off;  // capture failed once (e.g. an unsupported stream): launch directly
 };
 
 int fd_mg_destroy(fd_mg *mg)
 {
     if (!mg) return FD_OK;
+    if (mg->graph_exec) cudaGraphExecDestroy(mg->graph_exec);
     for (int l = 0; l < mg->nlevels; ++l) {
         if (mg->plan[l]) fd_destroy(mg->plan[l]);
         if (l > 0) {
@@ -544,7 +558,15 @@ int fd_mg_create(fd_mg **mg_out, const int32_t shape[3], const double h[3], int3
     if (cur != device) return FD_ERR_INVALID;
     fd_mg *mg = new (std::nothrow) fd_mg();
     if (!mg) return FD_ERR_NOMEM;
-    memset(mg, 0, sizeof(*mg));
+    mg->nlevels = 0;
+    mg->graph_exec = nullptr;
+    mg->graph_off = false;
+    memset(&mg->graph_key, 0, sizeof(mg->graph_key));
+    for (int l = 0; l < fd_mg::kMaxLevels; ++l) {
+        mg->plan[l] = nullptr;
+        mg->phi[l] = mg->rhs[l] = mg->tmp[l] = nullptr;
+        mg->npoints[l] = 0;
+    }
     mg->p = p;
     mg->device = device;
     mg->max_nbands = max_nbands;
@@ -618,15 +640,12 @@ int mg_smooth(const fd_mg *mg, int l, double *phi, const double *rhs, int64_t nb
 
 }  // namespace
 
-int fd_mg_vcycle(const fd_mg *mg, double *phi, const double *rhs, int64_t nbands, int32_t nu1,
-                 int32_t nu2, int32_t nu_coarse, double omega, void *cuda_stream)
+namespace {
+
+// the launches of one cycle, in order, on stream cuda_stream
+int mg_cycle_launches(const fd_mg *mg, double *phi, const double *rhs, int64_t nbands, int32_t nu1,
+                      int32_t nu2, int32_t nu_coarse, double omega, void *cuda_stream)
 {
-    if (!mg || nbands < 0 || nu1 < 0 || nu2 < 0 || nu_coarse < 0 || !isfinite(omega)) return FD_ERR_INVALID;
-    if (nbands > mg->max_nbands) return FD_ERR_INVALID;
-    if (nbands == 0) return FD_OK;
-    if (!phi || !rhs) return FD_ERR_INVALID;
-    const size_t nb0 = mg->npoints[0] * 8 * (size_t)nbands;
-    if (overlaps(phi, nb0, rhs, nb0)) return FD_ERR_ALIAS;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const int L = mg->nlevels;
     double *ph[fd_mg::kMaxLevels];
@@ -659,6 +678,65 @@ int fd_mg_vcycle(const fd_mg *mg, double *phi, const double *rhs, int64_t nbands
             return FD_ERR_CUDA;
         }
         if ((rc = mg_smooth(mg, l, ph[l], rh[l], nbands, nu2, omega, cuda_stream)) != FD_OK) return rc;
+    }
+    return FD_OK;
+}
+
+}  // namespace
+
+int fd_mg_vcycle(const fd_mg *mg, double *phi, const double *rhs, int64_t nbands, int32_t nu1,
+                 int32_t nu2, int32_t nu_coarse, double omega, void *cuda_stream)
+{
+    if (!mg || nbands < 0 || nu1 < 0 || nu2 < 0 || nu_coarse < 0 || !isfinite(omega)) return FD_ERR_INVALID;
+    if (nbands > mg->max_nbands) return FD_ERR_INVALID;
+    if (nbands == 0) return FD_OK;
+    if (!phi || !rhs) return FD_ERR_INVALID;
+    if (((uintptr_t)phi | (uintptr_t)rhs) & 15) return FD_ERR_INVALID;
+    const size_t nb0 = mg->npoints[0] * 8 * (size_t)nbands;
+    if (overlaps(phi, nb0, rhs, nb0)) return FD_ERR_ALIAS;
+    const int drc = check_device(mg->plan[0]);
+    if (drc != FD_OK) return drc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    // The legacy default stream cannot be captured: launch directly there.
+    if (st == nullptr || st == cudaStreamLegacy || mg->graph_off)
+        return mg_cycle_launches(mg, phi, rhs, nbands, nu1, nu2, nu_coarse, omega, cuda_stream);
+
+    std::lock_guard<std::mutex> lock(mg->graph_mutex);
+    const fd_mg::GraphKey key = {phi, rhs, nbands, nu1, nu2, nu_coarse, omega};
+    if (!mg->graph_exec || memcmp(&key, &mg->graph_key, sizeof(key)) != 0) {
+        if (mg->graph_exec) {
+            cudaGraphExecDestroy(mg->graph_exec);
+            mg->graph_exec = nullptr;
+        }
+        cudaGraph_t graph = nullptr;
+        if (cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+            cudaGetLastError();
+            mg->graph_off = true;
+            return mg_cycle_launches(mg, phi, rhs, nbands, nu1, nu2, nu_coarse, omega, cuda_stream);
+        }
+        const int rc = mg_cycle_launches(mg, phi, rhs, nbands, nu1, nu2, nu_coarse, omega, cuda_stream);
+        const cudaError_t ce = cudaStreamEndCapture(st, &graph);
+        if (rc != FD_OK || ce != cudaSuccess || !graph) {
+            if (graph) cudaGraphDestroy(graph);
+            cudaGetLastError();
+            // nothing was enqueued; whatever went wrong (a call that is not allowed inside a capture, a
+            // real launch error) shows again, with its proper status, in the direct launch
+            mg->graph_off = true;
+            return mg_cycle_launches(mg, phi, rhs, nbands, nu1, nu2, nu_coarse, omega, cuda_stream);
+        }
+        const cudaError_t ie = cudaGraphInstantiate(&mg->graph_exec, graph, 0);
+        cudaGraphDestroy(graph);
+        if (ie != cudaSuccess) {
+            cudaGetLastError();
+            mg->graph_exec = nullptr;
+            mg->graph_off = true;
+            return mg_cycle_launches(mg, phi, rhs, nbands, nu1, nu2, nu_coarse, omega, cuda_stream);
+        }
+        mg->graph_key = key;
+    }
+    if (cudaGraphLaunch(mg->graph_exec, st) != cudaSuccess) {
+        cudaGetLastError();
+        return FD_ERR_CUDA;
     }
     return FD_OK;
 }

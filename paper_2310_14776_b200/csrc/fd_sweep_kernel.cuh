@@ -1,8 +1,11 @@
 // fd_sweep_kernel.cuh -- the sweep kernel template (included by the fd_sweep_inst_*.cu translation
 // units, which instantiate it, so that they compile in parallel).
 //
-// Sweep kernel: the bandwidth path of libfdham (nn = 1..3; nn = 3 is GPAW's default 19-point star,
-// which the comments below use for concreteness: halo 3, seven accumulators).
+// Sweep kernel: the bandwidth path of libfdham (nn = 1..6; nn = 3 is GPAW's default 19-point star,
+// which the comments below use for concreteness: halo 3, seven accumulators).  The same template
+// also carries the SURVEY 8(f) forms that ride the stencil: the weighted-Jacobi / residual form
+// (MODE 2), the fused expectation values (EX), real Bloch factors -1 (PH on float64), nn = 4..6
+// (2-row micro tile) and float32 / complex64 (F32); see the template parameter list below.
 //
 // Operation: include/fdham.h -- out = -1/2 lap_FD psi + v_eff psi (Eq. 6 first two terms,
 // PAPER.md:187-188; FD kinetic operator PAPER.md:232; the stencil hot spot PAPER.md:150).
@@ -29,9 +32,10 @@
 //     access of a warp is conflict free (the shared-memory data pipe is what bounds this kernel).
 //   * The row length is a template parameter for the common grids (ROWD doubles per z row; 0 =
 //     run time), so every shared-memory and store address of a step is base register + immediate.
-//   * The warp that is last to release a ring slot refills it (election by a shared-memory
-//     counter whose result is consumed only at the end of the step), so no warp ever waits for
-//     the others in order to issue a load.
+//   * Warp specialisation: a fourth warpgroup's first lane is the producer.  It waits on the
+//     `empty` mbarrier of a slot (one arrival per compute warp) and issues that slot's bulk copies,
+//     v_eff rows first; setmaxnreg hands its registers to the 12 compute warps (24 / 160).  The
+//     compute warps never issue a load and never wait for each other.
 //   * Boundaries are resolved while staging / addressing, never by a padded copy:
 //       periodic y  -> the wrapped halo rows are a separate bulk copy from the other end;
 //       zero y      -> those shared-memory rows are zeroed once and never overwritten;
@@ -39,7 +43,8 @@
 //       zero z      -> the out-of-range chunk address points at a zero block of the stage;
 //       periodic x  -> the table's prologue/epilogue entries load planes from the other end;
 //       zero x      -> those entries carry no load (the value is taken as zero);
-//       Bloch phase -> multiply only wrapped rows / chunks / planes (complex128 only).
+//       Bloch phase -> multiply only wrapped rows / chunks / planes (complex; sign flips for
+//                      float64 at k = 1/2).
 //   * Persistent teams: the (band, x) planes are split evenly over sm_count / nytiles teams of
 //     nytiles CTAs (one CTA per SM, plain launch, no cluster: 147 of 148 SMs for 3 tiles).  The
 //     CTAs of a team sweep the same planes for adjacent y-tiles; the y-halo rows they share are

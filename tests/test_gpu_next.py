@@ -613,3 +613,37 @@ def test_poisson_residual_parity_and_mg_errors(oracle, fd):
     with pytest.raises(fd.FDError) as ei:
         fd.fd_mg_create((16, 16, 16), (0.5,) * 3, 3, (1, 1, 1), 5, 16, 2, 0)
     assert ei.value.status == -2
+
+
+def test_vcycle_graph_replay_on_a_side_stream_matches_direct_launches(fd):
+    """On a non-default stream the cycle is captured into a CUDA graph and replayed: same bits as the
+    direct launches on the default stream, also after the argument set changes."""
+    n, bc = (32, 32, 32), (1, 1, 1)
+    cfg = W.custom(n, (0.3, 0.3, 0.3), bc, nbands=2)
+    rng = np.random.default_rng(21)
+    rhs_np = rng.standard_normal((2,) + n)
+    rhs_np -= rhs_np.mean(axis=(1, 2, 3), keepdims=True)
+    mg = fd.fd_mg_create(n, cfg.h, 3, bc, 2, 16, 2, 0)
+    try:
+        rhs = torch.from_numpy(rhs_np).cuda()
+        ref = torch.zeros_like(rhs)
+        for _ in range(3):
+            fd.fd_mg_vcycle(mg, ref, rhs)                       # default stream: direct launches
+        torch.cuda.synchronize()
+        s = torch.cuda.Stream()
+        phi = torch.zeros_like(rhs)
+        for _ in range(3):
+            fd.fd_mg_vcycle(mg, phi, rhs, stream=s)             # capture, then two replays
+        s.synchronize()
+        assert torch.equal(phi, ref)
+        phi2 = torch.zeros_like(rhs)                            # new pointers: re-capture
+        fd.fd_mg_vcycle(mg, phi2, rhs, 1, 1, 4, 0.8, stream=s)
+        fd.fd_mg_vcycle(mg, phi2, rhs, 1, 1, 4, 0.8, stream=s)
+        s.synchronize()
+        ref2 = torch.zeros_like(rhs)
+        fd.fd_mg_vcycle(mg, ref2, rhs, 1, 1, 4, 0.8)
+        fd.fd_mg_vcycle(mg, ref2, rhs, 1, 1, 4, 0.8)
+        torch.cuda.synchronize()
+        assert torch.equal(phi2, ref2)
+    finally:
+        fd.fd_mg_destroy(mg)
