@@ -26,7 +26,8 @@ void fd_sweep_configure(fd_plan *plan, int tyc_override, int xchunk_override, in
     if (g.f32 && (g.nn > 3 || fd_plan_real_phase(plan))) return;  // float32: nn <= 3, no sign flips
     if (g.f32 && !g.cplx && (g.n[2] & 3)) return;                  // rows are whole 16-byte chunks
     if (g.n[0] > 65536) return;  // x index + 2 nn in 17 bits of a step-table entry
-    c.ty = g.nn <= 3 ? 4 : 2;  // 2 nn + 1 accumulator planes x ty rows per thread (registers)
+    // 2 nn + 1 accumulator planes x ty rows per thread must fit the registers (must match the kernel)
+    c.ty = g.nn <= 3 ? 4 : ((g.nn == 4 && !g.cplx) ? 3 : 2);
     c.tc = 1;
     const int pitch = g.n[2] * fd_elem_bytes(g.cplx, g.f32);
     const int pitchv = g.n[2] * (g.f32 ? 4 : 8);

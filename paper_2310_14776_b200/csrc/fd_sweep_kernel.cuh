@@ -288,8 +288,10 @@ fd_sweep_kernel(const __grid_constant__ FdGeom g, const __grid_constant__ FdSwee
     static_assert(!(F32 && (MODE == 2 || EX)), "float32: plain applies only");
     using VT = typename FdVec<F32>::type;  // one 16-byte chunk: double2 or float4
     using WT = typename FdVec<F32>::scalar;
-    constexpr int TY = (NN <= 3) ? 4 : 2;  // rows per thread: 2 NN + 1 accumulator planes x TY rows
-                                           // must fit the registers (nn = 4..6: half-height micro tile)
+    // rows per thread: 2 NN + 1 accumulator planes x TY rows must fit the registers
+    // (nn <= 3: 4 rows, 7 planes; float64 nn = 4: 3 rows, 9 planes; else 2 rows, 9 / 11 / 13 planes:
+    // complex128 nn = 4 with 3 rows spills and runs at half the speed)
+    constexpr int TY = (NN <= 3) ? 4 : ((NN == 4 && !CPLX) ? 3 : 2);
     constexpr int TC = 1;              // 16-byte chunks per thread per row (lane stride 16 B)
     // halo chunks per side along z (a chunk holds 2 / 1 points in double, 4 / 2 points in float)
     constexpr int ZH = F32 ? (NN * (CPLX ? 2 : 1) + 3) / 4 : (CPLX ? NN : (NN + 1) / 2);
