@@ -422,7 +422,7 @@ cudaError_t fd_paw_launch_project(const fd_paw *w, const void *psi, void *coef, 
         ph.im[d] = w->ph_im[d];
     }
     const long long band_d = (long long)w->npoints * (w->cplx ? 2 : 1);
-    const int tile = (w->cplx ? 2 : 1) * (kPawThreads / 32);  // bands per CTA
+    const int tile = 2 * (kPawThreads / 32);  // bands per CTA: 2 per warp
     for (int64_t b0 = 0; b0 < nbands; b0 += 65535LL * tile) {
         const int64_t nb = (nbands - b0 < 65535LL * tile) ? nbands - b0 : 65535LL * tile;
         const dim3 grid((unsigned)w->natoms, (unsigned)((nb + tile - 1) / tile));
@@ -432,7 +432,7 @@ cudaError_t fd_paw_launch_project(const fd_paw *w, const void *psi, void *coef, 
             fd_paw_project_kernel<true, 2, 8><<<grid, kPawThreads, 0, stream>>>(
                 w->atoms, w->idx, w->code, w->proj, p, c, band_d, nb, w->ntot, w->dv, ph);
         else
-            fd_paw_project_kernel<false, 1, 16><<<grid, kPawThreads, 0, stream>>>(
+            fd_paw_project_kernel<false, 2, 16><<<grid, kPawThreads, 0, stream>>>(
                 w->atoms, w->idx, w->code, w->proj, p, c, band_d, nb, w->ntot, w->dv, ph);
         cudaError_t e = cudaPeekAtLastError();
         if (e != cudaSuccess) return e;
