@@ -328,3 +328,12 @@ def vcycle(shape, h, nn: int, bc, p: int, phi: np.ndarray, rhs: np.ndarray, nu1:
     for _ in range(nu2):
         phi = jacobi(shape, hl, nn, bc, phi, rhs, omega, scale)
     return phi
+
+
+def paw_expect(shape, h, bc, k, psi: np.ndarray, box_start, box_size, nproj, proj, dmat) -> np.ndarray:
+    """<psi_b| sum_a sum_ii' |p~_i> dO_ii' <p~_i'| |psi_b> as the plain grid sum
+    sum_r conj(psi_b(r)) (N psi_b)(r) of the non-local term above (no dv, like `expect`): the PAW
+    part of <psi|H~|psi> (Eq. 6 third term, dO = Delta H) or of <psi|S~|psi> (Eq. 7, dO = Delta S).
+    Returned complex; real up to rounding for symmetric dO."""
+    npsi = paw_apply(shape, h, bc, k, psi, box_start, box_size, nproj, proj, dmat)
+    return np.sum(np.conj(psi) * npsi, axis=(1, 2, 3)).astype(np.complex128)

@@ -102,3 +102,20 @@ def test_one_point_projector_and_lattice_translation(oracle):
     nphi = oracle.paw_apply(cfg.shape, cfg.h, cfg.bc, cfg.k, phi, paw.box_start, paw.box_size,
                             paw.nproj, paw.proj, paw.dmat)
     assert abs(np.vdot(phi, ref) - np.conj(np.vdot(psi, nphi))) < 1e-12
+
+
+def test_paw_expectation_value_equals_projection_quadratic_form(oracle):
+    """sum_r conj(psi) (N psi) = (1/dv) P^H dO P with P = dv <p~|psi>: the grid sum against the
+    quadratic form of the projections (two different routes through the oracle's definition)."""
+    cfg = W.custom((9, 8, 10), (0.2, 0.22, 0.18), (1, 0, 1), k=(0.25, 0.0, -0.3), complex_=True, nbands=3)
+    paw = W.make_paw(cfg, 4, nproj=5)
+    psi = W.make_psi(cfg)
+    dv = np.prod(cfg.h)
+    got = oracle.paw_expect(cfg.shape, cfg.h, cfg.bc, cfg.k, psi, paw.box_start, paw.box_size, paw.nproj,
+                            paw.proj, paw.dmat)
+    Pm = _dense_projectors(cfg, paw)
+    D = _block_diag(paw)
+    P = dv * (psi.reshape(3, -1) @ Pm.conj())
+    want = np.einsum("bi,ij,bj->b", P.conj(), D, P) / dv
+    assert np.max(np.abs(got - want)) < 1e-12 * max(1.0, np.abs(want).max())
+    assert np.max(np.abs(got.imag)) < 1e-12 * max(1.0, np.abs(want).max())       # symmetric dO
