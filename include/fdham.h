@@ -246,6 +246,12 @@ FD_API int fd_interpolate(const int32_t shape_fine[3], const int32_t bc[3], int3
  * fd_apply_hamiltonian_paw -- out = -1/2 lap_FD psi + v_eff psi + the Delta H term: the complete
  *   H~ psi~ of Eq. 6 (v_eff == NULL: kinetic + non-local).
  * fd_apply_overlap -- out = psi + sum |p~> Delta S <p~|psi>  (Eq. 7).
+ * fd_paw_expect -- out[b] += (1/dv) Re sum_a P_b[a,:]^H dO^a P_b[a,:] for the projections `coef` of
+ *   fd_paw_project: the PAW part of the grid sum <psi_b|H~|psi_b> (which = 0, Delta H) or of
+ *   <psi_b|S~|psi_b> (which = 1, Delta S).  ACCUMULATES into out (double [nbands], device): applied to
+ *   the eps / norm of fd_apply_hamiltonian_expect it completes them to the PAW Rayleigh quotient
+ *   eps_b / norm_b = <psi|H~|psi> / <psi|S~|psi>, and fd_residual(plan, S~psi, H~psi, eps, norm, r)
+ *   is then the residual H~ psi - lambda S~ psi of the generalised eigenproblem.
  * Errors as fd_apply_hamiltonian; FD_ERR_INVALID also when paw does not belong to a plan of the
  * same grid, dtype and device, or the matrix the call needs was not given at fd_paw_create.
  */
@@ -264,6 +270,8 @@ FD_API int fd_apply_hamiltonian_paw(const fd_plan *plan, const fd_paw *paw, cons
                              void *cuda_stream);
 FD_API int fd_apply_overlap(const fd_plan *plan, const fd_paw *paw, const void *psi, void *out,
                      void *coef, int64_t nbands, void *cuda_stream);
+FD_API int fd_paw_expect(const fd_plan *plan, const fd_paw *paw, int32_t which, const void *coef, double *out,
+                  int64_t nbands, void *cuda_stream);
 
 /*
  * Multigrid V-cycle for lap_FD phi = rhs on the f3 kernels ("multigrid ... Jacobi" Poisson solvers,

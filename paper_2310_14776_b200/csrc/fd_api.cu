@@ -826,6 +826,19 @@ int fd_paw_project(const fd_plan *plan, const fd_paw *paw, const void *psi, void
     return paw_finish(plan, fd_paw_launch_project(paw, psi, coef, nbands, (cudaStream_t)cuda_stream, &n), n);
 }
 
+int fd_paw_expect(const fd_plan *plan, const fd_paw *paw, int32_t which, const void *coef, double *out,
+                  int64_t nbands, void *cuda_stream)
+{
+    if (!plan || !paw || nbands < 0 || (which != 0 && which != 1)) return FD_ERR_INVALID;
+    if (!fd_paw_matches(paw, plan) || !fd_paw_has(paw, which)) return FD_ERR_INVALID;
+    if (nbands == 0) return FD_OK;
+    if (!coef || !out || ((uintptr_t)coef & 15) || ((uintptr_t)out & 7)) return FD_ERR_INVALID;
+    const int drc = check_device(plan);
+    if (drc != FD_OK) return drc;
+    int n = 0;
+    return paw_finish(plan, fd_paw_launch_expect(paw, which, coef, out, nbands, (cudaStream_t)cuda_stream, &n), n);
+}
+
 // out += sum |p~> dO <p~|psi>, which: 0 = Delta H, 1 = Delta S
 static int paw_add(const fd_plan *plan, const fd_paw *paw, int which, const void *psi, void *out,
                    void *coef, int64_t nbands, cudaStream_t stream)

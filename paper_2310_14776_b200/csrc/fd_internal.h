@@ -139,5 +139,7 @@ int fd_paw_has(const fd_paw *w, int which);            // which: 0 = Delta H, 1 
 int fd_paw_matches(const fd_paw *w, const fd_plan *plan);
 cudaError_t fd_paw_launch_project(const fd_paw *w, const void *psi, void *coef, int64_t nbands,
                                   cudaStream_t stream, int *nlaunches);
+cudaError_t fd_paw_launch_expect(const fd_paw *w, int which, const void *coef, double *out, int64_t nbands,
+                                 cudaStream_t stream, int *nlaunches);
 cudaError_t fd_paw_launch_add(const fd_paw *w, int which, const void *coef, void *out, int64_t nbands,
                               cudaStream_t stream, int *nlaunches);

@@ -45,6 +45,7 @@ struct fd_paw {
     unsigned char *code; // device: bit d set = wrapped along axis d (nullptr when no Bloch phases)
     double *proj, *dH, *dS;
     int *colour_atoms;   // device: atom ids grouped by colour
+    int *row_atom;       // device: atom of every row of P (ntot entries)
     std::vector<int> colour_start;  // host: ncolours + 1 offsets into colour_atoms
 };
 
@@ -241,6 +242,45 @@ fd_paw_add_kernel(const PawAtom *__restrict__ atoms, const int *__restrict__ col
     }
 }
 
+// grid (bands): out[b] += (1/dv) Re sum_a sum_ii' conj(P_b[a,i]) dO^a_ii' P_b[a,i'] -- the PAW part of
+// <psi_b|H~|psi_b> (or of <psi_b|S~|psi_b>) from the projections.  One CTA per band, threads over
+// (atom, i) rows in a fixed order, fixed shuffle / shared-memory tree: deterministic.
+template <bool CPLX>
+__global__ void __launch_bounds__(kPawThreads)
+fd_paw_expect_kernel(const PawAtom *__restrict__ atoms, int natoms, const int *__restrict__ row_atom,
+                     const double *__restrict__ dmat, const double *__restrict__ coef,
+                     double *__restrict__ out, int ntot, double inv_dv)
+{
+    constexpr int E = CPLX ? 2 : 1;
+    const long long b = blockIdx.x;
+    const double *c = coef + b * ntot * E;
+    double s = 0.0;
+    for (int row = threadIdx.x; row < ntot; row += kPawThreads) {
+        const PawAtom at = atoms[row_atom[row]];
+        const int i = row - at.coef_off;
+        const double *m = dmat + at.dmat_off + i * at.ni;
+        const double *ca = c + at.coef_off * E;
+        double tx = 0.0, ty = 0.0;
+        for (int i2 = 0; i2 < at.ni; ++i2) {
+            tx = fma(m[i2], ca[i2 * E], tx);
+            if (CPLX) ty = fma(m[i2], ca[i2 * E + 1], ty);
+        }
+        s = fma(ca[i * E], tx, s);                 // Re conj(P_i) t
+        if (CPLX) s = fma(ca[i * E + 1], ty, s);
+    }
+    (void)natoms;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    __shared__ double part[kPawThreads / 32];
+    if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (int w = 0; w < kPawThreads / 32; ++w) t += part[w];
+        out[b] += inv_dv * t;
+    }
+}
+
 template <typename T>
 bool upload(T **dev, const void *host, size_t count)
 {
@@ -290,6 +330,7 @@ int fd_paw_build(fd_paw **out, const fd_plan *plan, int natoms, const int32_t *b
     w->code = nullptr;
     w->proj = w->dH = w->dS = nullptr;
     w->colour_atoms = nullptr;
+    w->row_atom = nullptr;
 
     std::vector<PawAtom> atoms((size_t)natoms);
     std::vector<int> start((size_t)natoms * 3);
@@ -378,6 +419,10 @@ int fd_paw_build(fd_paw **out, const fd_plan *plan, int natoms, const int32_t *b
     bool ok = upload(&w->atoms, atoms.data(), atoms.size()) && upload(&w->idx, idx.data(), idx.size()) &&
               upload(&w->proj, proj_host, (size_t)proj_total) &&
               upload(&w->colour_atoms, order.data(), order.size());
+    std::vector<int> row_atom;
+    for (int a = 0; a < natoms; ++a)
+        for (int i = 0; i < atoms[a].ni; ++i) row_atom.push_back(a);
+    if (ok) ok = upload(&w->row_atom, row_atom.data(), row_atom.size());
     if (ok && w->cplx && w->has_phase) ok = upload(&w->code, code.data(), code.size());
     if (ok && dh_host) ok = upload(&w->dH, dh_host, (size_t)dmat_total);
     if (ok && ds_host) ok = upload(&w->dS, ds_host, (size_t)dmat_total);
@@ -400,6 +445,7 @@ void fd_paw_free(fd_paw *w)
     cudaFree(w->dH);
     cudaFree(w->dS);
     cudaFree(w->colour_atoms);
+    cudaFree(w->row_atom);
     cudaGetLastError();
     delete w;
 }
@@ -472,6 +518,27 @@ cudaError_t fd_paw_launch_add(const fd_paw *w, int which, const void *coef, void
             if (e != cudaSuccess) return e;
             if (nlaunches) ++*nlaunches;
         }
+    }
+    return cudaSuccess;
+}
+
+cudaError_t fd_paw_launch_expect(const fd_paw *w, int which, const void *coef, double *out, int64_t nbands,
+                                 cudaStream_t stream, int *nlaunches)
+{
+    if (w->natoms == 0 || nbands == 0) return cudaSuccess;
+    const double *dm = which ? w->dS : w->dH;
+    for (int64_t b0 = 0; b0 < nbands; b0 += 0x7fffffffLL) {
+        const int64_t nb = (nbands - b0 < 0x7fffffffLL) ? nbands - b0 : 0x7fffffffLL;
+        const double *c = static_cast<const double *>(coef) + b0 * w->ntot * (w->cplx ? 2 : 1);
+        if (w->cplx)
+            fd_paw_expect_kernel<true><<<(unsigned)nb, kPawThreads, 0, stream>>>(
+                w->atoms, w->natoms, w->row_atom, dm, c, out + b0, w->ntot, 1.0 / w->dv);
+        else
+            fd_paw_expect_kernel<false><<<(unsigned)nb, kPawThreads, 0, stream>>>(
+                w->atoms, w->natoms, w->row_atom, dm, c, out + b0, w->ntot, 1.0 / w->dv);
+        cudaError_t e = cudaPeekAtLastError();
+        if (e != cudaSuccess) return e;
+        if (nlaunches) ++*nlaunches;
     }
     return cudaSuccess;
 }

@@ -28,7 +28,7 @@ EXPORTED_SYMBOLS = [
     "fd_apply_hamiltonian_host_ws", "fd_expect_workspace_bytes", "fd_apply_hamiltonian_expect",
     "fd_residual", "fd_jacobi_sweep", "fd_restrict", "fd_interpolate",
     "fd_paw_create", "fd_paw_destroy", "fd_paw_nproj_total", "fd_paw_project", "fd_paw_add_nonlocal",
-    "fd_apply_hamiltonian_paw", "fd_apply_overlap",
+    "fd_apply_hamiltonian_paw", "fd_apply_overlap", "fd_paw_expect",
     "fd_poisson_residual", "fd_mg_create", "fd_mg_destroy", "fd_mg_levels", "fd_mg_vcycle",
     "fd_destroy", "fd_strerror", "fd_plan_set_kernel", "fd_plan_get_kernel", "fd_plan_kernel_for", "fd_plan_launches",
     "fd_plan_get_weights", "fd_plan_get_info",
@@ -99,6 +99,8 @@ def load_library() -> ctypes.CDLL:
     lib.fd_apply_hamiltonian_paw.restype = ctypes.c_int
     lib.fd_apply_overlap.argtypes = [vp, vp, vp, vp, vp, i64, vp]
     lib.fd_apply_overlap.restype = ctypes.c_int
+    lib.fd_paw_expect.argtypes = [vp, vp, i32, vp, vp, i64, vp]
+    lib.fd_paw_expect.restype = ctypes.c_int
     lib.fd_poisson_residual.argtypes = [vp, vp, vp, vp, i64, vp]
     lib.fd_poisson_residual.restype = ctypes.c_int
     lib.fd_mg_create.argtypes = [ctypes.POINTER(vp), i32p, f64p, i32, i32p, i32, i32, i64, i32]
@@ -478,6 +480,15 @@ def fd_mg_vcycle(mg, phi, rhs, nu1: int = 2, nu2: int = 2, nu_coarse: int = 8,
     rc = load_library().fd_mg_vcycle(mg, _dev_ptr(phi), _dev_ptr(rhs), int(phi.shape[0]), int(nu1),
                                      int(nu2), int(nu_coarse), float(omega), _stream_ptr(stream))
     _check(rc, "fd_mg_vcycle")
+
+
+def fd_paw_expect(plan, paw, which: int, coef, out, stream=None) -> None:
+    """out[b] += (1/dv) Re P_b^H dO P_b from the projections coef (which: 0 Delta H, 1 Delta S)."""
+    if tuple(out.shape) != (coef.shape[0],) or str(out.dtype) != "torch.float64":
+        raise ValueError("fd_paw_expect: out must be float64 [nbands]")
+    rc = load_library().fd_paw_expect(plan, paw, int(which), _dev_ptr(coef), _dev_ptr(out),
+                                      int(coef.shape[0]), _stream_ptr(stream))
+    _check(rc, "fd_paw_expect")
 
 
 def fd_plan_set_kernel(plan, kernel: int, param: int = 0) -> None:

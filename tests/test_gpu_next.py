@@ -647,3 +647,57 @@ def test_vcycle_graph_replay_on_a_side_stream_matches_direct_launches(fd):
         assert torch.equal(phi2, ref2)
     finally:
         fd.fd_mg_destroy(mg)
+
+
+@pytest.mark.parametrize("cplx", [False, True])
+def test_paw_rayleigh_quotient_and_generalised_residual(oracle, fd, cplx):
+    """eps / norm of the stencil pass completed by fd_paw_expect to <psi|H~|psi> / <psi|S~|psi>, and
+    the generalised residual H~ psi - lambda S~ psi through fd_residual, against the oracle's sums"""
+    bc = (1, 1, 0)
+    k = (0.25, 0.125, 0.0) if cplx else (0, 0, 0)
+    cfg = W.custom((20, 16, 24), (0.2, 0.22, 0.18), bc, k=k, complex_=cplx, nbands=6)
+    paw = W.make_paw(cfg, 10, nproj=5)
+    ds = W.make_paw(W.custom(cfg.shape, cfg.h_angstrom, bc, k=k, complex_=cplx, nbands=6, index=3), 10,
+                    nproj=5).dmat * 0.1
+    psi, v = W.make_psi(cfg), W.make_veff(cfg)
+    kk = k if cplx else None
+    tdt = torch.complex128 if cplx else torch.float64
+    plan = fd.fd_create(cfg.shape, cfg.h, 3, bc, kk, fd.FD_C128 if cplx else fd.FD_F64, 0)
+    pw = fd.fd_paw_create(plan, paw.box_start, paw.box_size, paw.nproj, paw.proj, paw.dmat, ds)
+    try:
+        d_psi, d_v = torch.from_numpy(psi).cuda(), torch.from_numpy(v).cuda()
+        hpsi, spsi = torch.empty_like(d_psi), torch.empty_like(d_psi)
+        eps = torch.empty(6, dtype=torch.float64, device="cuda")
+        nrm = torch.empty_like(eps)
+        ws = torch.empty(fd.fd_expect_workspace_bytes(plan, 6) // 8 + 2, dtype=torch.float64, device="cuda")
+        coef = torch.empty((6, paw.ntot), dtype=tdt, device="cuda")
+        fd.fd_apply_hamiltonian_expect(plan, d_psi, d_v, hpsi, eps, nrm, ws)     # local part + sums
+        fd.fd_paw_project(plan, pw, d_psi, coef)
+        fd.fd_paw_expect(plan, pw, 0, coef, eps)                                  # + <psi|N_H|psi>
+        fd.fd_paw_expect(plan, pw, 1, coef, nrm)                                  # + <psi|N_S|psi>
+        fd.fd_paw_add_nonlocal(plan, pw, d_psi, hpsi, coef)                       # H~ psi
+        fd.fd_apply_overlap(plan, pw, d_psi, spsi, coef)                          # S~ psi
+        r = torch.empty_like(d_psi)
+        fd.fd_residual(plan, spsi, hpsi, eps, nrm, r)
+        torch.cuda.synchronize()
+        w_eps, w_n = oracle.expect(cfg.shape, cfg.h, 3, bc, kk, psi, v)
+        args = (cfg.shape, cfg.h, bc, kk, psi, paw.box_start, paw.box_size, paw.nproj, paw.proj)
+        w_eps = w_eps.real + oracle.paw_expect(*args, paw.dmat).real
+        w_n = w_n + oracle.paw_expect(*args, ds).real
+        te, tn = expect_tol(cfg.h, 3, psi, v)
+        tp = paw_tol(cfg, paw, psi, paw.dmat) * psi[0].size * np.abs(psi).max()
+        assert np.max(np.abs(eps.cpu().numpy() - w_eps)) <= te + tp
+        assert np.max(np.abs(nrm.cpu().numpy() - w_n)) <= tn + tp
+        w_h = oracle.apply(cfg.shape, cfg.h, 3, bc, kk, psi, v) + oracle.paw_apply(*args, paw.dmat)
+        w_s = oracle.paw_apply(*args, ds, out=psi)
+        lam = w_eps / w_n
+        w_r = w_h - lam[:, None, None, None] * w_s
+        tol = parity_tol(cfg.h, 3, psi, v) + paw_tol(cfg, paw, psi, paw.dmat) + \
+            np.abs(lam).max() * (paw_tol(cfg, paw, psi, ds) + 1e-14 * np.abs(psi).max())
+        assert np.max(np.abs(r.cpu().numpy() - w_r)) <= tol + 1e-12 * np.abs(w_s).max() * np.abs(lam).max()
+        # residual orthogonal to psi: sum conj(psi) r = 0 by construction of lambda
+        dots = (d_psi.conj() * r).sum(dim=(1, 2, 3))
+        assert float(dots.abs().max()) <= 1e-9 * float(np.abs(w_eps).max())
+    finally:
+        fd.fd_paw_destroy(pw)
+        fd.fd_destroy(plan)
