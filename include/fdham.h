@@ -86,9 +86,9 @@ enum {
  *              data stay real, e.g. the zone-boundary point k = 1/2) or FD_C128; FD_F32 / FD_C64:
  *              the same in single precision: psi, out AND v_eff are float32 /
  *              interleaved float32 pairs, fp32 accumulation, fd_apply_kinetic / fd_apply_hamiltonian
- *              only (every other call returns FD_ERR_UNSUPPORTED), nn <= 3, every axis >= 8,
- *              nz a multiple of 4 (FD_F32) or 2 (FD_C64), FD_F32 at Gamma only: FD_ERR_UNSUPPORTED
- *              at fd_create otherwise (there is no fallback to another precision)
+ *              only (every other call returns FD_ERR_UNSUPPORTED; there is no fallback to another
+ *              precision).  The bandwidth kernel takes nn <= 3, every axis >= 8, nz a multiple of 4
+ *              (FD_F32) or 2 (FD_C64), FD_F32 at Gamma; other plans run on the generic kernel
  *   device     CUDA device ordinal
  * Errors: FD_ERR_INVALID for any violated constraint above, FD_ERR_UNSUPPORTED for nx > 65535 or
  * ny > 262140 (no kernel of this build launches such a grid), FD_ERR_CUDA if the device cannot be

@@ -227,12 +227,7 @@ int fd_create_scaled(fd_plan **plan_out, const int32_t shape[3], const double h[
     p->kernel = p->sweep.supported ? FD_KERNEL_SWEEP : FD_KERNEL_GENERIC;
     if (tune_value("kernel") == FD_KERNEL_GENERIC) p->kernel = FD_KERNEL_GENERIC;
     if (tune_value("kernel") != 0) p->forced = 1;
-    if (g.f32 && p->kernel != FD_KERNEL_SWEEP) {
-        // float32 / complex64 exist on the sweep kernel only (nn <= 3, whole 16-byte chunks per row,
-        // axes >= 8): no generic float kernel, and no silent fallback to another precision
-        delete p;
-        return FD_ERR_UNSUPPORTED;
-    }
+
     if (p->sweep.supported && fd_sweep_prepare(p) != cudaSuccess) {
         cudaGetLastError();
         delete p;
@@ -913,7 +908,6 @@ int fd_plan_set_kernel(fd_plan *plan, int32_t kernel, int32_t param)
 {
     if (!plan) return FD_ERR_INVALID;
     if (kernel == FD_KERNEL_GENERIC) {
-        if (plan->g.f32) return FD_ERR_UNSUPPORTED;  // no generic float32 kernel
         plan->kernel = FD_KERNEL_GENERIC;
         plan->forced = 1;
         return FD_OK;

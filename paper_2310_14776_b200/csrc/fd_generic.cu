@@ -9,56 +9,64 @@
 
 namespace {
 
-template <bool CPLX>
+// One grid value: T = double (float64 / complex128) or float (float32 / complex64); CPLX = (re, im).
+template <bool CPLX, typename T>
 struct Val;
-template <>
-struct Val<false> {
-    double x;
-    __device__ __forceinline__ static Val zero() { return {0.0}; }
-    __device__ __forceinline__ void fma(double w, const Val &o) { x = ::fma(w, o.x, x); }
+template <typename T>
+struct Val<false, T> {
+    T x;
+    __device__ __forceinline__ static Val zero() { return {T(0)}; }
+    __device__ __forceinline__ void fma(T w, const Val &o) { x = w * o.x + x; }  // contracted to an FMA
     // real data: the Bloch factor is +1 or -1 (k_d = 1/2), its imaginary part 0
-    __device__ __forceinline__ Val mulphase(double pr, double) const { return {x * pr}; }
+    __device__ __forceinline__ Val mulphase(T pr, T) const { return {x * pr}; }
 };
-template <>
-struct Val<true> {
-    double x, y;
-    __device__ __forceinline__ static Val zero() { return {0.0, 0.0}; }
-    __device__ __forceinline__ void fma(double w, const Val &o)
+template <typename T>
+struct Val<true, T> {
+    T x, y;
+    __device__ __forceinline__ static Val zero() { return {T(0), T(0)}; }
+    __device__ __forceinline__ void fma(T w, const Val &o)
     {
-        x = ::fma(w, o.x, x);
-        y = ::fma(w, o.y, y);
+        x = w * o.x + x;
+        y = w * o.y + y;
     }
-    __device__ __forceinline__ Val mulphase(double pr, double pi) const
+    __device__ __forceinline__ Val mulphase(T pr, T pi) const
     {
         return {x * pr - y * pi, x * pi + y * pr};
     }
 };
 
-template <bool CPLX>
-__device__ __forceinline__ Val<CPLX> load(const double *p, long long idx);
+template <typename T>
+struct Pair;  // the 2-vector of T: one complex value moves as one 16- / 8-byte access
 template <>
-__device__ __forceinline__ Val<false> load<false>(const double *p, long long idx)
-{
-    return {__ldg(p + idx)};
-}
+struct Pair<double> {
+    typedef double2 type;
+};
 template <>
-__device__ __forceinline__ Val<true> load<true>(const double *p, long long idx)
-{
-    const double2 t = __ldg(reinterpret_cast<const double2 *>(p) + idx);
-    return {t.x, t.y};
-}
+struct Pair<float> {
+    typedef float2 type;
+};
 
-template <bool CPLX>
-__device__ __forceinline__ void store(double *p, long long idx, const Val<CPLX> &v);
-template <>
-__device__ __forceinline__ void store<false>(double *p, long long idx, const Val<false> &v)
+template <bool CPLX, typename T>
+__device__ __forceinline__ Val<CPLX, T> load(const T *p, long long idx)
 {
-    p[idx] = v.x;
+    if constexpr (CPLX) {
+        const typename Pair<T>::type t = __ldg(reinterpret_cast<const typename Pair<T>::type *>(p) + idx);
+        return {t.x, t.y};
+    } else {
+        return {__ldg(p + idx)};
+    }
 }
-template <>
-__device__ __forceinline__ void store<true>(double *p, long long idx, const Val<true> &v)
+template <bool CPLX, typename T>
+__device__ __forceinline__ void store(T *p, long long idx, const Val<CPLX, T> &v)
 {
-    reinterpret_cast<double2 *>(p)[idx] = make_double2(v.x, v.y);
+    if constexpr (CPLX) {
+        typename Pair<T>::type t;
+        t.x = v.x;
+        t.y = v.y;
+        reinterpret_cast<typename Pair<T>::type *>(p)[idx] = t;
+    } else {
+        p[idx] = v.x;
+    }
 }
 
 // Block = 64 z-points x 4 rows of one x plane (neighbours along z and y share L1 lines); the
@@ -68,11 +76,11 @@ constexpr int kBx = 64, kBy = 4;
 
 // MODE 0: T psi; 1: + v_eff psi (v_eff[nx,ny,nz]); 2: the weighted-Jacobi form, v_eff = the right-hand
 // side [nbands,nx,ny,nz], added as g.rhs_coef * rhs (g carries the pre-scaled weights; real only).
-template <bool CPLX, int MODE, int NN>
+// T: double, or float for FD_F32 / FD_C64 (psi, out AND v_eff are then float, fp32 accumulation).
+template <bool CPLX, int MODE, int NN, typename T>
 __global__ void __launch_bounds__(kBx * kBy)
-fd_generic_kernel(const __grid_constant__ FdGeom g, const double *__restrict__ psi,
-                  const double *__restrict__ v_eff, double *__restrict__ out, long long nbands,
-                  int bgroups)
+fd_generic_kernel(const __grid_constant__ FdGeom g, const T *__restrict__ psi,
+                  const T *__restrict__ v_eff, T *__restrict__ out, long long nbands, int bgroups)
 {
     constexpr bool HAS_V = MODE == 1;
     const int iz = blockIdx.x * kBx + threadIdx.x;
@@ -84,46 +92,46 @@ fd_generic_kernel(const __grid_constant__ FdGeom g, const double *__restrict__ p
     const long long lin = ((long long)ix * g.n[1] + iy) * g.n[2] + iz;
     const int idx[3] = {ix, iy, iz};
     const long long stride[3] = {(long long)g.n[1] * g.n[2], (long long)g.n[2], 1};
-    double diag = g.wdiag;
+    T diag = (T)g.wdiag;
     if (HAS_V) diag += __ldg(v_eff + lin);
 
     for (long long b = bg; b < nbands; b += bgroups) {
-        const double *pb = psi + (CPLX ? 2 : 1) * b * P;
-        const Val<CPLX> c = load<CPLX>(pb, lin);
-        Val<CPLX> acc = Val<CPLX>::zero();
+        const T *pb = psi + (CPLX ? 2 : 1) * b * P;
+        const Val<CPLX, T> c = load<CPLX, T>(pb, lin);
+        Val<CPLX, T> acc = Val<CPLX, T>::zero();
         acc.fma(diag, c);
 #pragma unroll
         for (int d = 0; d < 3; ++d) {
             const int n = g.n[d];
 #pragma unroll
             for (int j = 1; j <= NN; ++j) {
-                const double w = g.w[d][j];
+                const T w = (T)g.w[d][j];
                 // upper tap i + j
                 int p = idx[d] + j;
                 if (p < n) {
-                    acc.fma(w, load<CPLX>(pb, lin + j * stride[d]));
+                    acc.fma(w, load<CPLX, T>(pb, lin + j * stride[d]));
                 } else if (g.bc[d] == 1) {
-                    const Val<CPLX> t = load<CPLX>(pb, lin + (long long)(j - n) * stride[d]);
-                    acc.fma(w, t.mulphase(g.ph_re[d], g.ph_im[d]));
+                    const Val<CPLX, T> t = load<CPLX, T>(pb, lin + (long long)(j - n) * stride[d]);
+                    acc.fma(w, t.mulphase((T)g.ph_re[d], (T)g.ph_im[d]));
                 }
                 // lower tap i - j
                 p = idx[d] - j;
                 if (p >= 0) {
-                    acc.fma(w, load<CPLX>(pb, lin - j * stride[d]));
+                    acc.fma(w, load<CPLX, T>(pb, lin - j * stride[d]));
                 } else if (g.bc[d] == 1) {
-                    const Val<CPLX> t = load<CPLX>(pb, lin + (long long)(n - j) * stride[d]);
-                    acc.fma(w, t.mulphase(g.ph_re[d], -g.ph_im[d]));
+                    const Val<CPLX, T> t = load<CPLX, T>(pb, lin + (long long)(n - j) * stride[d]);
+                    acc.fma(w, t.mulphase((T)g.ph_re[d], -(T)g.ph_im[d]));
                 }
             }
         }
-        if constexpr (MODE == 2 && !CPLX) acc.x = ::fma(g.rhs_coef, __ldg(v_eff + b * P + lin), acc.x);
-        store<CPLX>(out, b * P + lin, acc);
+        if constexpr (MODE == 2 && !CPLX) acc.x = (T)g.rhs_coef * __ldg(v_eff + b * P + lin) + acc.x;
+        store<CPLX, T>(out, b * P + lin, acc);
     }
 }
 
-template <bool CPLX, int MODE>
-cudaError_t launch_nn(const FdGeom &g, const double *p, const double *v_eff, double *o,
-                      long long nbands, cudaStream_t stream)
+template <bool CPLX, int MODE, typename T>
+cudaError_t launch_nn(const FdGeom &g, const T *p, const T *v_eff, T *o, long long nbands,
+                      cudaStream_t stream)
 {
     // band groups: enough CTAs to fill the device, blockIdx.z <= 65535
     long long bgroups = nbands;
@@ -136,12 +144,12 @@ cudaError_t launch_nn(const FdGeom &g, const double *p, const double *v_eff, dou
     if (grid.y > 65535) return cudaErrorInvalidConfiguration;
     const int bgi = (int)bgroups;
     switch (g.nn) {
-    case 1: fd_generic_kernel<CPLX, MODE, 1><<<grid, block, 0, stream>>>(g, p, v_eff, o, nbands, bgi); break;
-    case 2: fd_generic_kernel<CPLX, MODE, 2><<<grid, block, 0, stream>>>(g, p, v_eff, o, nbands, bgi); break;
-    case 3: fd_generic_kernel<CPLX, MODE, 3><<<grid, block, 0, stream>>>(g, p, v_eff, o, nbands, bgi); break;
-    case 4: fd_generic_kernel<CPLX, MODE, 4><<<grid, block, 0, stream>>>(g, p, v_eff, o, nbands, bgi); break;
-    case 5: fd_generic_kernel<CPLX, MODE, 5><<<grid, block, 0, stream>>>(g, p, v_eff, o, nbands, bgi); break;
-    case 6: fd_generic_kernel<CPLX, MODE, 6><<<grid, block, 0, stream>>>(g, p, v_eff, o, nbands, bgi); break;
+    case 1: fd_generic_kernel<CPLX, MODE, 1, T><<<grid, block, 0, stream>>>(g, p, v_eff, o, nbands, bgi); break;
+    case 2: fd_generic_kernel<CPLX, MODE, 2, T><<<grid, block, 0, stream>>>(g, p, v_eff, o, nbands, bgi); break;
+    case 3: fd_generic_kernel<CPLX, MODE, 3, T><<<grid, block, 0, stream>>>(g, p, v_eff, o, nbands, bgi); break;
+    case 4: fd_generic_kernel<CPLX, MODE, 4, T><<<grid, block, 0, stream>>>(g, p, v_eff, o, nbands, bgi); break;
+    case 5: fd_generic_kernel<CPLX, MODE, 5, T><<<grid, block, 0, stream>>>(g, p, v_eff, o, nbands, bgi); break;
+    case 6: fd_generic_kernel<CPLX, MODE, 6, T><<<grid, block, 0, stream>>>(g, p, v_eff, o, nbands, bgi); break;
     default: return cudaErrorInvalidConfiguration;
     }
     return cudaPeekAtLastError();
@@ -154,14 +162,25 @@ cudaError_t fd_launch_generic(const fd_plan *plan, const FdGeom &g, int mode, co
 {
     (void)plan;
     if (g.n[0] > 65535) return cudaErrorInvalidConfiguration;
+    if (g.f32) {  // float32 / complex64: plain applies only (second = float v_eff)
+        const float *p = static_cast<const float *>(psi);
+        const float *v = reinterpret_cast<const float *>(second);
+        float *o = static_cast<float *>(out);
+        if (mode == 2) return cudaErrorInvalidValue;
+        if (g.cplx)
+            return mode ? launch_nn<true, 1, float>(g, p, v, o, nbands, stream)
+                        : launch_nn<true, 0, float>(g, p, nullptr, o, nbands, stream);
+        return mode ? launch_nn<false, 1, float>(g, p, v, o, nbands, stream)
+                    : launch_nn<false, 0, float>(g, p, nullptr, o, nbands, stream);
+    }
     const double *p = static_cast<const double *>(psi);
     double *o = static_cast<double *>(out);
     if (g.cplx) {
         if (mode == 2) return cudaErrorInvalidValue;
-        return mode ? launch_nn<true, 1>(g, p, second, o, nbands, stream)
-                    : launch_nn<true, 0>(g, p, nullptr, o, nbands, stream);
+        return mode ? launch_nn<true, 1, double>(g, p, second, o, nbands, stream)
+                    : launch_nn<true, 0, double>(g, p, nullptr, o, nbands, stream);
     }
-    if (mode == 2) return launch_nn<false, 2>(g, p, second, o, nbands, stream);
-    return mode ? launch_nn<false, 1>(g, p, second, o, nbands, stream)
-                : launch_nn<false, 0>(g, p, nullptr, o, nbands, stream);
+    if (mode == 2) return launch_nn<false, 2, double>(g, p, second, o, nbands, stream);
+    return mode ? launch_nn<false, 1, double>(g, p, second, o, nbands, stream)
+                : launch_nn<false, 0, double>(g, p, nullptr, o, nbands, stream);
 }

@@ -802,16 +802,32 @@ def test_float32_full_size_cfg3_grid_and_unsupported_forms(oracle, fd):
     assert np.max(np.abs(got[:1] - oracle.apply(cfg.shape, cfg.h, 3, cfg.bc, None,
                                                  psi32[:1].astype(np.float64), v32.astype(np.float64)))) \
         > 1e3 * parity_tol(cfg.h, 3, psi32[:1].astype(np.float64), v32.astype(np.float64))
-    for shape, nn, dt in [((8, 8, 10), 3, fd.FD_F32), ((8, 8, 9), 3, fd.FD_C64), ((12, 12, 12), 4, fd.FD_F32),
-                          ((6, 12, 12), 3, fd.FD_F32)]:
-        with pytest.raises(fd.FDError) as ei:
-            fd.fd_create(shape, (0.3,) * 3, nn, (1, 1, 1), None, dt, 0)
-        assert ei.value.status == -2
+    # shapes / orders the bandwidth kernel does not take run on the generic kernel in the same precision
+    for shape, nn, cplx, k in [((8, 8, 10), 3, False, None), ((8, 8, 9), 3, True, (0.25, 0.0, -0.3)),
+                               ((12, 12, 12), 4, False, None), ((6, 12, 12), 3, False, None),
+                               ((8, 8, 8), 3, False, (0.5, 0.0, 0.5)), ((7, 8, 9), 6, True, (0.1, 0.2, 0.3))]:
+        c2 = W.custom(shape, (0.3, 0.31, 0.29), (1, 1, 1), k=k or (0, 0, 0), complex_=cplx, nbands=3, nn=nn)
+        p32 = W.make_psi(c2).astype(np.complex64 if cplx else np.float32)
+        v32s = W.make_veff(c2).astype(np.float32)
+        plan = fd.fd_create(shape, c2.h, nn, (1, 1, 1), k, fd.FD_C64 if cplx else fd.FD_F32, 0)
+        try:
+            assert fd.fd_plan_kernel_for(plan, 3) == fd.FD_KERNEL_GENERIC
+            d_p = torch.from_numpy(p32).cuda()
+            d_o = torch.full_like(d_p, float("nan"))
+            fd.fd_apply_hamiltonian(plan, d_p, torch.from_numpy(v32s).cuda(), d_o)
+            torch.cuda.synchronize()
+            want = oracle.apply(shape, c2.h, nn, (1, 1, 1), k if (cplx or k) else None,
+                                p32.astype(np.complex128 if (cplx or k) else np.float64), v32s.astype(np.float64))
+            got = d_o.cpu().numpy()
+            assert got.dtype == p32.dtype
+            assert np.max(np.abs(got - (want if cplx else want.real))) <= tol_f32(c2.h, nn, p32, v32s)
+        finally:
+            fd.fd_destroy(plan)
     plan = fd.fd_create((8, 8, 8), (0.3,) * 3, 3, (1, 1, 1), None, fd.FD_F32, 0)
     try:
-        with pytest.raises(fd.FDError) as ei:
-            fd.fd_plan_set_kernel(plan, fd.FD_KERNEL_GENERIC)
-        assert ei.value.status == -2
+        fd.fd_plan_set_kernel(plan, fd.FD_KERNEL_GENERIC)          # both families exist in fp32
+        assert fd.fd_plan_kernel_for(plan, 2) == fd.FD_KERNEL_GENERIC
+        fd.fd_plan_set_kernel(plan, fd.FD_KERNEL_SWEEP)
         with pytest.raises(fd.FDError) as ei:
             fd.fd_expect_workspace_bytes(plan, 4)
         assert ei.value.status == -2
