@@ -27,10 +27,14 @@ struct TGeom {
 };
 
 // z index of a padded row -> source index in [0, n) or -1 (zero)
+// (one wrap by an add / subtract; the integer modulo -- ~40 instructions, and this is called for every
+// halo word of every staged row -- only for grids shorter than the halo)
 __device__ __forceinline__ int wrap_or_zero(int i, int n, int periodic)
 {
     if (i >= 0 && i < n) return i;
     if (!periodic) return -1;
+    i += (i < 0) ? n : -n;
+    if (i >= 0 && i < n) return i;
     i %= n;
     return i < 0 ? i + n : i;
 }
