@@ -896,3 +896,56 @@ def test_per_batch_kernel_choice_is_near_the_faster_kernel(fd):
         assert fd.fd_plan_kernel_for(plan, 16) == fd.FD_KERNEL_SWEEP
     finally:
         fd.fd_destroy(plan)
+
+
+# ------------------------------------------------------------------------------ seeded random configurations
+
+def test_random_configurations_both_kernels_against_the_oracle(oracle, fd):
+    """80 seeded random plans (shape 8..40 per axis, even nz, any BC mix, nn 1..6, float64 / complex128
+    with random Bloch vectors / float64 at k = 1/2, 1..9 bands, random tile height): the plan's own
+    kernel choice, the forced sweep kernel and the generic kernel against the oracle."""
+    rng = np.random.default_rng(20231014)
+    for trial in range(80):
+        nn = int(rng.integers(1, 7))
+        bc = tuple(int(b) for b in rng.integers(0, 2, 3))
+        shape = tuple(int(max(rng.integers(8, 41), nn)) for _ in range(3))
+        shape = (shape[0], shape[1], shape[2] + (shape[2] & 1))
+        kind = int(rng.integers(0, 3))                      # 0 real Gamma, 1 complex Bloch, 2 real k = 1/2
+        cplx = kind == 1
+        if kind == 1:
+            k = tuple(float(rng.uniform(-0.5, 0.5)) if b else 0.0 for b in bc)
+        elif kind == 2:
+            k = tuple(0.5 * int(rng.integers(0, 2)) if b else 0.0 for b in bc)
+        else:
+            k = (0.0, 0.0, 0.0)
+        nb = int(rng.integers(1, 10))
+        h = tuple(float(x) for x in rng.uniform(0.15, 0.3, 3))
+        cfg = W.custom(shape, h, bc, k=k, complex_=cplx, nbands=nb, nn=nn, index=100 + trial)
+        psi, v = W.make_psi(cfg), (W.make_veff(cfg) if rng.integers(0, 4) else None)
+        kk = k if (cplx or kind == 2) else None
+        want = oracle.apply(cfg.shape, cfg.h, nn, bc, kk, psi.astype(np.complex128) if kind == 2 else psi, v)
+        if kind == 2:
+            assert np.max(np.abs(want.imag)) <= 1e-12 * max(1.0, np.abs(want).max())
+            want = want.real
+        tol = parity_tol(cfg.h, nn, psi, v)
+        tyc = int(rng.choice([0, 0, 4, 8, 12]))
+        for kern in ("auto", fd.FD_KERNEL_SWEEP, fd.FD_KERNEL_GENERIC):
+            plan = fd.fd_create(cfg.shape, cfg.h, nn, bc, kk, fd.FD_C128 if cplx else fd.FD_F64, 0)
+            try:
+                if kern != "auto":
+                    try:
+                        fd.fd_plan_set_kernel(plan, kern, tyc if kern == fd.FD_KERNEL_SWEEP else 0)
+                    except fd.FDError as e:
+                        assert e.status == -2 and kern == fd.FD_KERNEL_SWEEP
+                        continue
+                d_psi = torch.from_numpy(psi).cuda()
+                d_out = torch.full_like(d_psi, float("nan"))
+                if v is None:
+                    fd.fd_apply_kinetic(plan, d_psi, d_out)
+                else:
+                    fd.fd_apply_hamiltonian(plan, d_psi, torch.from_numpy(v).cuda(), d_out)
+                torch.cuda.synchronize()
+                err = float(np.max(np.abs(d_out.cpu().numpy() - want)))
+                assert err <= tol, (trial, shape, bc, nn, kind, k, nb, tyc, kern, err, tol)
+            finally:
+                fd.fd_destroy(plan)
