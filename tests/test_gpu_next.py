@@ -701,3 +701,53 @@ def test_paw_rayleigh_quotient_and_generalised_residual(oracle, fd, cplx):
     finally:
         fd.fd_paw_destroy(pw)
         fd.fd_destroy(plan)
+
+
+# ------------------------------------------------------------------------------ seeded random configurations
+
+def test_random_configurations_of_the_next_rows(oracle, fd):
+    """40 seeded random cases each of: fused expectation values (any BC mix, nn 1..6, real / complex
+    Bloch, random tile height), Jacobi sweeps, restriction + interpolation (any BC mix, p 1..3)."""
+    rng = np.random.default_rng(7741)
+    for trial in range(40):
+        nn = int(rng.integers(1, 7))
+        bc = tuple(int(b) for b in rng.integers(0, 2, 3))
+        shape = tuple(int(max(rng.integers(8, 33), nn)) for _ in range(3))
+        shape = (shape[0], shape[1], shape[2] + (shape[2] & 1))
+        cplx = bool(rng.integers(0, 2))
+        k = tuple(float(rng.uniform(-0.5, 0.5)) if (b and cplx) else 0.0 for b in bc)
+        nb = int(rng.integers(1, 8))
+        h = tuple(float(x) for x in rng.uniform(0.15, 0.3, 3))
+        cfg = W.custom(shape, h, bc, k=k, complex_=cplx, nbands=nb, nn=nn, index=300 + trial)
+        kern = [fd.FD_KERNEL_SWEEP, fd.FD_KERNEL_GENERIC, "auto"][trial % 3]
+        try:
+            check_expect(oracle, fd, cfg, kern, tyc=int(rng.choice([0, 4, 8])) if kern == fd.FD_KERNEL_SWEEP else 0,
+                         with_v=bool(rng.integers(0, 3)))
+        except fd.FDError as e:
+            assert e.status == -2 and kern == fd.FD_KERNEL_SWEEP
+        if not cplx:
+            omega, scale = float(rng.uniform(0.5, 1.0)), float(rng.choice([1.0, -0.5]))
+            phi = W.make_psi(cfg)
+            rhs = W.make_psi(W.custom(shape, h, bc, nbands=nb, nn=nn, index=400 + trial)) * 10.0
+            plan = fd.fd_create_scaled(cfg.shape, cfg.h, nn, bc, None, fd.FD_F64, 0, scale)
+            try:
+                d_out = torch.full((nb,) + shape, float("nan"), dtype=torch.float64, device="cuda")
+                fd.fd_jacobi_sweep(plan, torch.from_numpy(phi).cuda(), torch.from_numpy(rhs).cuda(), d_out, omega)
+                torch.cuda.synchronize()
+                want = oracle.jacobi(cfg.shape, cfg.h, nn, bc, phi, rhs, omega, scale)
+                assert np.max(np.abs(d_out.cpu().numpy() - want)) <= jacobi_tol(cfg.h, nn, phi, rhs, omega, scale)
+            finally:
+                fd.fd_destroy(plan)
+        # grid transfer on an independent random fine grid
+        p = int(rng.integers(1, 4))
+        nc = tuple(int(rng.integers(1, 21)) for _ in range(3))
+        nf = tuple(2 * c if b else 2 * c + 1 for c, b in zip(nc, bc))
+        f = rng.standard_normal((nb,) + nf)
+        c = rng.standard_normal((nb,) + nc)
+        d_c = torch.full((nb,) + nc, float("nan"), dtype=torch.float64, device="cuda")
+        d_f = torch.full((nb,) + nf, float("nan"), dtype=torch.float64, device="cuda")
+        fd.fd_restrict(nf, bc, p, torch.from_numpy(f).cuda(), d_c)
+        fd.fd_interpolate(nf, bc, p, torch.from_numpy(c).cuda(), d_f)
+        torch.cuda.synchronize()
+        assert np.max(np.abs(d_c.cpu().numpy() - oracle.restrict(nf, bc, p, f))) <= transfer_tol(p, f), (trial, nf, bc, p)
+        assert np.max(np.abs(d_f.cpu().numpy() - oracle.interpolate(nf, bc, p, c))) <= transfer_tol(p, c), (trial, nf, bc, p)
