@@ -301,6 +301,37 @@ def parity_after_timing(torch, fd, cfg, plan, d_psi, d_v, v_host, h_psi, per_ban
             "tolerance": "1e-12 (max|psi| S + max|v_eff psi|), S = abs row sum of T"}
 
 
+def hardware_peaks(torch, fd, stream, local):
+    """read-only / write-only / copy bandwidth with float64 vectors and the
+    dependent-free DFMA rate, measured here with the library's own micro-benchmark kernels (2 GiB
+    arrays >> L2; best of 5, CUDA events), with the SM clock sampled under the DFMA load."""
+    n = 1 << 28                                     # doubles per array: 2 GiB
+    a = torch.empty(n, dtype=torch.float64, device="cuda").fill_(1.0)
+    b = torch.empty(n, dtype=torch.float64, device="cuda")
+    sms = torch.cuda.get_device_properties(local).multi_processor_count
+
+    def best(fn, reps=5):
+        return min(_time_stream(torch, stream, fn, 1, 1) for _ in range(reps))
+    out = {}
+    ms = best(lambda: fd.fd_peak_kernel(0, a, b, n, 0, stream))
+    out["read_GBps"] = n * 8 / ms / 1e6
+    ms = best(lambda: fd.fd_peak_kernel(1, a, None, n, 0, stream))
+    out["write_GBps"] = n * 8 / ms / 1e6
+    ms = best(lambda: fd.fd_peak_kernel(2, a, b, n, 0, stream))
+    out["copy_GBps"] = 2 * n * 8 / ms / 1e6
+    iters, blocks = 1 << 14, 8 * sms
+    sampler = ClockSampler(local)
+    sampler.start()
+    ms = best(lambda: fd.fd_peak_kernel(3, a, None, iters, blocks, stream), reps=8)
+    out["dfma_clocks"] = sampler.stop()
+    out["dfma_TFLOPs"] = 2.0 * 8 * iters * blocks * 256 / ms / 1e9
+    out["dfma_Tinstr_per_s"] = out["dfma_TFLOPs"] / 2.0
+    out["how"] = ("fd_peak_kernel: 2 GiB float64 arrays, grid-stride 16-byte accesses, 8 CTAs x 256 threads "
+                  "per SM, best of 5; DFMA: 8 independent chains per thread")
+    del a, b
+    return out
+
+
 def next_rows(torch, W, fd, cfg, plan, d_psi, d_v, d_out, stream, plain_ms, peak):
     """SURVEY 8(f) rows on the headline grid: ms, algorithmic GB/s and fraction of the copy peak."""
     import numpy as np
@@ -528,7 +559,9 @@ def run_ours(args):
                   "3-slot H2D/kernel/D2H ring)"}
 
     extras = rank == 0 and world == 1 and not args.quick
-    parity = rows = None
+    parity = rows = peaks = None
+    if extras and args.peaks:
+        peaks = hardware_peaks(torch, fd, stream, local)
     if extras:
         parity = parity_after_timing(torch, fd, cfg, plan, d_psi, d_v, v_host, h_psi)
     del h_out
@@ -559,7 +592,7 @@ def run_ours(args):
             "config": config_dict(cfg, world), "kernel": kernel,
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
             "roofline": roofline, "cpu_baseline": cpu, "sustained": sustained, "parity": parity,
-            "next_rows": rows, "other_workloads": others,
+            "next_rows": rows, "other_workloads": others, "hardware_peaks": peaks,
         }
         print(json.dumps(line), flush=True)
     if dist is not None:
@@ -579,6 +612,8 @@ def main():
                     help="budget of the cpu_baseline leg")
     ap.add_argument("--sustain-seconds", type=float, default=1.0,
                     help="length of the `sustained` leg (0 = skip)")
+    ap.add_argument("--peaks", action=argparse.BooleanOptionalAction, default=True,
+                    help="measure read / write / copy bandwidth and the DFMA rate (hardware_peaks)")
     ap.add_argument("--quick", action="store_true",
                     help="headline, sustained and e2e only (no parity / next_rows / other_workloads)")
     args = ap.parse_args()

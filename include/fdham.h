@@ -298,6 +298,15 @@ FD_API int32_t fd_mg_levels(const fd_mg *mg);
 FD_API int fd_mg_vcycle(const fd_mg *mg, double *phi, const double *rhs, int64_t nbands, int32_t nu1,
                  int32_t nu2, int32_t nu_coarse, double omega, void *cuda_stream);
 
+/*
+ * fd_peak_kernel -- micro-benchmark kernels behind the roofline denominators (
+ * not on the hot path; timed by bench.py --peaks with CUDA events).  kind 0: read n doubles of a
+ * (b: 1-double sink); 1: write n doubles to a; 2: copy n doubles a -> b; 3: n rounds of 8 independent
+ * DFMA per thread on blocks x 256 threads (a: 1-double sink).  blocks = 0: 8 CTAs per SM.  Device
+ * pointers on the current device, 16-byte aligned; n even.
+ */
+FD_API int fd_peak_kernel(int32_t kind, void *a, void *b, int64_t n, int32_t blocks, void *cuda_stream);
+
 /* fd_destroy -- free the plan; NULL is a no-op.  The caller must have synchronised any stream
  * still running an apply of this plan. */
 FD_API int fd_destroy(fd_plan *plan);

@@ -885,6 +885,24 @@ int fd_apply_overlap(const fd_plan *plan, const fd_paw *paw, const void *psi, vo
     return paw_add(plan, paw, 1, psi, out, coef, nbands, (cudaStream_t)cuda_stream);
 }
 
+int fd_peak_kernel(int32_t kind, void *a, void *b, int64_t n, int32_t blocks, void *cuda_stream)
+{
+    if (kind < 0 || kind > 3 || n < 0 || !a || (kind != 1 && kind != 3 && !b)) return FD_ERR_INVALID;
+    if (((uintptr_t)a | (uintptr_t)b) & 15) return FD_ERR_INVALID;
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+        cudaGetLastError();
+        return FD_ERR_CUDA;
+    }
+    if (fd_peak_launch(kind, static_cast<double *>(a), static_cast<double *>(b), n, blocks, sms,
+                       (cudaStream_t)cuda_stream) != cudaSuccess) {
+        cudaGetLastError();
+        return FD_ERR_CUDA;
+    }
+    return FD_OK;
+}
+
 int fd_destroy(fd_plan *plan)
 {
     delete plan;

@@ -143,3 +143,6 @@ cudaError_t fd_paw_launch_expect(const fd_paw *w, int which, const void *coef, d
                                  cudaStream_t stream, int *nlaunches);
 cudaError_t fd_paw_launch_add(const fd_paw *w, int which, const void *coef, void *out, int64_t nbands,
                               cudaStream_t stream, int *nlaunches);
+// fd_peaks.cu: bandwidth / DFMA micro-benchmarks (bench.py --peaks)
+cudaError_t fd_peak_launch(int kind, double *a, double *b, long long n, int blocks, int sm_count,
+                           cudaStream_t stream);

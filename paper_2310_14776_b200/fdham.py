@@ -29,7 +29,7 @@ EXPORTED_SYMBOLS = [
     "fd_residual", "fd_jacobi_sweep", "fd_restrict", "fd_interpolate",
     "fd_paw_create", "fd_paw_destroy", "fd_paw_nproj_total", "fd_paw_project", "fd_paw_add_nonlocal",
     "fd_apply_hamiltonian_paw", "fd_apply_overlap", "fd_paw_expect",
-    "fd_poisson_residual", "fd_mg_create", "fd_mg_destroy", "fd_mg_levels", "fd_mg_vcycle",
+    "fd_peak_kernel", "fd_poisson_residual", "fd_mg_create", "fd_mg_destroy", "fd_mg_levels", "fd_mg_vcycle",
     "fd_destroy", "fd_strerror", "fd_plan_set_kernel", "fd_plan_get_kernel", "fd_plan_kernel_for", "fd_plan_launches",
     "fd_plan_get_weights", "fd_plan_get_info",
 ]
@@ -111,6 +111,8 @@ def load_library() -> ctypes.CDLL:
     lib.fd_mg_levels.restype = ctypes.c_int32
     lib.fd_mg_vcycle.argtypes = [vp, vp, vp, i64, i32, i32, i32, ctypes.c_double, vp]
     lib.fd_mg_vcycle.restype = ctypes.c_int
+    lib.fd_peak_kernel.argtypes = [i32, vp, vp, i64, i32, vp]
+    lib.fd_peak_kernel.restype = ctypes.c_int
     lib.fd_destroy.argtypes = [vp]
     lib.fd_destroy.restype = ctypes.c_int
     lib.fd_strerror.argtypes = [ctypes.c_int]
@@ -489,6 +491,13 @@ def fd_paw_expect(plan, paw, which: int, coef, out, stream=None) -> None:
     rc = load_library().fd_paw_expect(plan, paw, int(which), _dev_ptr(coef), _dev_ptr(out),
                                       int(coef.shape[0]), _stream_ptr(stream))
     _check(rc, "fd_paw_expect")
+
+
+def fd_peak_kernel(kind: int, a, b, n: int, blocks: int = 0, stream=None) -> None:
+    """Micro-benchmark kernels (include/fdham.h: fd_peak_kernel); a, b float64 CUDA tensors."""
+    rc = load_library().fd_peak_kernel(int(kind), _dev_ptr(a), _dev_ptr(b) if b is not None else
+                                       ctypes.c_void_p(0), int(n), int(blocks), _stream_ptr(stream))
+    _check(rc, "fd_peak_kernel")
 
 
 def fd_plan_set_kernel(plan, kernel: int, param: int = 0) -> None:

@@ -751,3 +751,24 @@ def test_random_configurations_of_the_next_rows(oracle, fd):
         torch.cuda.synchronize()
         assert np.max(np.abs(d_c.cpu().numpy() - oracle.restrict(nf, bc, p, f))) <= transfer_tol(p, f), (trial, nf, bc, p)
         assert np.max(np.abs(d_f.cpu().numpy() - oracle.interpolate(nf, bc, p, c))) <= transfer_tol(p, c), (trial, nf, bc, p)
+
+
+def test_peak_microbenchmark_kernels_do_what_they_say(fd):
+    """bench.py's hardware_peaks leg times these: write fills, copy copies, read / DFMA leave memory alone"""
+    n = 1 << 16
+    a = torch.zeros(n, dtype=torch.float64, device="cuda")
+    b = torch.zeros(n, dtype=torch.float64, device="cuda")
+    fd.fd_peak_kernel(1, a, None, n)
+    torch.cuda.synchronize()
+    assert bool((a == 1.5).all())
+    fd.fd_peak_kernel(2, a, b, n)
+    fd.fd_peak_kernel(0, a, b[:2], n)
+    torch.cuda.synchronize()
+    assert bool((b == 1.5).all())
+    sink = torch.zeros(2, dtype=torch.float64, device="cuda")
+    fd.fd_peak_kernel(3, sink, None, 64, 4)
+    torch.cuda.synchronize()
+    assert bool((sink == 0.0).all())
+    with pytest.raises(fd.FDError) as ei:
+        fd.fd_peak_kernel(7, a, b, n)
+    assert ei.value.status == -1
