@@ -385,6 +385,32 @@ def next_rows(torch, W, fd, cfg, plan, d_psi, d_v, d_out, stream, plain_ms, peak
                                                 "2 + 2 Jacobi sweeps per level, p = 3" % (nlev, nt))
         fd.fd_mg_destroy(mg)
         del rhs, phi
+    # f1: the other stencil orders, single precision and the real zone-boundary point on this grid
+    for tag, nn_, dt, kvec in (("f1_nn4", 4, None, None), ("f1_nn6", 6, None, None),
+                               ("f1_single_precision", cfg.nn, "f32", None),
+                               ("f1_real_k_half", cfg.nn, None, (0.5, 0.5, 0.5))):
+        if kvec is not None and (cfg.complex or not all(cfg.bc)):
+            continue
+        if dt == "f32":
+            dtype = fd.FD_C64 if cfg.complex else fd.FD_F32
+            x = d_psi.to(torch.complex64 if cfg.complex else torch.float32)
+            vv = d_v.to(torch.float32)
+        else:
+            dtype = fd.FD_C128 if cfg.complex else fd.FD_F64
+            x, vv = d_psi, d_v
+        kk = kvec if kvec is not None else (cfg.k if cfg.complex else None)
+        pl = fd.fd_create(cfg.shape, cfg.h, nn_, cfg.bc, kk, dtype, torch.cuda.current_device())
+        y = torch.empty_like(x)
+        ms = _time_stream(torch, stream, lambda: fd.fd_apply_hamiltonian(pl, x, vv, y, stream), 20, 3)
+        nbytes = 2 * x.numel() * x.element_size() + vv.numel() * vv.element_size()
+        rows[tag] = entry(ms, nbytes, Gpoint_band_per_s=nb * P / (ms * 1e-3) / 1e9,
+                          kernel=_kernel_name(fd, pl, nb),
+                          what="H psi, nn = %d, %s%s" % (nn_, "fp32" if dt else "fp64",
+                                                        ", float64 at k = (1/2,1/2,1/2)" if kvec else ""))
+        fd.fd_destroy(pl)
+        del y
+        if dt == "f32":
+            del x, vv
     # PAW non-local term: ~1 atom per (9 A)^3 ... synthetic set of 128 atoms x (13 | 11) functions
     paw = W.make_paw(cfg, 128, nproj=13, radius_angstrom=1.1)
     pw = fd.fd_paw_create(plan, paw.box_start, paw.box_size, paw.nproj, paw.proj, paw.dmat, None)
