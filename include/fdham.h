@@ -62,7 +62,8 @@ enum {
     FD_ERR_UNSUPPORTED = -2, /* valid request this build cannot run                               */
     FD_ERR_ALIAS = -3,       /* out overlaps psi or v_eff                                         */
     FD_ERR_CUDA = -4,        /* CUDA runtime failure (no device, launch error, ...)               */
-    FD_ERR_NOMEM = -5        /* host or device allocation failed                                  */
+    FD_ERR_NOMEM = -5,       /* host or device allocation failed                                  */
+    FD_ERR_SCRATCH = -6      /* batch needs more than FD_STATIC_SCRATCH_BYTES of built-in scratch */
 };
 
 /* Kernel families, for fd_plan_set_kernel / fd_plan_get_kernel (diagnostics and A/B timing). */
@@ -174,6 +175,45 @@ FD_API int fd_apply_hamiltonian_expect(const fd_plan *plan, const void *psi, con
                                 int64_t workspace_bytes, void *cuda_stream);
 FD_API int fd_residual(const fd_plan *plan, const void *psi, const void *hpsi, const double *eps,
                 const double *norm, void *r, int64_t nbands, void *cuda_stream);
+
+/*
+ * fd_apply_hamiltonian_expect_static -- fd_apply_hamiltonian_expect without a workspace argument,
+ * for callers that cannot allocate device memory.  Who they are: a plug-in running under a host
+ * application whose memory pool owns the device and which forbids cudaMalloc in plug-ins; code on a
+ * latency path, where cudaMalloc / cudaFree would synchronise the whole device; code whose device
+ * memory belongs to a caching allocator that cannot be reached from C.  Such a caller has nowhere
+ * to get the workspace of fd_apply_hamiltonian_expect from, so the library brings its own: a fixed
+ * array of FD_STATIC_SCRATCH_BYTES (4 MiB) that is part of the library image.  Every GPU on which
+ * the library's code gets loaded holds that array from then until the process exits.
+ *
+ *   plan, psi, v_eff, out, eps, norm, nbands, cuda_stream: as fd_apply_hamiltonian_expect; the
+ *   caller still owns and passes every input and output.  Results are bit-identical to
+ *   fd_apply_hamiltonian_expect on the same arguments (same kernels, same order of additions).
+ *
+ * What the call does not do: it calls no cudaMalloc, cudaFree or other allocating routine, on any
+ * call.  What the first call on each device does in addition: it looks up the device address of
+ * the array (cudaGetSymbolAddress, with the plan's device current) and caches it; the runtime may
+ * load the library's code on that device at that moment.  Make that first call outside any stream
+ * capture.
+ *
+ * Limit: a batch whose partial sums need more than FD_STATIC_SCRATCH_BYTES (the figure
+ * fd_expect_workspace_bytes(plan, nbands) reports) is refused with FD_ERR_SCRATCH before anything
+ * is launched; split the batch, or use fd_apply_hamiltonian_expect with a workspace of your own.
+ * For scale: 96^3 x 256 bands on the fused form needs about 0.22 MiB; the two-pass form (batches on
+ * the generic kernel) needs 16 bytes per band and per 16384 grid values.
+ *
+ * Sharing: all calls on one device use the same array, on whatever stream and for whatever plan,
+ * and the array keeps what the last call wrote (no call depends on it: every value read was stored
+ * earlier in the same call).  Two calls that can overlap on the GPU -- different streams without
+ * an event between them, or different host threads -- race on the array and give wrong eps / norm
+ * (out is unaffected).  Calls on one stream are ordered and safe.
+ * Other errors as fd_apply_hamiltonian_expect (FD_ERR_UNSUPPORTED for FD_F32 / FD_C64 plans,
+ * FD_ERR_INVALID when the plan's device is not current, ...).
+ */
+#define FD_STATIC_SCRATCH_BYTES (4 * 1024 * 1024)
+FD_API int fd_apply_hamiltonian_expect_static(const fd_plan *plan, const void *psi, const double *v_eff,
+                                       void *out, double *eps, double *norm, int64_t nbands,
+                                       void *cuda_stream);
 
 /*
  * fd_jacobi_sweep: one weighted-Jacobi relaxation sweep for A phi = rhs with

@@ -19,7 +19,8 @@ SOURCES = ["fd_sweep_inst_real.cu", "fd_sweep_inst_real_ex.cu",
            "fd_sweep_inst_cplx_ph3_ex.cu", "fd_sweep_inst_real_jacobi.cu", "fd_sweep_inst_real_ph.cu",
            "fd_sweep_inst_real_hi.cu", "fd_sweep_inst_cplx_hi4.cu", "fd_sweep_inst_cplx_hi5.cu",
            "fd_sweep_inst_cplx_hi6.cu", "fd_sweep_inst_f32.cu",
-           "fd_api.cu", "fd_generic.cu", "fd_sweep.cu", "fd_aux.cu", "fd_transfer.cu", "fd_paw.cu", "fd_peaks.cu"]
+           "fd_api.cu", "fd_generic.cu", "fd_sweep.cu", "fd_aux.cu", "fd_transfer.cu", "fd_paw.cu", "fd_peaks.cu",
+           "fd_noalloc.cu"]
 HEADERS = [os.path.join(CSRC, "fd_internal.h"), os.path.join(CSRC, "fd_sweep_kernel.cuh"),
            os.path.join(CSRC, "fd_sweep_inst.h"), os.path.join(ROOT, "include", "fdham.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

@@ -918,6 +918,7 @@ const char *fd_strerror(int status)
     case FD_ERR_ALIAS: return "output overlaps an input";
     case FD_ERR_CUDA: return "CUDA error (no device, or launch/copy failure)";
     case FD_ERR_NOMEM: return "out of memory";
+    case FD_ERR_SCRATCH: return "batch needs more scratch than the library's built-in array holds";
     default: return "unknown fd_status";
     }
 }

@@ -26,6 +26,7 @@ EXPORTED_SYMBOLS = [
     "fd_create", "fd_create_scaled", "fd_apply_kinetic", "fd_apply_hamiltonian",
     "fd_apply_hamiltonian_host", "fd_workspace_create", "fd_workspace_destroy",
     "fd_apply_hamiltonian_host_ws", "fd_expect_workspace_bytes", "fd_apply_hamiltonian_expect",
+    "fd_apply_hamiltonian_expect_static",
     "fd_residual", "fd_jacobi_sweep", "fd_restrict", "fd_interpolate",
     "fd_paw_create", "fd_paw_destroy", "fd_paw_nproj_total", "fd_paw_project", "fd_paw_add_nonlocal",
     "fd_apply_hamiltonian_paw", "fd_apply_overlap", "fd_paw_expect",
@@ -77,6 +78,8 @@ def load_library() -> ctypes.CDLL:
     lib.fd_expect_workspace_bytes.restype = ctypes.c_int64
     lib.fd_apply_hamiltonian_expect.argtypes = [vp, vp, vp, vp, vp, vp, i64, vp, i64, vp]
     lib.fd_apply_hamiltonian_expect.restype = ctypes.c_int
+    lib.fd_apply_hamiltonian_expect_static.argtypes = [vp, vp, vp, vp, vp, vp, i64, vp]
+    lib.fd_apply_hamiltonian_expect_static.restype = ctypes.c_int
     lib.fd_residual.argtypes = [vp, vp, vp, vp, vp, vp, i64, vp]
     lib.fd_residual.restype = ctypes.c_int
     lib.fd_jacobi_sweep.argtypes = [vp, vp, vp, vp, i64, ctypes.c_double, vp]
@@ -311,6 +314,27 @@ def fd_apply_hamiltonian_expect(plan, psi, v_eff, out, eps, norm, workspace, str
         _dev_ptr(out), _dev_ptr(eps), _dev_ptr(norm), int(psi.shape[0]), _dev_ptr(workspace),
         int(workspace.numel() * workspace.element_size()), _stream_ptr(stream))
     _check(rc, "fd_apply_hamiltonian_expect")
+
+
+FD_STATIC_SCRATCH_BYTES = 4 * 1024 * 1024  # include/fdham.h
+FD_ERR_SCRATCH = -6
+
+
+def fd_apply_hamiltonian_expect_static(plan, psi, v_eff, out, eps, norm, stream=None) -> None:
+    """fd_apply_hamiltonian_expect for callers that cannot allocate device memory (a plug-in under a
+    host application that owns the device's memory, a latency path that must not hit the device-wide
+    synchronisation of cudaMalloc / cudaFree): no workspace argument, the partial sums go to a
+    4 MiB array built into libfdham.so.  Same results, bit for bit.  Batches that need more raise
+    FDError with status FD_ERR_SCRATCH; calls that overlap on the GPU race on the shared array; the
+    first call per device should come before any stream capture (include/fdham.h has the details)."""
+    _check_arrays(plan, "fd_apply_hamiltonian_expect_static", batch=(psi, out), grid=(v_eff,))
+    for name, t in (("eps", eps), ("norm", norm)):
+        if tuple(t.shape) != (psi.shape[0],) or str(t.dtype) != "torch.float64":
+            raise ValueError(f"fd_apply_hamiltonian_expect_static: {name} must be float64 [nbands]")
+    rc = load_library().fd_apply_hamiltonian_expect_static(
+        plan, _dev_ptr(psi), _dev_ptr(v_eff) if v_eff is not None else ctypes.c_void_p(0),
+        _dev_ptr(out), _dev_ptr(eps), _dev_ptr(norm), int(psi.shape[0]), _stream_ptr(stream))
+    _check(rc, "fd_apply_hamiltonian_expect_static")
 
 
 def fd_residual(plan, psi, hpsi, eps, norm, r, stream=None) -> None:
