@@ -292,8 +292,12 @@ FD_API int fd_interpolate(const int32_t shape_fine[3], const int32_t bc[3], int3
  *   the eps / norm of fd_apply_hamiltonian_expect it completes them to the PAW Rayleigh quotient
  *   eps_b / norm_b = <psi|H~|psi> / <psi|S~|psi>, and fd_residual(plan, S~psi, H~psi, eps, norm, r)
  *   is then the residual H~ psi - lambda S~ psi of the generalised eigenproblem.
- * Errors as fd_apply_hamiltonian; FD_ERR_INVALID also when paw does not belong to a plan of the
- * same grid, dtype and device, or the matrix the call needs was not given at fd_paw_create.
+ * FD_F64 plans with Bloch factors -1 (2 k_d integer) are supported: a box point that wraps such an
+ * axis, and a box that starts an odd number of cells from the home cell along it, take the sign.
+ * Errors as fd_apply_hamiltonian; FD_ERR_INVALID also when paw was built for a plan that differs
+ * from `plan` in shape, spacing, boundaries, k, dtype or device (its index tables, Bloch factors and
+ * dv are the creating plan's), or when the matrix the call needs was not given at fd_paw_create;
+ * FD_ERR_ALIAS also when coef overlaps psi or out.
  */
 typedef struct fd_paw fd_paw;
 FD_API int fd_paw_create(fd_paw **paw, const fd_plan *plan, int32_t natoms, const int32_t *box_start,

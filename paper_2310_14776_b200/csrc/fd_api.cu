@@ -802,6 +802,17 @@ static int paw_args(const fd_plan *plan, const fd_paw *paw, const void *psi, con
     return check_device(plan);
 }
 
+// coef (nbands x ntot elements, written by the projection) must not overlap psi or out
+static int paw_coef_alias(const fd_plan *plan, const fd_paw *paw, const void *psi, const void *out,
+                          const void *coef, int64_t nbands)
+{
+    const size_t elem = plan->g.cplx ? 16 : 8;
+    const size_t nb = (size_t)plan->g.n[0] * plan->g.n[1] * plan->g.n[2] * (size_t)nbands * elem;
+    const size_t nc = (size_t)nbands * (size_t)fd_paw_ntot(paw) * elem;
+    if (overlaps(coef, nc, psi, nb) || (out && overlaps(coef, nc, out, nb))) return FD_ERR_ALIAS;
+    return FD_OK;
+}
+
 static int paw_finish(const fd_plan *plan, cudaError_t e, int n)
 {
     if (e != cudaSuccess) {
@@ -815,8 +826,10 @@ static int paw_finish(const fd_plan *plan, cudaError_t e, int n)
 int fd_paw_project(const fd_plan *plan, const fd_paw *paw, const void *psi, void *coef,
                    int64_t nbands, void *cuda_stream)
 {
-    const int rc = paw_args(plan, paw, psi, coef, nbands);
+    int rc = paw_args(plan, paw, psi, coef, nbands);
     if (rc != FD_OK || nbands == 0) return rc;
+    rc = paw_coef_alias(plan, paw, psi, nullptr, coef, nbands);
+    if (rc != FD_OK) return rc;
     int n = 0;
     return paw_finish(plan, fd_paw_launch_project(paw, psi, coef, nbands, (cudaStream_t)cuda_stream, &n), n);
 }
@@ -852,6 +865,8 @@ int fd_paw_add_nonlocal(const fd_plan *plan, const fd_paw *paw, const void *psi,
     if (rc != FD_OK || nbands == 0) return rc;
     rc = check_apply_args(plan, psi, nullptr, false, out, nbands);
     if (rc != FD_OK) return rc;
+    rc = paw_coef_alias(plan, paw, psi, out, coef, nbands);
+    if (rc != FD_OK) return rc;
     return paw_add(plan, paw, 0, psi, out, coef, nbands, (cudaStream_t)cuda_stream);
 }
 
@@ -862,6 +877,8 @@ int fd_apply_hamiltonian_paw(const fd_plan *plan, const fd_paw *paw, const void 
     int rc = paw_args(plan, paw, psi, coef, nbands);
     if (rc != FD_OK || nbands == 0) return rc;
     rc = check_apply_args(plan, psi, v_eff, false, out, nbands);
+    if (rc != FD_OK) return rc;
+    rc = paw_coef_alias(plan, paw, psi, out, coef, nbands);
     if (rc != FD_OK) return rc;
     rc = apply_device(plan, plan->g, v_eff ? 1 : 0, psi, v_eff, out, nbands, nullptr, nullptr, nullptr,
                       (cudaStream_t)cuda_stream);
@@ -875,6 +892,8 @@ int fd_apply_overlap(const fd_plan *plan, const fd_paw *paw, const void *psi, vo
     int rc = paw_args(plan, paw, psi, coef, nbands);
     if (rc != FD_OK || nbands == 0) return rc;
     rc = check_apply_args(plan, psi, nullptr, false, out, nbands);
+    if (rc != FD_OK) return rc;
+    rc = paw_coef_alias(plan, paw, psi, out, coef, nbands);
     if (rc != FD_OK) return rc;
     const size_t nb = (size_t)plan->g.n[0] * plan->g.n[1] * plan->g.n[2] * (size_t)nbands *
                       (plan->g.cplx ? 16 : 8);

@@ -37,6 +37,8 @@ struct fd_paw {
     int cplx;
     int natoms, ntot, ncolours;
     int has_phase;
+    int n[3], bc[3];     // of the plan the tables were built for (fd_paw_matches)
+    double h[3], k[3];
     size_t npoints;
     double dv;
     double ph_re[3], ph_im[3];
@@ -99,6 +101,17 @@ __device__ __forceinline__ void phase_of(unsigned code, const Phases &ph, double
         }
 }
 
+// float64 plans at k_d = 1/2 (Bloch factors -1): the factor of a wrapped box point is the product of
+// the +-1 of the wrapped axes
+__device__ __forceinline__ double sign_of(unsigned code, const Phases &ph)
+{
+    double s = 1.0;
+#pragma unroll
+    for (int d = 0; d < 3; ++d)
+        if (code & (1u << d)) s *= ph.re[d];
+    return s;
+}
+
 // grid (atoms, tiles of 8 NB bands); coef[b][coef_off + i] = dv sum_r p~_i(r) psi^_b(r).
 // A warp owns NB bands of the atom: lanes run over the box points, every lane keeps NI x NB partial
 // sums (psi is gathered once per point and meets NI projector values), projector functions go by
@@ -143,8 +156,9 @@ fd_paw_project_kernel(const PawAtom *__restrict__ atoms, const int *__restrict__
                     v[b].y = t.x * pi + t.y * pr;
                 }
             } else {
+                const double sg = code ? sign_of(code[at.idx_off + r], ph) : 1.0;
 #pragma unroll
-                for (int b = 0; b < NB; ++b) v[b].x = pb[b][gi];
+                for (int b = 0; b < NB; ++b) v[b].x = pb[b][gi] * sg;
             }
 #pragma unroll
             for (int i = 0; i < NI; ++i) {
@@ -167,7 +181,7 @@ fd_paw_project_kernel(const PawAtom *__restrict__ atoms, const int *__restrict__
                         c[0] = dv * (acc[i][b].x * at.ph0_re - acc[i][b].y * at.ph0_im);
                         c[1] = dv * (acc[i][b].x * at.ph0_im + acc[i][b].y * at.ph0_re);
                     } else {
-                        c[0] = dv * acc[i][b].x;
+                        c[0] = dv * (acc[i][b].x * at.ph0_re);  // +-1 (lattice shift at k = 1/2)
                     }
                 }
             }
@@ -202,7 +216,7 @@ fd_paw_add_kernel(const PawAtom *__restrict__ atoms, const int *__restrict__ col
             d[i][b][0] = sx * at.ph0_re + sy * at.ph0_im;
             d[i][b][E - 1] = sy * at.ph0_re - sx * at.ph0_im;
         } else {
-            d[i][b][0] = sx;
+            d[i][b][0] = sx * at.ph0_re;
         }
     }
     __syncthreads();
@@ -235,9 +249,10 @@ fd_paw_add_kernel(const PawAtom *__restrict__ atoms, const int *__restrict__ col
                     *o = v;
                 }
         } else {
+            const double sg = code ? sign_of(code[at.idx_off + r], ph) : 1.0;
 #pragma unroll
             for (int b = 0; b < NB; ++b)
-                if (b0 + b < nbands) out[(b0 + b) * band_d + gi] += sx[b];
+                if (b0 + b < nbands) out[(b0 + b) * band_d + gi] += sx[b] * sg;
         }
     }
 }
@@ -321,6 +336,10 @@ int fd_paw_build(fd_paw **out, const fd_plan *plan, int natoms, const int32_t *b
     w->dv = plan->h[0] * plan->h[1] * plan->h[2];
     w->has_phase = 0;
     for (int d = 0; d < 3; ++d) {
+        w->n[d] = g.n[d];
+        w->bc[d] = g.bc[d];
+        w->h[d] = plan->h[d];
+        w->k[d] = plan->k[d];
         w->ph_re[d] = g.ph_re[d];
         w->ph_im[d] = g.ph_im[d];
         if (g.bc[d] && (g.ph_re[d] != 1.0 || g.ph_im[d] != 0.0)) w->has_phase = 1;
@@ -340,6 +359,7 @@ int fd_paw_build(fd_paw **out, const fd_plan *plan, int natoms, const int32_t *b
         const int32_t *sz = box_size + 3 * a;
         if (nproj[a] < 1 || nproj[a] > kMaxNi) { delete w; return nproj[a] > kMaxNi ? -2 : -1; }
         double shift_phase = 0.0;
+        int shift_odd = 0;  // float64 plans: parity of the cells moved along the axes with factor -1
         for (int d = 0; d < 3; ++d) {
             if (sz[d] < 1) { delete w; return -1; }
             if (g.bc[d] && sz[d] > g.n[d]) { delete w; return -2; }  // a box may not meet itself
@@ -349,11 +369,16 @@ int fd_paw_build(fd_paw **out, const fd_plan *plan, int natoms, const int32_t *b
                 if (s - w0 * g.n[d] < 0) --w0;  // floor
                 s -= w0 * g.n[d];
                 shift_phase += 2.0 * 3.14159265358979323846264338327950288 * plan->k[d] * (double)w0;
+                if (g.ph_re[d] < 0.0) shift_odd ^= (w0 & 1);
             }
             start[3 * a + d] = s;
         }
         atoms[a].ph0_re = (shift_phase == 0.0) ? 1.0 : cos(shift_phase);
         atoms[a].ph0_im = (shift_phase == 0.0) ? 0.0 : sin(shift_phase);
+        if (!g.cplx) {  // Bloch factors are exactly +-1 (2 k_d integer): no rounding from cos / sin
+            atoms[a].ph0_re = shift_odd ? -1.0 : 1.0;
+            atoms[a].ph0_im = 0.0;
+        }
         const long long np = (long long)sz[0] * sz[1] * sz[2];
         if (np > (1LL << 30)) { delete w; return -2; }
         atoms[a].npts = (int)np;
@@ -423,7 +448,7 @@ int fd_paw_build(fd_paw **out, const fd_plan *plan, int natoms, const int32_t *b
     for (int a = 0; a < natoms; ++a)
         for (int i = 0; i < atoms[a].ni; ++i) row_atom.push_back(a);
     if (ok) ok = upload(&w->row_atom, row_atom.data(), row_atom.size());
-    if (ok && w->cplx && w->has_phase) ok = upload(&w->code, code.data(), code.size());
+    if (ok && w->has_phase) ok = upload(&w->code, code.data(), code.size());
     if (ok && dh_host) ok = upload(&w->dH, dh_host, (size_t)dmat_total);
     if (ok && ds_host) ok = upload(&w->dS, ds_host, (size_t)dmat_total);
     if (!ok) {
@@ -452,10 +477,16 @@ void fd_paw_free(fd_paw *w)
 
 int fd_paw_ntot(const fd_paw *w) { return w->ntot; }
 int fd_paw_has(const fd_paw *w, int which) { return which ? w->dS != nullptr : w->dH != nullptr; }
+// The index tables, Bloch factors and dv belong to the plan the set was built for: another plan is
+// accepted only if it describes the same grid (shape, spacing, boundaries, k, dtype, device).
 int fd_paw_matches(const fd_paw *w, const fd_plan *plan)
 {
-    return w->device == plan->device && w->cplx == plan->g.cplx &&
-           w->npoints == (size_t)plan->g.n[0] * plan->g.n[1] * plan->g.n[2];
+    if (w->device != plan->device || w->cplx != plan->g.cplx) return 0;
+    for (int d = 0; d < 3; ++d)
+        if (w->n[d] != plan->g.n[d] || w->bc[d] != plan->g.bc[d] || w->h[d] != plan->h[d] ||
+            w->k[d] != plan->k[d])
+            return 0;
+    return 1;
 }
 
 cudaError_t fd_paw_launch_project(const fd_paw *w, const void *psi, void *coef, int64_t nbands,

@@ -413,15 +413,31 @@ def test_transfer_argument_errors(fd):
 
 # ------------------------------------------------------------------------------ f4: PAW non-local term
 
-def paw_tol(cfg, paw, psi, dmat):
-    """|d| <= 1e-12 * (sum over an output point's atoms of sum_ii' |p_i| |dO_ii'| * dv sum_r |p_i'| |psi|):
-    bounded with maxima; the projections carry ~npts rounding errors each."""
-    dv = float(np.prod(cfg.h))
-    pmax = float(np.abs(paw.proj).max())
-    npts = int(np.prod(paw.box_size, axis=1).max())
-    ni = int(paw.nproj.max())
-    return 1e-12 * paw.natoms * ni * ni * pmax * pmax * float(np.abs(dmat).max()) * dv * npts * \
-        float(np.abs(psi).max())
+def paw_bound(oracle, cfg, paw, psi, dmat, want_coef=False):
+    """Per output point, the sum of the ABSOLUTE values of every term of the non-local sum:
+    the oracle itself on |p~|, |dO|, |psi| with all Bloch factors 1 (k = None, real data).  A sum of n
+    terms evaluated in float64 in any order is within n u of that (u = 1.1e-16; n < 4000 here: box
+    points + functions), so 1e-12 x this bounds the difference between two correct float64
+    evaluations, and it is computed from the data, not from products of maxima.  With want_coef also
+    the same bound for the projections, dv sum_r |p~_i(r)| |psi(r)|."""
+    return oracle.paw_apply(cfg.shape, cfg.h, cfg.bc, None, np.abs(psi), paw.box_start, paw.box_size,
+                            paw.nproj, np.abs(paw.proj), np.abs(dmat), want_coef=want_coef)
+
+
+def paw_tol(oracle, cfg, paw, psi, dmat):
+    """scalar form: 1e-12 x the largest per-point sum of |terms|"""
+    return 1e-12 * float(paw_bound(oracle, cfg, paw, psi, dmat).max())
+
+
+def assert_tolerance_resolves_single_precision(oracle, cfg, k, paw, psi, dmat, want, bound):
+    """The gate must be able to tell float64 from float32: psi rounded to single precision (the
+    smallest trace fp32 arithmetic could leave) moves the oracle's result by far more than the
+    tolerance the kernel is held to."""
+    psi32 = psi.astype(np.complex64 if np.iscomplexobj(psi) else np.float32).astype(psi.dtype)
+    moved = oracle.paw_apply(cfg.shape, cfg.h, cfg.bc, k, psi32, paw.box_start, paw.box_size,
+                             paw.nproj, paw.proj, dmat)
+    inside = bound > 0
+    assert np.max(np.abs(moved - want)[inside] / bound[inside]) > 100 * 1e-12
 
 
 @pytest.mark.parametrize("bc,cplx", [((1, 1, 1), False), ((1, 1, 1), True), ((1, 0, 1), True),
@@ -443,18 +459,21 @@ def test_paw_nonlocal_term_overlap_and_full_hamiltonian(oracle, fd, bc, cplx):
         coef = torch.full((7, paw.ntot), float("nan"), dtype=tdt, device="cuda")
         want_nl, want_c = oracle.paw_apply(cfg.shape, cfg.h, bc, kk, psi, paw.box_start, paw.box_size,
                                            paw.nproj, paw.proj, paw.dmat, want_coef=True)
-        tol = paw_tol(cfg, paw, psi, paw.dmat)
+        bound, bound_c = paw_bound(oracle, cfg, paw, psi, paw.dmat, want_coef=True)
+        tol = 1e-12 * float(bound.max())
+        assert_tolerance_resolves_single_precision(oracle, cfg, kk, paw, psi, paw.dmat, want_nl, bound)
         # projections
         fd.fd_paw_project(plan, pw, d_psi, coef)
         torch.cuda.synchronize()
-        assert np.max(np.abs(coef.cpu().numpy() - want_c)) <= 1e-12 * np.prod(cfg.h) * \
-            np.prod(paw.box_size, axis=1).max() * np.abs(paw.proj).max() * np.abs(psi).max()
+        assert np.all(np.abs(coef.cpu().numpy() - want_c) <= 1e-12 * bound_c)
         # non-local term added to an existing array
         base = W.make_psi(W.custom(cfg.shape, cfg.h_angstrom, bc, k=k, complex_=cplx, nbands=7, index=8))
         d_out = torch.from_numpy(base).cuda()
         fd.fd_paw_add_nonlocal(plan, pw, d_psi, d_out, coef)
         torch.cuda.synchronize()
-        assert np.max(np.abs(d_out.cpu().numpy() - (base + want_nl))) <= tol + 1e-15 * np.abs(base).max()
+        # point by point: 1e-12 x the sum of |terms| at that point (+ the rounding of base + term);
+        # points outside every box keep base exactly
+        assert np.all(np.abs(d_out.cpu().numpy() - (base + want_nl)) <= 1e-12 * bound + 1e-15 * np.abs(base))
         # full H~ psi~ (Eq. 6) and S~ psi~ (Eq. 7)
         want_h = oracle.apply(cfg.shape, cfg.h, 3, bc, kk, psi, v) + want_nl
         d_out = torch.full_like(d_psi, float("nan"))
@@ -466,7 +485,8 @@ def test_paw_nonlocal_term_overlap_and_full_hamiltonian(oracle, fd, bc, cplx):
         d_out = torch.full_like(d_psi, float("nan"))
         fd.fd_apply_overlap(plan, pw, d_psi, d_out, coef)
         torch.cuda.synchronize()
-        assert np.max(np.abs(d_out.cpu().numpy() - want_s)) <= paw_tol(cfg, paw, psi, ds) + 1e-15 * np.abs(psi).max()
+        assert np.all(np.abs(d_out.cpu().numpy() - want_s) <=
+                      1e-12 * paw_bound(oracle, cfg, paw, psi, ds) + 1e-15 * np.abs(psi))
         # deterministic: same bits on a second call
         d_out2 = torch.full_like(d_psi, float("nan"))
         fd.fd_apply_overlap(plan, pw, d_psi, d_out2, coef)
@@ -478,31 +498,108 @@ def test_paw_nonlocal_term_overlap_and_full_hamiltonian(oracle, fd, bc, cplx):
         fd.fd_destroy(plan)
 
 
-def test_paw_full_size_grid_sampled_bands(oracle, fd):
-    """cfg3's grid, 64 atoms x up to 13 functions, 32 bands: the configuration the bench times;
-    two whole bands against the oracle"""
-    cfg = W.get(3).with_bands(32)
-    paw = W.make_paw(cfg, 64, nproj=13, radius_angstrom=1.1)
+def test_paw_full_size_grid_every_band(oracle, fd):
+    """cfg3's grid, 128 atoms x up to 13 functions, 256 bands -- the configuration bench.py's
+    next_rows times (same seeded projector set): EVERY element of the non-local term of every band
+    against the oracle, point by point within 1e-12 x the sum of |terms| at that point."""
+    cfg = W.get(3)
+    paw = W.make_paw(cfg, 128, nproj=13, radius_angstrom=1.1)
     psi = W.make_psi(cfg)
+    nb = cfg.nbands
     plan = fd.fd_create(cfg.shape, cfg.h, 3, cfg.bc)
     pw = fd.fd_paw_create(plan, paw.box_start, paw.box_size, paw.nproj, paw.proj, paw.dmat, None)
     try:
         d_psi = torch.from_numpy(psi).cuda()
         d_out = torch.zeros_like(d_psi)
-        coef = torch.empty((32, paw.ntot), dtype=torch.float64, device="cuda")
+        coef = torch.empty((nb, paw.ntot), dtype=torch.float64, device="cuda")
         fd.fd_paw_add_nonlocal(plan, pw, d_psi, d_out, coef)
         torch.cuda.synchronize()
         got = d_out.cpu().numpy()
-        for b in (0, 31):
-            want = oracle.paw_apply(cfg.shape, cfg.h, cfg.bc, None, psi[b:b + 1], paw.box_start,
-                                    paw.box_size, paw.nproj, paw.proj, paw.dmat)
-            assert np.max(np.abs(got[b:b + 1] - want)) <= paw_tol(cfg, paw, psi, paw.dmat)
+        worst = 0.0
+        for b0 in range(0, nb, 32):
+            sl = slice(b0, b0 + 32)
+            want, want_c = oracle.paw_apply(cfg.shape, cfg.h, cfg.bc, None, psi[sl], paw.box_start,
+                                            paw.box_size, paw.nproj, paw.proj, paw.dmat, want_coef=True)
+            bound, bound_c = paw_bound(oracle, cfg, paw, psi[sl], paw.dmat, want_coef=True)
+            err = np.abs(got[sl] - want)
+            assert np.all(err <= 1e-12 * bound), b0
+            assert np.all(np.abs(coef[sl].cpu().numpy() - want_c) <= 1e-12 * bound_c), b0
+            inside = bound > 0
+            worst = max(worst, float(np.max(err[inside] / bound[inside])))
+            if b0 == 0:
+                assert_tolerance_resolves_single_precision(oracle, cfg, None, paw, psi[sl], paw.dmat,
+                                                           want, bound)
+        assert worst <= 1e-12
         with pytest.raises(fd.FDError) as ei:                      # Delta S was not given
             fd.fd_apply_overlap(plan, pw, d_psi, d_out, coef)
         assert ei.value.status == -1
     finally:
         fd.fd_paw_destroy(pw)
         fd.fd_destroy(plan)
+
+
+@pytest.mark.parametrize("k", [(0.5, 0.0, 0.0), (0.0, 0.5, 0.5), (0.5, 0.5, 0.5), (-0.5, 1.0, 1.5)])
+def test_paw_real_dtype_at_zone_boundary_k(oracle, fd, k):
+    """FD_F64 plans with Bloch factors -1 (2 k_d integer): a box point that wraps a k_d = 1/2 axis
+    takes the factor -1, and so does a box whose start lies an odd number of cells away from the home
+    cell.  Boxes are placed so that they cross the upper and the lower end of every axis, and some
+    start one or two cells below / above the home cell.  The oracle runs the complex definition on
+    the real input (its imaginary part must vanish)."""
+    for bc in [(1, 1, 1), (1, 0, 1)]:
+        kk = tuple(x if b else 0.0 for x, b in zip(k, bc))
+        cfg = W.custom((12, 14, 16), (0.2, 0.22, 0.18), bc, nbands=5)
+        paw = W.make_paw(cfg, 10, nproj=4)
+        start = paw.box_start.copy()
+        n = np.array(cfg.shape)
+        start[0] = -2                       # crosses the lower end of every axis
+        start[1] = n - 3                    # crosses the upper end
+        start[2] = start[2] - n             # one cell below the home cell (odd shift)
+        start[3] = start[3] + 2 * n         # two cells above (even shift)
+        start[4] = start[4] - 3 * n * np.array([1, 0, 1])   # odd shift along x and z only
+        for d in range(3):
+            if not bc[d]:
+                start[:, d] = paw.box_start[:, d]           # zero-BC axis: no lattice shifts
+        ds = W.make_paw(W.custom(cfg.shape, cfg.h_angstrom, bc, nbands=5, index=3), 10, nproj=4).dmat * 0.1
+        psi, v = W.make_psi(cfg), W.make_veff(cfg)
+        args = (paw.box_size, paw.nproj, paw.proj)
+        want_c, coef_c = oracle.paw_apply(cfg.shape, cfg.h, bc, kk, psi.astype(np.complex128), start,
+                                          *args, paw.dmat, want_coef=True)
+        assert np.max(np.abs(want_c.imag)) <= 1e-13 * np.abs(want_c).max()
+        # the factor matters: the Gamma-point result differs by O(1) where boxes wrap
+        gamma = oracle.paw_apply(cfg.shape, cfg.h, bc, None, psi, start, *args, paw.dmat)
+        if any(kk):
+            assert np.max(np.abs(gamma - want_c.real)) > 1e-3 * np.abs(gamma).max()
+        shifted = type(paw)(start, paw.box_size, paw.nproj, paw.proj, paw.dmat)
+        bound, bound_c = paw_bound(oracle, cfg, shifted, psi, paw.dmat, want_coef=True)
+        plan = fd.fd_create(cfg.shape, cfg.h, 3, bc, kk, fd.FD_F64, 0)
+        pw = fd.fd_paw_create(plan, start, paw.box_size, paw.nproj, paw.proj, paw.dmat, ds)
+        try:
+            d_psi = torch.from_numpy(psi).cuda()
+            coef = torch.full((5, paw.ntot), float("nan"), dtype=torch.float64, device="cuda")
+            fd.fd_paw_project(plan, pw, d_psi, coef)
+            torch.cuda.synchronize()
+            assert np.all(np.abs(coef.cpu().numpy() - coef_c.real) <= 1e-12 * bound_c)
+            d_out = torch.full_like(d_psi, float("nan"))
+            fd.fd_apply_hamiltonian_paw(plan, pw, d_psi, torch.from_numpy(v).cuda(), d_out, coef)
+            torch.cuda.synchronize()
+            want_h = oracle.apply(cfg.shape, cfg.h, 3, bc, kk, psi.astype(np.complex128), v).real + want_c.real
+            assert np.all(np.abs(d_out.cpu().numpy() - want_h) <= 1e-12 * bound + parity_tol(cfg.h, 3, psi, v))
+            want_s = oracle.paw_apply(cfg.shape, cfg.h, bc, kk, psi.astype(np.complex128), start, *args, ds,
+                                      out=psi.astype(np.complex128)).real
+            fd.fd_apply_overlap(plan, pw, d_psi, d_out, coef)
+            torch.cuda.synchronize()
+            assert np.all(np.abs(d_out.cpu().numpy() - want_s) <=
+                          1e-12 * paw_bound(oracle, cfg, shifted, psi, ds) + 1e-15 * np.abs(psi))
+            # the PAW part of <psi|H~|psi> from the projections
+            e = torch.zeros(5, dtype=torch.float64, device="cuda")
+            fd.fd_paw_project(plan, pw, d_psi, coef)
+            fd.fd_paw_expect(plan, pw, 0, coef, e)
+            torch.cuda.synchronize()
+            w_e = np.sum(psi * want_c.real, axis=(1, 2, 3))
+            assert np.max(np.abs(e.cpu().numpy() - w_e)) <= 1e-12 * float(np.sum(np.abs(psi) * bound, axis=(1, 2, 3)).max())
+        finally:
+            fd.fd_paw_destroy(pw)
+            fd.fd_destroy(plan)
 
 
 def test_paw_create_errors(fd):
@@ -522,6 +619,38 @@ def test_paw_create_errors(fd):
             with pytest.raises(fd.FDError) as ei:                  # paw of another grid
                 fd.fd_paw_project(other, pw, x, c)
             assert ei.value.status == -1
+            # same number of points is not enough: permuted shape, other spacing, other boundaries,
+            # other k (float64 at the zone boundary) all carry different tables / factors / dv
+            y = torch.zeros((1, 8, 8, 8), dtype=torch.float64, device="cuda")
+            for kw in [dict(shape=(8, 8, 8), h=(0.4, 0.4, 0.41)), dict(shape=(8, 8, 8), h=(0.4,) * 3, bc=(1, 0, 1)),
+                       dict(shape=(8, 8, 8), h=(0.4,) * 3, k=(0.5, 0.0, 0.0))]:
+                p2 = fd.fd_create(**kw)
+                try:
+                    with pytest.raises(fd.FDError) as ei:
+                        fd.fd_paw_project(p2, pw, y, c)
+                    assert ei.value.status == -1, kw
+                finally:
+                    fd.fd_destroy(p2)
+            perm_a, perm_b = fd.fd_create((8, 12, 16), (0.4,) * 3), fd.fd_create((16, 12, 8), (0.4,) * 3)
+            pw2 = fd.fd_paw_create(perm_a, [[0, 0, 0]], [[2, 2, 2]], [1], np.ones(8), np.ones(1))
+            try:
+                z = torch.zeros((1, 16, 12, 8), dtype=torch.float64, device="cuda")
+                with pytest.raises(fd.FDError) as ei:
+                    fd.fd_paw_project(perm_b, pw2, z, c)
+                assert ei.value.status == -1
+            finally:
+                fd.fd_paw_destroy(pw2)
+                fd.fd_destroy(perm_a)
+                fd.fd_destroy(perm_b)
+            # coef may not overlap psi or out (FD_ERR_ALIAS): views into one buffer
+            buf = torch.zeros(2 * 512 + 2, dtype=torch.float64, device="cuda")
+            psi_v, out_v = buf[:512].view(1, 8, 8, 8), buf[512:1024].view(1, 8, 8, 8)
+            for bad_coef in (buf[0:1].view(1, 1), buf[512:513].view(1, 1)):
+                with pytest.raises(fd.FDError) as ei:
+                    fd.fd_paw_add_nonlocal(plan, pw, psi_v, out_v, bad_coef)
+                assert ei.value.status == -3
+            fd.fd_paw_add_nonlocal(plan, pw, psi_v, out_v, buf[1024:1025].view(1, 1))
+            torch.cuda.synchronize()
         finally:
             fd.fd_paw_destroy(pw)
             fd.fd_destroy(other)
@@ -685,15 +814,15 @@ def test_paw_rayleigh_quotient_and_generalised_residual(oracle, fd, cplx):
         w_eps = w_eps.real + oracle.paw_expect(*args, paw.dmat).real
         w_n = w_n + oracle.paw_expect(*args, ds).real
         te, tn = expect_tol(cfg.h, 3, psi, v)
-        tp = paw_tol(cfg, paw, psi, paw.dmat) * psi[0].size * np.abs(psi).max()
+        tp = paw_tol(oracle, cfg, paw, psi, paw.dmat) * psi[0].size * np.abs(psi).max()
         assert np.max(np.abs(eps.cpu().numpy() - w_eps)) <= te + tp
         assert np.max(np.abs(nrm.cpu().numpy() - w_n)) <= tn + tp
         w_h = oracle.apply(cfg.shape, cfg.h, 3, bc, kk, psi, v) + oracle.paw_apply(*args, paw.dmat)
         w_s = oracle.paw_apply(*args, ds, out=psi)
         lam = w_eps / w_n
         w_r = w_h - lam[:, None, None, None] * w_s
-        tol = parity_tol(cfg.h, 3, psi, v) + paw_tol(cfg, paw, psi, paw.dmat) + \
-            np.abs(lam).max() * (paw_tol(cfg, paw, psi, ds) + 1e-14 * np.abs(psi).max())
+        tol = parity_tol(cfg.h, 3, psi, v) + paw_tol(oracle, cfg, paw, psi, paw.dmat) + \
+            np.abs(lam).max() * (paw_tol(oracle, cfg, paw, psi, ds) + 1e-14 * np.abs(psi).max())
         assert np.max(np.abs(r.cpu().numpy() - w_r)) <= tol + 1e-12 * np.abs(w_s).max() * np.abs(lam).max()
         # residual orthogonal to psi: sum conj(psi) r = 0 by construction of lambda
         dots = (d_psi.conj() * r).sum(dim=(1, 2, 3))
