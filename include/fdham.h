@@ -330,7 +330,10 @@ FD_API int fd_paw_expect(const fd_plan *plan, const fd_paw *paw, int32_t which, 
  *   rhs likewise, no overlap); a sequence of kernel launches on cuda_stream, no synchronisation.
  *   On a non-default stream the sequence is captured into a CUDA graph the first time an argument
  *   set (phi, rhs, nbands, nu1, nu2, nu_coarse, omega) is seen and replayed afterwards (the coarse
- *   levels are launch bound); the last argument set is kept.  Calls on one fd_mg are serialised.
+ *   levels are launch bound); the four most recently used argument sets are kept, so a solver
+ *   that alternates a few right-hand-side buffers re-captures none of them.  On a stream the
+ *   caller is capturing already the launches join the caller's graph.  Calls on one fd_mg are
+ *   serialised.
  *   A single-level hierarchy (a grid that cannot be coarsened) does nu_coarse sweeps.  Errors as fd_jacobi_sweep / fd_restrict;
  *   FD_ERR_INVALID for nbands > max_nbands.
  */
@@ -341,6 +344,10 @@ FD_API int fd_mg_destroy(fd_mg *mg);
 FD_API int32_t fd_mg_levels(const fd_mg *mg);
 FD_API int fd_mg_vcycle(const fd_mg *mg, double *phi, const double *rhs, int64_t nbands, int32_t nu1,
                  int32_t nu2, int32_t nu_coarse, double omega, void *cuda_stream);
+/* fd_mg_get_info: info[0..2] = finest shape; [3] = max_nbands; [4] = device; [5] = levels;
+ *   [6] = graph captures so far; [7] = 1 if graph capture was given up for this hierarchy (direct
+ *   launches).  Lets a binding check phi / rhs before passing raw pointers on. */
+FD_API int fd_mg_get_info(const fd_mg *mg, int64_t info[8]);
 
 /*
  * fd_peak_kernel -- micro-benchmark kernels behind the roofline denominators (

@@ -510,23 +510,35 @@ struct fd_mg {
     double *phi[kMaxLevels], *rhs[kMaxLevels], *tmp[kMaxLevels];  // phi / rhs of level 0: the caller's
     int64_t max_nbands;
     // The cycle is ~15 launches per level and launch bound on the coarse levels: it is captured once
-    // into a CUDA graph per argument set (the last one is kept) and replayed.
+    // into a CUDA graph per argument set and replayed; the last kGraphSlots argument sets are kept
+    // (a solver that alternates a few right-hand-side buffers re-captures none of them).
     struct GraphKey {
         const void *phi, *rhs;
         int64_t nbands;
         int nu1, nu2, nu_coarse;
         double omega;
+        // field by field: the struct has padding bytes, which a memcmp would compare too
+        bool same(const GraphKey &o) const
+        {
+            return phi == o.phi && rhs == o.rhs && nbands == o.nbands && nu1 == o.nu1 &&
+                   nu2 == o.nu2 && nu_coarse == o.nu_coarse && omega == o.omega;
+        }
     };
+    static const int kGraphSlots = 4;
     mutable std::mutex graph_mutex;
-    mutable GraphKey graph_key;
-    mutable cudaGraphExec_t graph_exec;
+    mutable GraphKey graph_key[kGraphSlots];
+    mutable cudaGraphExec_t graph_exec[kGraphSlots];
+    mutable unsigned long long graph_used[kGraphSlots];  // tick of the last launch (least recent goes)
+    mutable unsigned long long graph_tick;
+    mutable long long graph_captures;  // captures so far (diagnostic, fd_mg_get_info)
     mutable bool graph_off;  // capture failed once (e.g. an unsupported stream): launch directly
 };
 
 int fd_mg_destroy(fd_mg *mg)
 {
     if (!mg) return FD_OK;
-    if (mg->graph_exec) cudaGraphExecDestroy(mg->graph_exec);
+    for (int i = 0; i < fd_mg::kGraphSlots; ++i)
+        if (mg->graph_exec[i]) cudaGraphExecDestroy(mg->graph_exec[i]);
     for (int l = 0; l < mg->nlevels; ++l) {
         if (mg->plan[l]) fd_destroy(mg->plan[l]);
         if (l > 0) {
@@ -554,9 +566,14 @@ int fd_mg_create(fd_mg **mg_out, const int32_t shape[3], const double h[3], int3
     fd_mg *mg = new (std::nothrow) fd_mg();
     if (!mg) return FD_ERR_NOMEM;
     mg->nlevels = 0;
-    mg->graph_exec = nullptr;
+    for (int i = 0; i < fd_mg::kGraphSlots; ++i) {
+        mg->graph_exec[i] = nullptr;
+        mg->graph_used[i] = 0;
+        mg->graph_key[i] = fd_mg::GraphKey{nullptr, nullptr, 0, 0, 0, 0, 0.0};
+    }
+    mg->graph_tick = 0;
+    mg->graph_captures = 0;
     mg->graph_off = false;
-    memset(&mg->graph_key, 0, sizeof(mg->graph_key));
     for (int l = 0; l < fd_mg::kMaxLevels; ++l) {
         mg->plan[l] = nullptr;
         mg->phi[l] = mg->rhs[l] = mg->tmp[l] = nullptr;
@@ -593,7 +610,15 @@ int fd_mg_create(fd_mg **mg_out, const int32_t shape[3], const double h[3], int3
             c[d] = bc[d] ? s[d] / 2 : (s[d] - 1) / 2;
             ok = ok && c[d] >= (nn > 2 ? nn : 2);
         }
-        if (!ok) break;
+        if (!ok || l + 1 >= max_levels) break;
+        // both transfers between this level and the next must fit the kernels (z-row limits): fail
+        // here with FD_ERR_UNSUPPORTED rather than in the first fd_mg_vcycle
+        // (the tile choice depends on the batch size: both ends of the allowed range are checked)
+        for (int interp = 0; interp < 2 && rc == FD_OK; ++interp) {
+            rc = fd_transfer_check(interp, s, bc, p, max_nbands);
+            if (rc == FD_OK) rc = fd_transfer_check(interp, s, bc, p, 1);
+        }
+        if (rc != FD_OK) break;
         for (int d = 0; d < 3; ++d) {
             s[d] = c[d];
             hl[d] *= 2.0;
@@ -695,13 +720,33 @@ int fd_mg_vcycle(const fd_mg *mg, double *phi, const double *rhs, int64_t nbands
     // The legacy default stream cannot be captured: launch directly there.
     if (st == nullptr || st == cudaStreamLegacy || mg->graph_off)
         return mg_cycle_launches(mg, phi, rhs, nbands, nu1, nu2, nu_coarse, omega, cuda_stream);
+    // A stream the caller is capturing already: the launches simply join the caller's graph.
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(st, &cap) != cudaSuccess) {
+        cudaGetLastError();
+        return FD_ERR_CUDA;
+    }
+    if (cap != cudaStreamCaptureStatusNone)
+        return mg_cycle_launches(mg, phi, rhs, nbands, nu1, nu2, nu_coarse, omega, cuda_stream);
 
     std::lock_guard<std::mutex> lock(mg->graph_mutex);
     const fd_mg::GraphKey key = {phi, rhs, nbands, nu1, nu2, nu_coarse, omega};
-    if (!mg->graph_exec || memcmp(&key, &mg->graph_key, sizeof(key)) != 0) {
-        if (mg->graph_exec) {
-            cudaGraphExecDestroy(mg->graph_exec);
-            mg->graph_exec = nullptr;
+    int slot = -1;
+    for (int i = 0; i < fd_mg::kGraphSlots; ++i)
+        if (mg->graph_exec[i] && mg->graph_key[i].same(key)) slot = i;
+    if (slot < 0) {
+        // an empty slot, else the least recently launched one
+        slot = 0;
+        for (int i = 0; i < fd_mg::kGraphSlots; ++i) {
+            if (!mg->graph_exec[i]) {
+                slot = i;
+                break;
+            }
+            if (mg->graph_used[i] < mg->graph_used[slot]) slot = i;
+        }
+        if (mg->graph_exec[slot]) {
+            cudaGraphExecDestroy(mg->graph_exec[slot]);
+            mg->graph_exec[slot] = nullptr;
         }
         cudaGraph_t graph = nullptr;
         if (cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
@@ -719,19 +764,38 @@ int fd_mg_vcycle(const fd_mg *mg, double *phi, const double *rhs, int64_t nbands
             mg->graph_off = true;
             return mg_cycle_launches(mg, phi, rhs, nbands, nu1, nu2, nu_coarse, omega, cuda_stream);
         }
-        const cudaError_t ie = cudaGraphInstantiate(&mg->graph_exec, graph, 0);
+        const cudaError_t ie = cudaGraphInstantiate(&mg->graph_exec[slot], graph, 0);
         cudaGraphDestroy(graph);
         if (ie != cudaSuccess) {
             cudaGetLastError();
-            mg->graph_exec = nullptr;
+            mg->graph_exec[slot] = nullptr;
             mg->graph_off = true;
             return mg_cycle_launches(mg, phi, rhs, nbands, nu1, nu2, nu_coarse, omega, cuda_stream);
         }
-        mg->graph_key = key;
+        mg->graph_key[slot] = key;
+        ++mg->graph_captures;
     }
-    if (cudaGraphLaunch(mg->graph_exec, st) != cudaSuccess) {
+    mg->graph_used[slot] = ++mg->graph_tick;
+    if (cudaGraphLaunch(mg->graph_exec[slot], st) != cudaSuccess) {
         cudaGetLastError();
         return FD_ERR_CUDA;
+    }
+    return FD_OK;
+}
+
+int fd_mg_get_info(const fd_mg *mg, int64_t info[8])
+{
+    if (!mg || !info) return FD_ERR_INVALID;
+    info[0] = mg->shape[0][0];
+    info[1] = mg->shape[0][1];
+    info[2] = mg->shape[0][2];
+    info[3] = mg->max_nbands;
+    info[4] = mg->device;
+    info[5] = mg->nlevels;
+    {
+        std::lock_guard<std::mutex> lock(mg->graph_mutex);
+        info[6] = mg->graph_captures;
+        info[7] = mg->graph_off ? 1 : 0;
     }
     return FD_OK;
 }

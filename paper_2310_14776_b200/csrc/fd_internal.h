@@ -128,6 +128,8 @@ cudaError_t fd_launch_sweep(const fd_plan *plan, const FdGeom &g, int mode, cons
 // `shape_fine` and its coarse grid; returns an fd_status value
 int fd_transfer_run(int interp, const int32_t shape_fine[3], const int32_t bc[3], int p,
                     const double *src, double *dst, int64_t nbands, cudaStream_t stream);
+int fd_transfer_check(int interp, const int32_t shape_fine[3], const int32_t bc[3], int p,
+                      int64_t nbands);  // same status without launching (tile / shared-memory fit)
 // fd_paw.cu: PAW non-local term
 struct fd_paw;
 int fd_paw_build(fd_paw **out, const fd_plan *plan, int natoms, const int32_t *box_start,

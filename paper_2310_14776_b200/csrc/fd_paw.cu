@@ -117,7 +117,9 @@ __device__ __forceinline__ double sign_of(unsigned code, const Phases &ph)
 // sums (psi is gathered once per point and meets NI projector values), projector functions go by
 // in chunks of NI; fixed shuffle tree at the end of a chunk.  The 8 warps of a CTA share the atom's
 // projector values through L1.
-template <bool CPLX, int NB, int NI>
+// SG (float64 only): the plan has Bloch factors -1; a separate instantiation so that the Gamma-point
+// code stays exactly what it was (the gather loop is sensitive to anything added to it).
+template <bool CPLX, int NB, int NI, bool SG>
 __global__ void __launch_bounds__(kPawThreads)
 fd_paw_project_kernel(const PawAtom *__restrict__ atoms, const int *__restrict__ idx,
                       const unsigned char *__restrict__ code, const double *__restrict__ proj,
@@ -156,9 +158,14 @@ fd_paw_project_kernel(const PawAtom *__restrict__ atoms, const int *__restrict__
                     v[b].y = t.x * pi + t.y * pr;
                 }
             } else {
-                const double sg = code ? sign_of(code[at.idx_off + r], ph) : 1.0;
+                if constexpr (SG) {
+                    const double sg = sign_of(code[at.idx_off + r], ph);
 #pragma unroll
-                for (int b = 0; b < NB; ++b) v[b].x = pb[b][gi] * sg;
+                    for (int b = 0; b < NB; ++b) v[b].x = pb[b][gi] * sg;
+                } else {
+#pragma unroll
+                    for (int b = 0; b < NB; ++b) v[b].x = pb[b][gi];
+                }
             }
 #pragma unroll
             for (int i = 0; i < NI; ++i) {
@@ -181,7 +188,10 @@ fd_paw_project_kernel(const PawAtom *__restrict__ atoms, const int *__restrict__
                         c[0] = dv * (acc[i][b].x * at.ph0_re - acc[i][b].y * at.ph0_im);
                         c[1] = dv * (acc[i][b].x * at.ph0_im + acc[i][b].y * at.ph0_re);
                     } else {
-                        c[0] = dv * (acc[i][b].x * at.ph0_re);  // +-1 (lattice shift at k = 1/2)
+                        if constexpr (SG)
+                            c[0] = dv * (acc[i][b].x * at.ph0_re);  // +-1 (lattice shift at k = 1/2)
+                        else
+                            c[0] = dv * acc[i][b].x;
                     }
                 }
             }
@@ -189,7 +199,7 @@ fd_paw_project_kernel(const PawAtom *__restrict__ atoms, const int *__restrict__
 }
 
 // grid (atoms of one colour, band tiles); out_b(r') += conj(phase) sum_i p~_i(r) (dO P_b)_i
-template <bool CPLX, int NB>
+template <bool CPLX, int NB, bool SG>
 __global__ void __launch_bounds__(kPawThreads)
 fd_paw_add_kernel(const PawAtom *__restrict__ atoms, const int *__restrict__ colour_atoms,
                   const int *__restrict__ idx, const unsigned char *__restrict__ code,
@@ -216,7 +226,7 @@ fd_paw_add_kernel(const PawAtom *__restrict__ atoms, const int *__restrict__ col
             d[i][b][0] = sx * at.ph0_re + sy * at.ph0_im;
             d[i][b][E - 1] = sy * at.ph0_re - sx * at.ph0_im;
         } else {
-            d[i][b][0] = sx * at.ph0_re;
+            d[i][b][0] = SG ? sx * at.ph0_re : sx;
         }
     }
     __syncthreads();
@@ -249,10 +259,16 @@ fd_paw_add_kernel(const PawAtom *__restrict__ atoms, const int *__restrict__ col
                     *o = v;
                 }
         } else {
-            const double sg = code ? sign_of(code[at.idx_off + r], ph) : 1.0;
+            if constexpr (SG) {
+                const double sg = sign_of(code[at.idx_off + r], ph);
 #pragma unroll
-            for (int b = 0; b < NB; ++b)
-                if (b0 + b < nbands) out[(b0 + b) * band_d + gi] += sx[b] * sg;
+                for (int b = 0; b < NB; ++b)
+                    if (b0 + b < nbands) out[(b0 + b) * band_d + gi] += sx[b] * sg;
+            } else {
+#pragma unroll
+                for (int b = 0; b < NB; ++b)
+                    if (b0 + b < nbands) out[(b0 + b) * band_d + gi] += sx[b];
+            }
         }
     }
 }
@@ -506,10 +522,13 @@ cudaError_t fd_paw_launch_project(const fd_paw *w, const void *psi, void *coef, 
         const double *p = static_cast<const double *>(psi) + b0 * band_d;
         double *c = static_cast<double *>(coef) + b0 * w->ntot * (w->cplx ? 2 : 1);
         if (w->cplx)
-            fd_paw_project_kernel<true, 2, 8><<<grid, kPawThreads, 0, stream>>>(
+            fd_paw_project_kernel<true, 2, 8, false><<<grid, kPawThreads, 0, stream>>>(
+                w->atoms, w->idx, w->code, w->proj, p, c, band_d, nb, w->ntot, w->dv, ph);
+        else if (w->code)  // float64 at k = 1/2
+            fd_paw_project_kernel<false, 2, 16, true><<<grid, kPawThreads, 0, stream>>>(
                 w->atoms, w->idx, w->code, w->proj, p, c, band_d, nb, w->ntot, w->dv, ph);
         else
-            fd_paw_project_kernel<false, 2, 16><<<grid, kPawThreads, 0, stream>>>(
+            fd_paw_project_kernel<false, 2, 16, false><<<grid, kPawThreads, 0, stream>>>(
                 w->atoms, w->idx, w->code, w->proj, p, c, band_d, nb, w->ntot, w->dv, ph);
         cudaError_t e = cudaPeekAtLastError();
         if (e != cudaSuccess) return e;
@@ -538,11 +557,15 @@ cudaError_t fd_paw_launch_add(const fd_paw *w, int which, const void *coef, void
             const double *cf = static_cast<const double *>(coef) + b0 * w->ntot * (w->cplx ? 2 : 1);
             double *o = static_cast<double *>(out) + b0 * band_d;
             if (w->cplx)
-                fd_paw_add_kernel<true, 4><<<grid, kPawThreads, 0, stream>>>(
+                fd_paw_add_kernel<true, 4, false><<<grid, kPawThreads, 0, stream>>>(
+                    w->atoms, w->colour_atoms + w->colour_start[c], w->idx, w->code, w->proj, dm, cf,
+                    o, band_d, nb, w->ntot, ph);
+            else if (w->code)  // float64 at k = 1/2
+                fd_paw_add_kernel<false, 8, true><<<grid, kPawThreads, 0, stream>>>(
                     w->atoms, w->colour_atoms + w->colour_start[c], w->idx, w->code, w->proj, dm, cf,
                     o, band_d, nb, w->ntot, ph);
             else
-                fd_paw_add_kernel<false, 8><<<grid, kPawThreads, 0, stream>>>(
+                fd_paw_add_kernel<false, 8, false><<<grid, kPawThreads, 0, stream>>>(
                     w->atoms, w->colour_atoms + w->colour_start[c], w->idx, w->code, w->proj, dm, cf,
                     o, band_d, nb, w->ntot, ph);
             cudaError_t e = cudaPeekAtLastError();

@@ -14,6 +14,8 @@
 //   interpolation -- gather: the y-z-interpolated coarse plane enters a queue of 2p planes; the
 //                    even fine plane is the plane itself, the odd one the b_j-weighted sum.
 // Each fine value therefore crosses HBM once (plus the tile / chunk halos, which hit L2).
+#include <atomic>
+
 #include "fd_internal.h"
 
 namespace {
@@ -481,16 +483,41 @@ void tile_choice(int pts_per_row, bool interp, int ncx, int ncy, int64_t nbands,
     *ic = (int)((ncx + chunks - 1) / chunks);
 }
 
+// Current device and its SM count; the count is looked up once per device.
+cudaError_t device_sms(int *dev_out, int *sms_out)
+{
+    static std::atomic<int> cached[64];  // 0 = not looked up yet
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    int sms = (dev >= 0 && dev < 64) ? cached[dev].load(std::memory_order_relaxed) : 0;
+    if (sms == 0) {
+        e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        if (e != cudaSuccess) return e;
+        if (dev >= 0 && dev < 64) cached[dev].store(sms, std::memory_order_relaxed);
+    }
+    *dev_out = dev;
+    *sms_out = sms;
+    return cudaSuccess;
+}
+
 template <int P, int NPT>
 cudaError_t launch_npt(bool interp, const TGeom &g, const double *src, double *dst, int64_t nbands,
-                       int jt, int ic, size_t smem, cudaStream_t stream)
+                       int jt, int ic, size_t smem, int dev, cudaStream_t stream)
 {
     const void *fn = interp ? (const void *)fd_interp_kernel<P, NPT> : (const void *)fd_restrict_kernel<P, NPT>;
-    cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, kFdSweepSmemMax);
-    if (e != cudaSuccess) return e;
-    // two CTAs per SM need the shared-memory carve-out at its maximum
-    e = cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
-    if (e != cudaSuccess) return e;
+    // The two function attributes belong to (instantiation, device): set once each, not per call
+    // (the coarse levels of a V-cycle are launch bound).  Bit d of prepared[k]: done on device d.
+    static std::atomic<unsigned long long> prepared[2];
+    const bool tracked = dev >= 0 && dev < 64;
+    if (!tracked || !((prepared[interp ? 1 : 0].load(std::memory_order_acquire) >> dev) & 1ULL)) {
+        cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, kFdSweepSmemMax);
+        if (e != cudaSuccess) return e;
+        // two CTAs per SM need the shared-memory carve-out at its maximum
+        e = cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+        if (e != cudaSuccess) return e;
+        if (tracked) prepared[interp ? 1 : 0].fetch_or(1ULL << dev, std::memory_order_release);
+    }
     const unsigned gx = (unsigned)((g.nc[1] + jt - 1) / jt), gy = (unsigned)((g.nc[0] + ic - 1) / ic);
     if (gy > 65535) return cudaErrorInvalidConfiguration;
     const long long band_f = (long long)g.nf[0] * g.nf[1] * g.nf[2];
@@ -503,19 +530,18 @@ cudaError_t launch_npt(bool interp, const TGeom &g, const double *src, double *d
         else
             fd_restrict_kernel<P, NPT><<<dim3(gx, gy, nb), kThreads, smem, stream>>>(
                 g, src + b0 * band_f, dst + b0 * band_c, jt, ic);
-        e = cudaPeekAtLastError();
+        const cudaError_t e = cudaPeekAtLastError();
         if (e != cudaSuccess) return e;
     }
     return cudaSuccess;
 }
 
+// Tile and shared-memory footprint of a transfer; cudaErrorInvalidConfiguration when a z row is too
+// long for the kernels (fine nz > 682 or so for restriction, coarse nz > 2048 for interpolation).
 template <int P>
-cudaError_t launch(bool interp, const TGeom &g, const double *src, double *dst, int64_t nbands,
-                   cudaStream_t stream)
+cudaError_t transfer_cfg(bool interp, const TGeom &g, int64_t nbands, int sms, int *jt_out, int *ic_out,
+                         size_t *smem_out, int *npt_out)
 {
-    int dev = 0, sms = 148;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     int jt, ic;
     tile_choice(interp ? g.nf[2] : g.nc[2], interp, g.nc[0], g.nc[1], nbands, sms, &jt, &ic);
     const int pts = interp ? (2 * jt + 1) * g.nf[2] : jt * g.nc[2];
@@ -527,13 +553,30 @@ cudaError_t launch(bool interp, const TGeom &g, const double *src, double *dst, 
         smem = sizeof(double) * (size_t)(2 * jt - 1 + 2 * (2 * P - 1)) *
                (2 * (size_t)((g.nf[2] + 2 * (2 * P - g.off[2]) + 5) & ~1) + g.nc[2]);
     if (smem > (size_t)kFdSweepSmemMax) return cudaErrorInvalidConfiguration;
-    const int npt = (pts + kThreads - 1) / kThreads;
-    if (npt <= 1) return launch_npt<P, 1>(interp, g, src, dst, nbands, jt, ic, smem, stream);
-    if (npt <= 2) return launch_npt<P, 2>(interp, g, src, dst, nbands, jt, ic, smem, stream);
-    if (npt <= 3) return launch_npt<P, 3>(interp, g, src, dst, nbands, jt, ic, smem, stream);
-    if (npt <= 4) return launch_npt<P, 4>(interp, g, src, dst, nbands, jt, ic, smem, stream);
-    if (npt <= 6) return launch_npt<P, 6>(interp, g, src, dst, nbands, jt, ic, smem, stream);
-    return launch_npt<P, 8>(interp, g, src, dst, nbands, jt, ic, smem, stream);
+    *jt_out = jt;
+    *ic_out = ic;
+    *smem_out = smem;
+    *npt_out = (pts + kThreads - 1) / kThreads;
+    return cudaSuccess;
+}
+
+template <int P>
+cudaError_t launch(bool interp, const TGeom &g, const double *src, double *dst, int64_t nbands,
+                   cudaStream_t stream)
+{
+    int dev = 0, sms = 148;
+    cudaError_t e = device_sms(&dev, &sms);
+    if (e != cudaSuccess) return e;
+    int jt, ic, npt;
+    size_t smem;
+    e = transfer_cfg<P>(interp, g, nbands, sms, &jt, &ic, &smem, &npt);
+    if (e != cudaSuccess) return e;
+    if (npt <= 1) return launch_npt<P, 1>(interp, g, src, dst, nbands, jt, ic, smem, dev, stream);
+    if (npt <= 2) return launch_npt<P, 2>(interp, g, src, dst, nbands, jt, ic, smem, dev, stream);
+    if (npt <= 3) return launch_npt<P, 3>(interp, g, src, dst, nbands, jt, ic, smem, dev, stream);
+    if (npt <= 4) return launch_npt<P, 4>(interp, g, src, dst, nbands, jt, ic, smem, dev, stream);
+    if (npt <= 6) return launch_npt<P, 6>(interp, g, src, dst, nbands, jt, ic, smem, dev, stream);
+    return launch_npt<P, 8>(interp, g, src, dst, nbands, jt, ic, smem, dev, stream);
 }
 
 }  // namespace
@@ -562,4 +605,29 @@ int fd_transfer_run(int interp, const int32_t shape_fine[3], const int32_t bc[3]
         return -4;
     }
     return 0;
+}
+
+// Would fd_transfer_run accept this transfer on the current device?  0 yes, -1 / -2 / -4 as there.
+// Nothing is launched (fd_mg_create asks for every level, so that a hierarchy whose z rows are too
+// long for the kernels fails at create and not in the first cycle).
+int fd_transfer_check(int interp, const int32_t shape_fine[3], const int32_t bc[3], int p, int64_t nbands)
+{
+    TGeom g;
+    if (p < 1 || p > 3) return (p >= 1 && p <= 6) ? -2 : -1;
+    if (fill_geom(g, shape_fine, bc, p) != 0) return -1;
+    for (int d = 0; d < 3; ++d)
+        if (g.nc[d] < 1) return -1;
+    int dev = 0, sms = 148, jt, ic, npt;
+    size_t smem;
+    if (device_sms(&dev, &sms) != cudaSuccess) {
+        cudaGetLastError();
+        return -4;
+    }
+    cudaError_t e;
+    switch (p) {
+    case 1: e = transfer_cfg<1>(interp != 0, g, nbands, sms, &jt, &ic, &smem, &npt); break;
+    case 2: e = transfer_cfg<2>(interp != 0, g, nbands, sms, &jt, &ic, &smem, &npt); break;
+    default: e = transfer_cfg<3>(interp != 0, g, nbands, sms, &jt, &ic, &smem, &npt); break;
+    }
+    return e == cudaSuccess ? 0 : -2;
 }

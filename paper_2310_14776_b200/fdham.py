@@ -30,7 +30,7 @@ EXPORTED_SYMBOLS = [
     "fd_residual", "fd_jacobi_sweep", "fd_restrict", "fd_interpolate",
     "fd_paw_create", "fd_paw_destroy", "fd_paw_nproj_total", "fd_paw_project", "fd_paw_add_nonlocal",
     "fd_apply_hamiltonian_paw", "fd_apply_overlap", "fd_paw_expect",
-    "fd_peak_kernel", "fd_poisson_residual", "fd_mg_create", "fd_mg_destroy", "fd_mg_levels", "fd_mg_vcycle",
+    "fd_peak_kernel", "fd_poisson_residual", "fd_mg_create", "fd_mg_destroy", "fd_mg_levels", "fd_mg_vcycle", "fd_mg_get_info",
     "fd_destroy", "fd_strerror", "fd_plan_set_kernel", "fd_plan_get_kernel", "fd_plan_kernel_for", "fd_plan_launches",
     "fd_plan_get_weights", "fd_plan_get_info",
 ]
@@ -114,6 +114,8 @@ def load_library() -> ctypes.CDLL:
     lib.fd_mg_levels.restype = ctypes.c_int32
     lib.fd_mg_vcycle.argtypes = [vp, vp, vp, i64, i32, i32, i32, ctypes.c_double, vp]
     lib.fd_mg_vcycle.restype = ctypes.c_int
+    lib.fd_mg_get_info.argtypes = [vp, ctypes.POINTER(ctypes.c_int64)]
+    lib.fd_mg_get_info.restype = ctypes.c_int
     lib.fd_peak_kernel.argtypes = [i32, vp, vp, i64, i32, vp]
     lib.fd_peak_kernel.restype = ctypes.c_int
     lib.fd_destroy.argtypes = [vp]
@@ -175,6 +177,7 @@ def fd_create_scaled(shape: Sequence[int], h: Sequence[float], nn: int = 3,
 
 
 def fd_destroy(plan) -> None:
+    _PLAN_INFO.pop(plan.value if hasattr(plan, "value") else int(plan), None)
     _check(load_library().fd_destroy(plan), "fd_destroy")
 
 
@@ -201,6 +204,20 @@ def fd_plan_get_info(plan) -> dict:
             "bc": (buf[6] & 1, (buf[6] >> 1) & 1, (buf[6] >> 2) & 1), "kernel": buf[7]}
 
 
+# shape / dtype / device of a plan never change after fd_create: one ABI call per handle, not one per
+# apply (the launch-bound small batches would pay for it).  Evicted by fd_destroy.
+_PLAN_INFO: dict = {}
+
+
+def _plan_info(plan) -> dict:
+    key = plan.value if hasattr(plan, "value") else int(plan)
+    info = _PLAN_INFO.get(key)
+    if info is None:
+        info = fd_plan_get_info(plan)
+        _PLAN_INFO[key] = info
+    return info
+
+
 def _torch_dtypes(dtype: int):
     """(torch dtype of psi / out, torch dtype of v_eff) for an FD_* dtype."""
     import torch
@@ -213,7 +230,7 @@ def _check_arrays(plan, where: str, batch=(), grid=(), real=()):
     out-of-bounds access on the device, so the binding checks them against the plan first.
     batch: tensors [nbands, nx, ny, nz] of the plan's dtype (same nbands); grid: [nx, ny, nz] of the
     plan's real dtype; real: batch-shaped tensors of the plan's real dtype."""
-    info = fd_plan_get_info(plan)
+    info = _plan_info(plan)
     shape, (tdt, rdt) = tuple(info["shape"]), _torch_dtypes(info["dtype"])
     nb = None
     for kind, tensors, want_dt in (("batch", batch, tdt), ("real", real, rdt)):
@@ -337,9 +354,17 @@ def fd_apply_hamiltonian_expect_static(plan, psi, v_eff, out, eps, norm, stream=
     _check(rc, "fd_apply_hamiltonian_expect_static")
 
 
+def _check_band_vectors(where: str, psi, **vectors) -> None:
+    """eps / norm style arguments: float64 [nbands] on the device of psi."""
+    for name, t in vectors.items():
+        if tuple(t.shape) != (psi.shape[0],) or str(t.dtype) != "torch.float64" or t.device != psi.device:
+            raise ValueError(f"{where}: {name} must be float64 [{psi.shape[0]}] on {psi.device}")
+
+
 def fd_residual(plan, psi, hpsi, eps, norm, r, stream=None) -> None:
     """r_b = hpsi_b - (eps[b] / norm[b]) psi_b; r may be hpsi itself."""
     _check_arrays(plan, "fd_residual", batch=(psi, hpsi, r))
+    _check_band_vectors("fd_residual", psi, eps=eps, norm=norm)
     rc = load_library().fd_residual(plan, _dev_ptr(psi), _dev_ptr(hpsi), _dev_ptr(eps),
                                     _dev_ptr(norm), _dev_ptr(r), int(psi.shape[0]),
                                     _stream_ptr(stream))
@@ -498,11 +523,25 @@ def fd_mg_levels(mg) -> int:
     return int(load_library().fd_mg_levels(mg))
 
 
+def fd_mg_get_info(mg) -> dict:
+    """Finest shape, max_nbands, device, levels, graph captures so far, whether capture was given up."""
+    buf = (ctypes.c_int64 * 8)()
+    _check(load_library().fd_mg_get_info(mg, buf), "fd_mg_get_info")
+    return {"shape": (buf[0], buf[1], buf[2]), "max_nbands": buf[3], "device": buf[4], "levels": buf[5],
+            "graph_captures": buf[6], "graph_off": bool(buf[7])}
+
+
 def fd_mg_vcycle(mg, phi, rhs, nu1: int = 2, nu2: int = 2, nu_coarse: int = 8,
                  omega: float = 2.0 / 3.0, stream=None) -> None:
     """One V-cycle in place on phi (float64 CUDA tensors [nbands, nx, ny, nz])."""
     if phi.shape != rhs.shape or phi.dtype != rhs.dtype or str(phi.dtype) != "torch.float64":
         raise ValueError("fd_mg_vcycle: phi and rhs must be float64 tensors of the same shape")
+    info = fd_mg_get_info(mg)
+    # (nbands > max_nbands is the library's own check: FD_ERR_INVALID, nothing is touched)
+    if phi.dim() != 4 or tuple(phi.shape[1:]) != info["shape"]:
+        raise ValueError(f"fd_mg_vcycle: expected [nbands, {info['shape']}], got {tuple(phi.shape)}")
+    if phi.device.index != info["device"] or rhs.device.index != info["device"]:
+        raise ValueError(f"fd_mg_vcycle: tensors must be on cuda:{info['device']}")
     rc = load_library().fd_mg_vcycle(mg, _dev_ptr(phi), _dev_ptr(rhs), int(phi.shape[0]), int(nu1),
                                      int(nu2), int(nu_coarse), float(omega), _stream_ptr(stream))
     _check(rc, "fd_mg_vcycle")
@@ -510,8 +549,13 @@ def fd_mg_vcycle(mg, phi, rhs, nu1: int = 2, nu2: int = 2, nu_coarse: int = 8,
 
 def fd_paw_expect(plan, paw, which: int, coef, out, stream=None) -> None:
     """out[b] += (1/dv) Re P_b^H dO P_b from the projections coef (which: 0 Delta H, 1 Delta S)."""
-    if tuple(out.shape) != (coef.shape[0],) or str(out.dtype) != "torch.float64":
-        raise ValueError("fd_paw_expect: out must be float64 [nbands]")
+    info = _plan_info(plan)
+    ntot = fd_paw_nproj_total(paw)
+    if coef.dim() != 2 or coef.shape[1] != ntot or coef.dtype != _torch_dtypes(info["dtype"])[0] or \
+            coef.device.index != info["device"]:
+        raise ValueError(f"fd_paw_expect: coef must be [nbands, {ntot}] of the plan's dtype on its device")
+    if tuple(out.shape) != (coef.shape[0],) or str(out.dtype) != "torch.float64" or out.device != coef.device:
+        raise ValueError("fd_paw_expect: out must be float64 [nbands] on the device of coef")
     rc = load_library().fd_paw_expect(plan, paw, int(which), _dev_ptr(coef), _dev_ptr(out),
                                       int(coef.shape[0]), _stream_ptr(stream))
     _check(rc, "fd_paw_expect")

@@ -744,6 +744,26 @@ def test_poisson_residual_parity_and_mg_errors(oracle, fd):
     assert ei.value.status == -2
 
 
+def test_mg_create_rejects_hierarchies_whose_transfers_do_not_fit(fd):
+    """z rows too long for the transfer kernels (fine nz > ~682): fd_mg_create says
+    FD_ERR_UNSUPPORTED itself instead of the first fd_mg_vcycle; a single level (no transfer) and a
+    long x or y axis are fine."""
+    h = (0.3,) * 3
+    with pytest.raises(fd.FDError) as ei:
+        fd.fd_mg_create((8, 8, 4096), h, 3, (1, 1, 1), 2, 16, 1, 0)
+    assert ei.value.status == -2
+    for shape, levels in [((8, 8, 4096), 1), ((1024, 8, 8), 16), ((8, 1024, 8), 16)]:
+        mg = fd.fd_mg_create(shape, h, 3, (1, 1, 1), 2, levels, 1, 0)
+        try:
+            phi = torch.zeros((1,) + shape, dtype=torch.float64, device="cuda")
+            rhs = torch.randn((1,) + shape, dtype=torch.float64, device="cuda")
+            fd.fd_mg_vcycle(mg, phi, rhs - rhs.mean())
+            torch.cuda.synchronize()
+            assert bool(torch.isfinite(phi).all())
+        finally:
+            fd.fd_mg_destroy(mg)
+
+
 def test_vcycle_graph_replay_on_a_side_stream_matches_direct_launches(fd):
     """On a non-default stream the cycle is captured into a CUDA graph and replayed: same bits as the
     direct launches on the default stream, also after the argument set changes."""
@@ -774,6 +794,34 @@ def test_vcycle_graph_replay_on_a_side_stream_matches_direct_launches(fd):
         fd.fd_mg_vcycle(mg, ref2, rhs, 1, 1, 4, 0.8)
         torch.cuda.synchronize()
         assert torch.equal(phi2, ref2)
+        # capture bookkeeping: one capture per argument set, none on replays, and a solver that
+        # alternates buffers (here 4 argument sets round robin) re-captures none of them
+        info = fd.fd_mg_get_info(mg)
+        assert info["shape"] == n and info["max_nbands"] == 2 and info["levels"] == fd.fd_mg_levels(mg)
+        assert not info["graph_off"] and info["graph_captures"] == 2
+        bufs = [torch.zeros_like(rhs) for _ in range(4)]
+        for rounds in range(3):
+            for b in bufs:
+                fd.fd_mg_vcycle(mg, b, rhs, stream=s)
+        s.synchronize()
+        assert fd.fd_mg_get_info(mg)["graph_captures"] == 2 + 4
+        for b in bufs:
+            assert torch.equal(b, ref)                           # 3 cycles each, as ref
+        # a stream the caller is capturing: the launches join the caller's graph, nothing breaks
+        phi3 = torch.zeros_like(rhs)
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            fd.fd_mg_vcycle(mg, phi3, rhs, stream=s)
+        for _ in range(3):
+            g.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(phi3, ref)
+        info = fd.fd_mg_get_info(mg)
+        assert not info["graph_off"] and info["graph_captures"] == 6
+        # the binding checks phi / rhs against the hierarchy before passing raw pointers on
+        with pytest.raises(ValueError):
+            fd.fd_mg_vcycle(mg, torch.zeros((2, 32, 32, 16), dtype=torch.float64, device="cuda"),
+                            torch.zeros((2, 32, 32, 16), dtype=torch.float64, device="cuda"))
     finally:
         fd.fd_mg_destroy(mg)
 

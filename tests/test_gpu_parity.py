@@ -855,6 +855,32 @@ def test_binding_rejects_arrays_that_do_not_match_the_plan(fd):
                 fd.fd_apply_hamiltonian(plan, bad_psi, bad_v, bad_out)
         with pytest.raises(ValueError):
             fd.fd_apply_kinetic(plan, good, good.cpu())
+        # eps / norm of fd_residual, coef / out of fd_paw_expect
+        eps = torch.ones(2, dtype=torch.float64, device="cuda")
+        r = torch.empty_like(good)
+        fd.fd_residual(plan, good, good.clone(), eps, eps.clone(), r)
+        for bad_eps in (torch.ones(3, dtype=torch.float64, device="cuda"), eps.to(torch.float32), eps.cpu()):
+            with pytest.raises(ValueError):
+                fd.fd_residual(plan, good, good.clone(), bad_eps, eps, r)
+            with pytest.raises(ValueError):
+                fd.fd_residual(plan, good, good.clone(), eps, bad_eps, r)
+        pw = fd.fd_paw_create(plan, [[0, 0, 0]], [[2, 2, 2]], [3], np.ones(24), np.eye(3).ravel())
+        try:
+            coef = torch.zeros((2, 3), dtype=torch.float64, device="cuda")
+            fd.fd_paw_expect(plan, pw, 0, coef, eps)
+            for bad_coef in (coef[:, :2].contiguous(), coef.to(torch.complex128), coef.cpu()):
+                with pytest.raises(ValueError):
+                    fd.fd_paw_expect(plan, pw, 0, bad_coef, eps)
+            with pytest.raises(ValueError):
+                fd.fd_paw_expect(plan, pw, 0, coef, eps.cpu())
+        finally:
+            fd.fd_paw_destroy(pw)
+        # a destroyed plan's cached description must not leak to a new plan at the same address
+        for shape in [(8, 8, 8), (8, 8, 16), (16, 8, 8)] * 3:
+            p2 = fd.fd_create(shape, (0.4,) * 3)
+            x = torch.zeros((1,) + shape, dtype=torch.float64, device="cuda")
+            fd.fd_apply_kinetic(p2, x, torch.empty_like(x))
+            fd.fd_destroy(p2)
         torch.cuda.synchronize()
     finally:
         fd.fd_destroy(plan)
