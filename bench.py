@@ -301,6 +301,43 @@ def parity_after_timing(torch, fd, cfg, plan, d_psi, d_v, v_host, h_psi, per_ban
             "tolerance": "1e-12 (max|psi| S + max|v_eff psi|), S = abs row sum of T"}
 
 
+def sampled_parity(torch, fd, shape, h, nn, bc, k, plan, x_dev, v_host, y_dev, rel=1e-12, per_band=8,
+                   seed=0):
+    """max|d| / tol over sampled points of EVERY band of y_dev = H x_dev (already computed by the timed
+    launches) against the oracle's point evaluation on the same inputs brought back to the host (in
+    float64; single-precision inputs are converted exactly).  tol = rel (max|x| S + max|v x|) with S
+    the absolute row sum of the plan's own weights; rel = 1e-12 (north_star) or 2e-6 (fp32, DESIGN.md
+    R18).  k given for a real x: the complex definition on the real input, real part compared."""
+    import numpy as np
+    from oracle import fd_oracle
+    w = fd.fd_plan_get_weights(plan, nn)
+    S = sum(abs(r[0]) + 2.0 * sum(abs(t) for t in r[1:]) for r in w)
+    rng = np.random.default_rng(seed + 29)
+    nbands, worst, npts, chunk = x_dev.shape[0], 0.0, 0, 16
+    for b0 in range(0, nbands, chunk):
+        nb = min(chunk, nbands - b0)
+        xc = x_dev[b0:b0 + nb]
+        xc = xc.to(torch.complex128 if xc.is_complex() else torch.float64).cpu().numpy()
+        p = np.stack([rng.integers(0, n, nb * per_band) for n in shape], axis=1)
+        edge = rng.integers(0, 3, size=p.shape) == 0
+        lohi = np.where(rng.integers(0, 2, size=p.shape) == 0, rng.integers(0, 4, size=p.shape),
+                        np.array(shape)[None, :] - 1 - rng.integers(0, 4, size=p.shape))
+        p = np.where(edge, lohi, p)
+        pts = np.concatenate([np.repeat(np.arange(nb), per_band)[:, None], p], axis=1).astype(np.int64)
+        real_at_k = k is not None and not np.iscomplexobj(xc)
+        want = fd_oracle.points(shape, h, nn, bc, k, xc.astype(np.complex128) if real_at_k else xc,
+                                v_host, pts)
+        if real_at_k:
+            want = want.real
+        idx = torch.from_numpy(pts).cuda()
+        got = y_dev[idx[:, 0] + b0, idx[:, 1], idx[:, 2], idx[:, 3]]
+        got = got.to(torch.complex128 if got.is_complex() else torch.float64).cpu().numpy()
+        tol = rel * (float(np.abs(xc).max()) * S + float(np.abs(v_host[None] * xc).max()))
+        worst = max(worst, float(np.max(np.abs(got - want))) / tol)
+        npts += pts.shape[0]
+    return {"max_err_over_tol": worst, "ok": bool(worst <= 1.0), "points": npts, "rel_tol": rel}
+
+
 def hardware_peaks(torch, fd, stream, local):
     """read-only / write-only / copy bandwidth with float64 vectors and the
     dependent-free DFMA rate, measured here with the library's own micro-benchmark kernels (2 GiB
@@ -403,8 +440,12 @@ def next_rows(torch, W, fd, cfg, plan, d_psi, d_v, d_out, stream, plain_ms, peak
         y = torch.empty_like(x)
         ms = _time_stream(torch, stream, lambda: fd.fd_apply_hamiltonian(pl, x, vv, y, stream), 20, 3)
         nbytes = 2 * x.numel() * x.element_size() + vv.numel() * vv.element_size()
+        # the timed launches left y = H x: sampled points of every band against the oracle
+        par = sampled_parity(torch, fd, cfg.shape, cfg.h, nn_, cfg.bc, kk, pl, x,
+                             vv.to(torch.float64).cpu().numpy(), y, rel=2e-6 if dt == "f32" else 1e-12,
+                             seed=cfg.seed + nn_)
         rows[tag] = entry(ms, nbytes, Gpoint_band_per_s=nb * P / (ms * 1e-3) / 1e9,
-                          kernel=_kernel_name(fd, pl, nb),
+                          kernel=_kernel_name(fd, pl, nb), parity=par,
                           what="H psi, nn = %d, %s%s" % (nn_, "fp32" if dt else "fp64",
                                                         ", float64 at k = (1/2,1/2,1/2)" if kvec else ""))
         fd.fd_destroy(pl)
@@ -421,8 +462,26 @@ def next_rows(torch, W, fd, cfg, plan, d_psi, d_v, d_out, stream, plain_ms, peak
                                     what="128 atoms, %d projector functions, %d box points: gather psi, "
                                          "read-modify-write out over the boxes" % (paw.ntot, box_pts))
     ms = _time_stream(torch, stream, lambda: fd.fd_apply_hamiltonian_paw(plan, pw, d_psi, d_v, d_out, coef, stream), 10, 2)
+    # the timed launches left d_out = H~ psi~: two whole bands against the oracle (stencil + v_eff +
+    # non-local term), point by point within 1e-12 x (north_star bound + sum of |terms| of the PAW sum)
+    from oracle import fd_oracle
+    kk = cfg.k if cfg.complex else None
+    sel = sorted({0, nb - 1})
+    xs = d_psi[sel].cpu().numpy()
+    v_host = d_v.cpu().numpy()
+    want = fd_oracle.apply(cfg.shape, cfg.h, cfg.nn, cfg.bc, kk, xs, v_host)
+    want = fd_oracle.paw_apply(cfg.shape, cfg.h, cfg.bc, kk, xs, paw.box_start, paw.box_size, paw.nproj,
+                               paw.proj, paw.dmat, out=want)
+    bound = fd_oracle.paw_apply(cfg.shape, cfg.h, cfg.bc, None, np.abs(xs), paw.box_start, paw.box_size,
+                                paw.nproj, np.abs(paw.proj), np.abs(paw.dmat))
+    wts = fd.fd_plan_get_weights(plan, cfg.nn)
+    S = sum(abs(r[0]) + 2.0 * sum(abs(t) for t in r[1:]) for r in wts)
+    tol = 1e-12 * (float(np.abs(xs).max()) * S + float(np.abs(v_host[None] * xs).max()) + bound)
+    worst = float(np.max(np.abs(d_out[sel].cpu().numpy() - want) / tol))
     rows["f4_full_paw_hamiltonian"] = entry(ms, cfg.min_bytes + 3 * box_pts * E * nb + paw.proj.size * 8,
-                                            what="Eq. 6 complete: stencil + v_eff + non-local term")
+                                            what="Eq. 6 complete: stencil + v_eff + non-local term",
+                                            parity={"max_err_over_tol": worst, "ok": bool(worst <= 1.0),
+                                                    "bands": sel, "points": int(want.size)})
     fd.fd_paw_destroy(pw)
     return rows
 

@@ -123,10 +123,13 @@ FD_API int fd_apply_kinetic(const fd_plan *plan, const void *psi, void *out, int
 /*
  * fd_apply_hamiltonian -- out = T psi + v_eff psi (adds step a4: the local potential of Eq. 6,
  * one real array shared by all bands).
- *   v_eff      device pointer, double [nx,ny,nz], 16-byte aligned
+ *   v_eff      device pointer, [nx,ny,nz] of the plan's REAL type -- double for FD_F64 / FD_C128
+ *              plans, float for FD_F32 / FD_C64 plans (hence const void *: a single-precision
+ *              caller passes its float array without a cast through the wrong type) -- 16-byte
+ *              aligned
  * Other arguments and errors as fd_apply_kinetic.
  */
-FD_API int fd_apply_hamiltonian(const fd_plan *plan, const void *psi, const double *v_eff, void *out,
+FD_API int fd_apply_hamiltonian(const fd_plan *plan, const void *psi, const void *v_eff, void *out,
                          int64_t nbands, void *cuda_stream);
 
 /*

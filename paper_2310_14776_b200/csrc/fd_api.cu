@@ -246,9 +246,11 @@ int fd_apply_kinetic(const fd_plan *plan, const void *psi, void *out, int64_t nb
                         (cudaStream_t)cuda_stream);
 }
 
-int fd_apply_hamiltonian(const fd_plan *plan, const void *psi, const double *v_eff, void *out,
+int fd_apply_hamiltonian(const fd_plan *plan, const void *psi, const void *v_eff_any, void *out,
                          int64_t nbands, void *cuda_stream)
 {
+    // float for single-precision plans (the kernels reinterpret it), double otherwise
+    const double *v_eff = static_cast<const double *>(v_eff_any);
     const int rc = check_apply_args(plan, psi, v_eff, true, out, nbands);
     if (rc != FD_OK || nbands == 0) return rc;
     return apply_device(plan, plan->g, 1, psi, v_eff, out, nbands, nullptr, nullptr, nullptr,

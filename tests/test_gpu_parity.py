@@ -84,8 +84,9 @@ def test_small_configs_full_compare(oracle, fd, idx, kernel):
         assert used == forced
 
 
-def _big_config_check(oracle, fd, cfg, full_bands, chunk=32, nsample=4000):
-    """All bands on the GPU in one apply; oracle on `full_bands` in full + sampled points."""
+def _big_config_check(oracle, fd, cfg, chunk=32):
+    """All bands on the GPU in one apply (the launch configuration bench.py times); the oracle on
+    every band, element by element."""
     plan = fd.fd_create(cfg.shape, cfg.h, cfg.nn, cfg.bc, cfg.k if cfg.complex else None,
                         fd.FD_C128 if cfg.complex else fd.FD_F64, 0)
     try:
@@ -102,49 +103,33 @@ def _big_config_check(oracle, fd, cfg, full_bands, chunk=32, nsample=4000):
         torch.cuda.synchronize()
         assert bool(torch.isfinite(torch.view_as_real(d_out) if cfg.complex else d_out).all())
         k = cfg.k if cfg.complex else None
-        # (1) full bands
-        psi_f = W.make_psi(cfg, full_bands)
-        want = oracle.apply(cfg.shape, cfg.h, cfg.nn, cfg.bc, k, psi_f, v)
-        got = d_out[list(full_bands)].cpu().numpy()
-        tol = parity_tol(cfg.h, cfg.nn, psi_f, v)
-        err = float(np.max(np.abs(got - want)))
-        assert err <= tol, f"{cfg.name}: max|d|={err:.3e} > tol={tol:.3e}"
-        # (2) sampled points of every band, biased towards faces / tile seams
-        rng = np.random.default_rng(cfg.seed)
-        per_band = max(4, nsample // cfg.nbands)
+        # EVERY element of EVERY band against the oracle (OpenMP over bands on the host cores), in
+        # chunks of `chunk` bands
+        worst = 0.0
         for b0 in range(0, cfg.nbands, chunk):
             bands = list(range(b0, min(cfg.nbands, b0 + chunk)))
             psi_c = W.make_psi(cfg, bands)
-            pts = []
-            for lb in range(len(bands)):
-                p = np.stack([rng.integers(0, n, per_band) for n in cfg.shape], axis=1)
-                edge = rng.integers(0, 2, size=p.shape).astype(bool)
-                lohi = np.where(rng.integers(0, 2, size=p.shape) == 0,
-                                rng.integers(0, 4, size=p.shape),
-                                np.array(cfg.shape)[None, :] - 1 - rng.integers(0, 4, size=p.shape))
-                p = np.where(edge, lohi, p)
-                pts.append(np.concatenate([np.full((per_band, 1), lb), p], axis=1))
-            pts = np.concatenate(pts).astype(np.int64)
-            want_p = oracle.points(cfg.shape, cfg.h, cfg.nn, cfg.bc, k, psi_c, v, pts)
-            idx = torch.from_numpy(pts).cuda()
-            got_p = d_out[idx[:, 0] + b0, idx[:, 1], idx[:, 2], idx[:, 3]].cpu().numpy()
+            want = oracle.apply(cfg.shape, cfg.h, cfg.nn, cfg.bc, k, psi_c, v)
+            got = d_out[b0:b0 + len(bands)].cpu().numpy()
             tol = parity_tol(cfg.h, cfg.nn, psi_c, v)
-            err = float(np.max(np.abs(got_p - want_p)))
-            assert err <= tol, f"{cfg.name} bands {b0}..: sampled max|d|={err:.3e} > {tol:.3e}"
+            err = float(np.max(np.abs(got - want)))
+            assert err <= tol, f"{cfg.name} bands {b0}..: max|d|={err:.3e} > tol={tol:.3e}"
+            worst = max(worst, err / tol)
+        print(f"{cfg.name}: every element of {cfg.nbands} bands, max|d|/tol = {worst:.3e}")
     finally:
         fd.fd_destroy(plan)
 
 
 def test_config3_96c_256_bands(oracle, fd):
-    _big_config_check(oracle, fd, W.get(3), [0, 1, 100, 127, 128, 254, 255, 37])
+    _big_config_check(oracle, fd, W.get(3))
 
 
 def test_config4_bloch_c128_128_bands(oracle, fd):
-    _big_config_check(oracle, fd, W.get(4), [0, 1, 63, 64, 126, 127])
+    _big_config_check(oracle, fd, W.get(4))
 
 
 def test_config5_slab_384_bands(oracle, fd):
-    _big_config_check(oracle, fd, W.get(5), [0, 191, 383], nsample=3000)
+    _big_config_check(oracle, fd, W.get(5))
 
 
 # ------------------------------------------------------------------------------ shape sweep (M8)
