@@ -25,6 +25,17 @@ int main(void)
     if (fd_paw_nproj_total(NULL) != FD_ERR_INVALID) return 7;
     if (fd_destroy(NULL) != FD_OK || fd_paw_destroy(NULL) != FD_OK || fd_workspace_destroy(NULL) != FD_OK)
         return 8;
+    /* the no-allocation entry point: usable from C, its limit is a compile-time constant, its own
+     * status code has a message; a single-precision caller passes float * as v_eff without a cast */
+    if (fd_apply_hamiltonian_expect_static(NULL, NULL, NULL, NULL, NULL, NULL, 1, NULL) != FD_ERR_INVALID)
+        return 12;
+    if (FD_STATIC_SCRATCH_BYTES != 4 * 1024 * 1024 || !strstr(fd_strerror(FD_ERR_SCRATCH), "scratch"))
+        return 13;
+    {
+        const float *v32 = NULL;
+        if (fd_apply_hamiltonian(NULL, NULL, v32, NULL, 1, NULL) != FD_ERR_INVALID) return 14;
+    }
+    if (fd_mg_get_info(NULL, NULL) != FD_ERR_INVALID) return 15;
     rc = fd_create(&plan, shape, h, 3, bc, NULL, FD_C128, 0);
     if (rc == FD_OK) {
         if (fd_plan_get_info(plan, info) != FD_OK || info[0] != 8 || info[3] != 3 || info[4] != FD_C128)
